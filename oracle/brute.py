@@ -1,0 +1,76 @@
+"""Brute-force checker for the C oracle: numpy, one window at a time.
+
+TEST INFRASTRUCTURE, NOT PRODUCT.  Written separately from umi_oracle.c (it
+does not load it) so that the two can be compared: full `np.sort` for the
+median, boolean masks for the one-sided scale, and direct weighted means with
+`np.average`.  Pure-Python loops over positions: only for small cases.
+
+Follows PAPER.md section 2 (lines 35-63) and the readings R1..R18 in DESIGN.md.
+"""
+import numpy as np
+
+SCALE_CONST = 0.6745
+
+
+def bisquare_weights(u, alpha):
+    """PAPER.md:56-58 (Eq. 2-3) on an array of standardized residuals."""
+    u = np.asarray(u, dtype=np.float64)
+    u_eff = np.where(u < 0.0, alpha * u, u)
+    inside = np.abs(u_eff) < 1.0
+    return np.where(inside, (1.0 - u_eff ** 2) ** 2, 0.0)
+
+
+def window_samples(flux_row, i, W, time_row=None):
+    """Valid samples of the centred window [i-h, i+h] clipped to the series (R1-R3)."""
+    N = len(flux_row)
+    h = (W - 1) // 2
+    lo, hi = max(0, i - h), min(N, i + h + 1)
+    x = np.asarray(flux_row[lo:hi], dtype=np.float64)
+    ok = np.isfinite(x)
+    if time_row is not None:
+        ok &= np.isfinite(np.asarray(time_row[lo:hi], dtype=np.float64))
+    return x[ok]
+
+
+def location(x, alpha=2.0, c=5.0, n_iter=5, history=False):
+    """UMI location of the 1-D sample x (all valid).  Returns (mu, median, s)."""
+    x = np.asarray(x, dtype=np.float64)
+    n = x.size
+    med = np.sort(x)[(n - 1) // 2]                      # PAPER.md:39; lower median (R6)
+    upper = x[x > med]                                  # Eq. 1, strict (R7)
+    if upper.size == 0:
+        return (med, med, 0.0) if not history else (med, med, 0.0, [])
+    s = SCALE_CONST * np.sqrt(np.mean((upper - med) ** 2))
+    if not s > 0.0:
+        return (med, med, s) if not history else (med, med, s, [])
+    mu = med
+    trace = []
+    for _ in range(n_iter):
+        w = bisquare_weights((x - mu) / (c * s), alpha)
+        if not w.sum() > 0.0:
+            break
+        mu = np.average(x, weights=w)                   # Eq. 4
+        trace.append(mu)
+    return (mu, med, s) if not history else (mu, med, s, trace)
+
+
+def detrend(flux, W, alpha=2.0, n_iter=5, c=5.0, time=None, min_valid=None):
+    """Brute-force trend, median and scale for a [S, N] (or [N]) array."""
+    flux = np.atleast_2d(np.asarray(flux, dtype=np.float32))
+    if time is not None:
+        time = np.atleast_2d(np.asarray(time, dtype=np.float64))
+    S, N = flux.shape
+    if min_valid is None:
+        min_valid = max(1, W // 3)                      # PAPER.md:192 (R4)
+    trend = np.full((S, N), np.nan)
+    median = np.full((S, N), np.nan)
+    scale = np.full((S, N), np.nan)
+    for b in range(S):
+        trow = None if time is None else time[b]
+        for i in range(N):
+            own_ok = np.isfinite(flux[b, i]) and (trow is None or np.isfinite(trow[i]))
+            x = window_samples(flux[b], i, W, trow)
+            if not own_ok or x.size < min_valid:        # (R4, R5)
+                continue
+            trend[b, i], median[b, i], scale[b, i] = location(x, alpha, c, n_iter)
+    return trend, median, scale

@@ -1,0 +1,259 @@
+/*
+ * umi_oracle.c -- fp64 CPU oracle for the UMI sliding-window estimator.
+ *
+ * TEST INFRASTRUCTURE, NOT PRODUCT.  Only tests/, __graft_entry__.smoke() and
+ * bench.py's cpu_baseline / --impl reference legs may build, load or call this
+ * file.  It shares no code, header, table or helper with the CUDA path under
+ * paper_2604_06602_b200/csrc/ and neither includes the other.
+ *
+ * What it is: the algorithm of PAPER.md section 2 written out per window, step
+ * by step, in the paper's order and notation, in double precision, with no
+ * sliding trick, no blocking and no fusion:
+ *   window rule        PAPER.md:35   W = floor(0.5/dt) | 1
+ *   Phase 1 median     PAPER.md:39   exact sample median (here: full sort, pick rank)
+ *   Phase 2 upper-RMS  PAPER.md:43-48 (Eq. 1), s = 0.6745 * sigma_upper
+ *   Phase 3 iterations PAPER.md:54-63 (Eq. 2-4), c = 5, alpha = 2, 5 passes
+ *   minimum length     PAPER.md:192  W/3
+ * Where the paper is silent the readings R1..R18 of DESIGN.md ("Readings of the
+ * paper") are taken; each is marked (Rn) at the line that implements it.
+ *
+ * Pins (tests/test_oracle_*.py, all -m "not gpu"): the paper-printed window
+ * lengths and weight values, a hand-computed worked example, an independent
+ * numpy brute force (oracle/brute.py), numpy/scipy median and mean routines,
+ * the Gaussian closed forms, and the invariants listed in DESIGN.md.
+ * Parity unpinned: none of the functions below; the paper's real-data accuracy
+ * tables are out of scope and are not reproduced.
+ *
+ * Build: gcc -O2 -fopenmp -shared -fPIC (no -ffast-math), see oracle/build.py.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define UMI_ORACLE_SCALE_CONST 0.6745
+
+/* W = floor(0.5/dt) | 1, dt in days.
+ * (R15) the quotient is nudged up by 2^-20 relative before the floor so that a
+ * cadence that passed through fp32 (0.5/dt = 359.99999) still gives the
+ * paper's 361.  Returns 0 for dt <= 0 or non-finite. */
+int umi_oracle_window_len(double dt_days)
+{
+    if (!(dt_days > 0.0) || !isfinite(dt_days)) return 0;
+    double q = (0.5 / dt_days) * (1.0 + ldexp(1.0, -20));
+    if (!(q < 2147483646.0)) return 0;
+    int w = (int)floor(q);
+    return w | 1;
+}
+
+/* PAPER.md:56-58, Eq. 2 and Eq. 3: weight of a standardized residual u. */
+double umi_oracle_weight(double u, double alpha)
+{
+    double ueff = (u < 0.0) ? alpha * u : u;          /* Eq. 2 (R13: u < 0) */
+    if (fabs(ueff) < 1.0) {                            /* Eq. 3 (R12: strict) */
+        double t = 1.0 - ueff * ueff;
+        return t * t;
+    }
+    return 0.0;
+}
+
+static int cmp_double(const void *a, const void *b)
+{
+    double x = *(const double *)a, y = *(const double *)b;
+    return (x > y) - (x < y);
+}
+
+/* (R3, R16) a slot is valid iff it is inside the series, its flux is finite
+ * and, when a time array is given, its time stamp is finite. */
+static int slot_valid(const double *time, const float *flux, int64_t N, int64_t j)
+{
+    if (j < 0 || j >= N) return 0;                    /* (R2) edges truncate */
+    if (!isfinite(flux[j])) return 0;
+    if (time && !isfinite(time[j])) return 0;
+    return 1;
+}
+
+/*
+ * One window: star row (time, flux) of length N, position i.
+ * Outputs (any may be NULL): trend (double), median (float), scale s, n valid,
+ * n_plus, near_cutoff flag.  work[] must hold 2*W doubles.
+ * Returns 1 if a trend value was produced, 0 if the output is NaN.
+ */
+static int oracle_window(const double *time, const float *flux, int64_t N, int64_t i,
+                         int W, double alpha, double c, int n_iter, int min_valid,
+                         double cutoff_tol, double *work,
+                         double *trend, float *median, double *scale,
+                         int32_t *n_valid, int32_t *n_plus_out, uint8_t *near_cutoff)
+{
+    const int64_t h = (W - 1) / 2;                    /* (R1) centred window [i-h, i+h] */
+    double *x = work, *sorted = work + W;
+    int n = 0;
+    for (int64_t j = i - h; j <= i + h; ++j)
+        if (slot_valid(time, flux, N, j)) x[n++] = (double)flux[j];   /* exact widening */
+
+    if (trend) *trend = NAN;
+    if (median) *median = NAN;
+    if (scale) *scale = NAN;
+    if (n_valid) *n_valid = n;
+    if (n_plus_out) *n_plus_out = 0;
+    if (near_cutoff) *near_cutoff = 0;
+
+    /* (R4) PAPER.md:192 minimum length W/3; (R5) invalid own slot -> NaN */
+    if (!slot_valid(time, flux, N, i) || n < min_valid) return 0;
+
+    /* Phase 1: the exact sample median.  Definition written out:
+     * sort ascending, take rank k = (n-1)/2 (R6: lower middle when n is even). */
+    memcpy(sorted, x, (size_t)n * sizeof(double));
+    qsort(sorted, (size_t)n, sizeof(double), cmp_double);
+    const double med = sorted[(n - 1) / 2];
+    if (median) *median = (float)med;                 /* a selected fp32 sample: exact */
+
+    /* Phase 2, Eq. 1: RMS of residuals strictly above the median (R7). */
+    int n_plus = 0;
+    double ss = 0.0;
+    for (int j = 0; j < n; ++j)
+        if (x[j] > med) { double r = x[j] - med; ss += r * r; ++n_plus; }
+    if (n_plus_out) *n_plus_out = n_plus;
+    if (n_plus == 0) {                                /* (R8) */
+        if (trend) *trend = med;
+        if (scale) *scale = 0.0;
+        return 1;
+    }
+    const double sigma_upper = sqrt(ss / (double)n_plus);
+    const double s = UMI_ORACLE_SCALE_CONST * sigma_upper;
+    if (scale) *scale = s;
+    if (!(s > 0.0)) {                                 /* (R8) */
+        if (trend) *trend = med;
+        return 1;
+    }
+
+    /* Phase 3: n_iter passes of Eq. 2-4, s held fixed (R9),
+     * no convergence test (R10). */
+    double mu = med;
+    int flagged = 0;
+    for (int it = 0; it < n_iter; ++it) {
+        double sw = 0.0, swx = 0.0;
+        for (int j = 0; j < n; ++j) {
+            double u = (x[j] - mu) / (c * s);
+            double ueff = (u < 0.0) ? alpha * u : u;  /* Eq. 2 */
+            double w;
+            if (fabs(ueff) < 1.0) { double t = 1.0 - ueff * ueff; w = t * t; }   /* Eq. 3 */
+            else w = 0.0;
+            if (fabs(fabs(ueff) - 1.0) <= cutoff_tol) flagged = 1;
+            sw += w;
+            swx += w * x[j];
+        }
+        if (!(sw > 0.0)) break;                       /* (R11) */
+        mu = swx / sw;                                /* Eq. 4 */
+    }
+    if (trend) *trend = mu;
+    if (near_cutoff) *near_cutoff = (uint8_t)flagged;
+    return 1;
+}
+
+static int resolve_min_valid(int W, int min_valid)
+{
+    if (min_valid >= 0) return min_valid;
+    int m = W / 3;                                    /* (R4) PAPER.md:192 */
+    return m < 1 ? 1 : m;
+}
+
+/*
+ * Evaluate a list of (star, position) pairs.  flux is [n_stars, n_cadences]
+ * row-major fp32; time is NULL or the same shape in fp64.
+ * min_valid < 0 selects the default max(1, W/3).
+ * Every output array has `count` entries and may be NULL.
+ * Returns 0 on success, 1 on invalid arguments.
+ */
+int umi_oracle_positions(const double *time, const float *flux,
+                         int64_t n_stars, int64_t n_cadences,
+                         const int64_t *star_idx, const int64_t *pos_idx, int64_t count,
+                         int W, double alpha, double c, int n_iter, int min_valid,
+                         double cutoff_tol,
+                         double *trend64, float *trend32, float *median,
+                         double *scale, int32_t *n_valid, int32_t *n_plus,
+                         uint8_t *near_cutoff)
+{
+    if (!flux || n_stars < 0 || n_cadences < 0 || W < 1 || (W & 1) == 0 || n_iter < 0 ||
+        !(alpha > 0.0) || !(c > 0.0) || count < 0)
+        return 1;
+    const int mv = resolve_min_valid(W, min_valid);
+    int bad = 0;
+#pragma omp parallel
+    {
+        double *work = (double *)malloc((size_t)2 * (size_t)W * sizeof(double));
+#pragma omp for schedule(dynamic, 256)
+        for (int64_t q = 0; q < count; ++q) {
+            int64_t b = star_idx[q], i = pos_idx[q];
+            if (!work || b < 0 || b >= n_stars || i < 0 || i >= n_cadences) {
+#pragma omp atomic write
+                bad = 1;
+                continue;
+            }
+            const float *frow = flux + b * n_cadences;
+            const double *trow = time ? time + b * n_cadences : NULL;
+            double t64;
+            oracle_window(trow, frow, n_cadences, i, W, alpha, c, n_iter, mv, cutoff_tol, work,
+                          &t64, median ? median + q : NULL, scale ? scale + q : NULL,
+                          n_valid ? n_valid + q : NULL, n_plus ? n_plus + q : NULL,
+                          near_cutoff ? near_cutoff + q : NULL);
+            if (trend64) trend64[q] = t64;
+            if (trend32) trend32[q] = (float)t64;     /* round-to-nearest-even */
+        }
+        free(work);
+    }
+    return bad;
+}
+
+/* Every position of every star, in [n_stars, n_cadences] order. */
+int umi_oracle_detrend(const double *time, const float *flux,
+                       int64_t n_stars, int64_t n_cadences,
+                       int W, double alpha, double c, int n_iter, int min_valid,
+                       double cutoff_tol,
+                       double *trend64, float *trend32, float *median,
+                       double *scale, int32_t *n_valid, int32_t *n_plus,
+                       uint8_t *near_cutoff)
+{
+    if (!flux || n_stars < 0 || n_cadences < 0 || W < 1 || (W & 1) == 0 || n_iter < 0 ||
+        !(alpha > 0.0) || !(c > 0.0))
+        return 1;
+    const int mv = resolve_min_valid(W, min_valid);
+    const int64_t total = n_stars * n_cadences;
+    int bad = 0;
+#pragma omp parallel
+    {
+        double *work = (double *)malloc((size_t)2 * (size_t)W * sizeof(double));
+#pragma omp for schedule(dynamic, 256)
+        for (int64_t q = 0; q < total; ++q) {
+            if (!work) {
+#pragma omp atomic write
+                bad = 1;
+                continue;
+            }
+            int64_t b = q / n_cadences, i = q % n_cadences;
+            const float *frow = flux + b * n_cadences;
+            const double *trow = time ? time + b * n_cadences : NULL;
+            double t64;
+            oracle_window(trow, frow, n_cadences, i, W, alpha, c, n_iter, mv, cutoff_tol, work,
+                          &t64, median ? median + q : NULL, scale ? scale + q : NULL,
+                          n_valid ? n_valid + q : NULL, n_plus ? n_plus + q : NULL,
+                          near_cutoff ? near_cutoff + q : NULL);
+            if (trend64) trend64[q] = t64;
+            if (trend32) trend32[q] = (float)t64;
+        }
+        free(work);
+    }
+    return bad;
+}
+
+int umi_oracle_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
