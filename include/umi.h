@@ -1,0 +1,133 @@
+/*
+ * umi.h -- C ABI of the B200 (sm_100a) UMI sliding-window detrender.
+ *
+ * UMI = the sliding-window asymmetric robust location estimator of
+ * arxiv/paper_2604_06602, section 2 (lines 33-63):
+ *   window rule   PAPER.md:35     W = floor(0.5/dt) | 1
+ *   Phase 1       PAPER.md:37-39  exact sample median of the window
+ *   Phase 2       PAPER.md:41-50  upper-RMS scale, Eq. 1, s = 0.6745 * sigma_upper
+ *   Phase 3       PAPER.md:52-63  n_iter asymmetric Tukey-bisquare passes, Eq. 2-4, c = 5
+ *   min. length   PAPER.md:192    fewer than max(1, W/3) valid samples -> NaN
+ * Readings of everything the paper leaves open (edges, gaps, even counts,
+ * ties, degenerate scale): DESIGN.md, "Readings of the paper", R1..R18.
+ *
+ * Conventions
+ *  - Every entry point returns a umi_status (int); nothing throws or aborts
+ *    across this boundary.  Arguments are validated on the host before any
+ *    work is enqueued.
+ *  - No torch types, no hidden allocation that outlives a call, no mutable
+ *    global state: the library is re-entrant.
+ *  - "DEVICE pointer": memory of the current CUDA device, readable/writable by
+ *    kernels launched on `stream`.  "HOST pointer": ordinary host memory
+ *    (pinned memory makes the copies asynchronous and faster, but is not
+ *    required).
+ *  - Layout: [n_stars, n_cadences] row-major, contiguous, row stride
+ *    n_cadences elements, 64-bit indexing.
+ *  - Invalid sample: flux not finite (NaN, +Inf, -Inf), or time given and not
+ *    finite.  Invalid samples and slots outside [0, n_cadences) are skipped by
+ *    every window (R2, R3, R16).
+ *  - Supported dynamic range: within one tile of ~512 consecutive cadences,
+ *    (max - min) * 8 * max(1, 1/alpha) must be finite in fp32.
+ */
+#ifndef UMI_B200_H
+#define UMI_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    UMI_OK = 0,
+    UMI_ERR_INVALID_ARG = 1, /* null pointer, negative size, even or < 1 W, alpha/c not finite or <= 0, n_iter < 0 */
+    UMI_ERR_UNSUPPORTED = 2, /* W > UMI_MAX_WINDOW */
+    UMI_ERR_CUDA = 3         /* launch / copy / allocation failure (the CUDA error is cleared) */
+} umi_status;
+
+/* Largest window the compiled kernels accept (TESS 20 s needs 2161). */
+#define UMI_MAX_WINDOW 4097
+
+/*
+ * Window rule: W = floor(0.5/dt) | 1, dt = cadence in days.
+ * (R15) the quotient is multiplied by (1 + 2^-20) before the floor so that a
+ * cadence that passed through fp32 (0.5/dt = 359.99999) still gives 361.
+ * Host only.  Returns W (odd, >= 1), or 0 if dt <= 0, non-finite, or W would
+ * not fit an int.
+ */
+int umi_window_len(double dt_days);
+
+/*
+ * The hot path: trend_out[b, i] = UMI location of the centred window
+ * [i-h, i+h], h = (W-1)/2, of star b, for every b and i.
+ *
+ *   time      DEVICE, const double [n_stars*n_cadences], or NULL.  Only
+ *             finiteness is used: a non-finite time marks the cadence invalid.
+ *   flux      DEVICE, const float [n_stars*n_cadences].
+ *   n_stars, n_cadences   >= 0; either 0 -> UMI_OK, nothing enqueued.
+ *   W         odd, 1 <= W <= UMI_MAX_WINDOW; may exceed n_cadences (clipped).
+ *   alpha     asymmetry factor of Eq. 2 (2 = TESS default, 1 = symmetric); finite, > 0.
+ *   n_iter    number of Eq. 2-4 passes (paper: 5); 0 returns the Phase-1
+ *             median, bit-exact (it is a selected input sample; -0.0 reads as +0.0).
+ *   trend_out DEVICE, float [n_stars*n_cadences]; must not overlap flux/time.
+ *             NaN where the cadence itself is invalid or its window holds
+ *             fewer than max(1, W/3) valid samples (R4, R5).  Also used as
+ *             scratch between the two kernels of the call.
+ *   stream    cudaStream_t (as void*), or NULL for the legacy default stream.
+ *             Work is enqueued; the call does not synchronise.  The caller
+ *             keeps all three buffers alive until the stream has drained.
+ *
+ * c is fixed at 5.0.  Errors: see umi_status.
+ */
+int umi_detrend(const double* time, const float* flux,
+                int64_t n_stars, int64_t n_cadences,
+                int W, float alpha, int n_iter,
+                float* trend_out, void* stream);
+
+/*
+ * Same path with the remaining parameters of PAPER.md Table 4 (lines 202-209)
+ * exposed: tuning constant c (5.0 default, 2.5 "aggressive"; finite, > 0) and
+ * min_valid (< 0 selects max(1, W/3)).  All pointers DEVICE.
+ */
+int umi_detrend_ex(const double* time, const float* flux,
+                   int64_t n_stars, int64_t n_cadences,
+                   int W, float alpha, float c, int n_iter, int min_valid,
+                   float* trend_out, void* stream);
+
+/*
+ * Batch driver (the paper streams 50-star batches): the same
+ * computation with HOST buffers.  Stars are cut into batches of
+ * `stars_per_batch` (<= 0: chosen so that a batch is about 64 MiB of flux),
+ * and host->device copy, kernels and device->host copy of successive batches
+ * are pipelined over `n_streams` CUDA streams (<= 0: 3) with one device buffer
+ * set per stream, allocated and freed inside the call.
+ *
+ *   time, flux, trend_out   HOST pointers, same shapes as above; time may be NULL.
+ * The call returns after every batch has been copied back (it synchronises).
+ */
+int umi_detrend_host(const double* time, const float* flux,
+                     int64_t n_stars, int64_t n_cadences,
+                     int W, float alpha, int n_iter,
+                     float* trend_out,
+                     int64_t stars_per_batch, int n_streams);
+
+/*
+ * Launch geometry the library uses for this W (for reports and roofline
+ * arithmetic; host only).  Any pointer may be NULL.
+ *   median_tile    positions per CTA of the Phase-1 (median) kernel
+ *   median_sort_n  power-of-two length of the per-tile sort
+ *   weight_tile    positions per CTA of the Phase-2/3 (reweighting) kernel
+ * Returns UMI_OK, or INVALID_ARG / UNSUPPORTED for a bad W.
+ */
+int umi_launch_geometry(int W, int* median_tile, int* median_sort_n, int* weight_tile);
+
+/* Static, never-freed string for a umi_status value. */
+const char* umi_status_string(int status);
+
+/* Library version: major*10000 + minor*100 + patch. */
+int umi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* UMI_B200_H */

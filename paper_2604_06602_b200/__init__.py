@@ -1,0 +1,177 @@
+"""paper_2604_06602_b200 -- B200 (sm_100a) UMI sliding-window detrender.
+
+Thin Python binding over the C-ABI library declared in include/umi.h
+(libumi_b200.so, built by paper_2604_06602_b200/build.py).  Argument
+marshalling only: every step of the path runs in the CUDA kernels.  There is no
+CPU fallback: if the library is missing the import of any entry point raises.
+
+    W = umi_window_len(dt_days)
+    trend = umi_detrend(None, flux_cuda, W)             # PAPER.md:37-63, [S, N] fp32 CUDA tensor
+    trend = umi_detrend_host(None, flux_numpy, W)       # host buffers, streamed batches
+"""
+import ctypes
+import os
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libumi_b200.so")
+
+UMI_OK, UMI_ERR_INVALID_ARG, UMI_ERR_UNSUPPORTED, UMI_ERR_CUDA = 0, 1, 2, 3
+UMI_MAX_WINDOW = 4097
+
+EXPORTS = ("umi_window_len", "umi_detrend", "umi_detrend_ex", "umi_detrend_host",
+           "umi_launch_geometry", "umi_status_string", "umi_version")
+
+_lib = None
+
+
+class UmiError(RuntimeError):
+    def __init__(self, status, message):
+        super().__init__(message)
+        self.status = status
+
+
+def lib():
+    """The loaded C-ABI library.  Raises if it has not been built (no fallback)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(
+            "%s not found: build it with `python -m paper_2604_06602_b200.build` "
+            "(nvcc, sm_100a).  There is no CPU fallback." % LIB_PATH)
+    L = ctypes.CDLL(LIB_PATH)
+    vp, i64, ci, cf = ctypes.c_void_p, ctypes.c_int64, ctypes.c_int, ctypes.c_float
+    L.umi_window_len.restype = ci
+    L.umi_window_len.argtypes = [ctypes.c_double]
+    L.umi_detrend.restype = ci
+    L.umi_detrend.argtypes = [vp, vp, i64, i64, ci, cf, ci, vp, vp]
+    L.umi_detrend_ex.restype = ci
+    L.umi_detrend_ex.argtypes = [vp, vp, i64, i64, ci, cf, cf, ci, ci, vp, vp]
+    L.umi_detrend_host.restype = ci
+    L.umi_detrend_host.argtypes = [vp, vp, i64, i64, ci, cf, ci, vp, i64, ci]
+    L.umi_launch_geometry.restype = ci
+    L.umi_launch_geometry.argtypes = [ci] + [ctypes.POINTER(ci)] * 3
+    L.umi_status_string.restype = ctypes.c_char_p
+    L.umi_status_string.argtypes = [ci]
+    L.umi_version.restype = ci
+    L.umi_version.argtypes = []
+    _lib = L
+    return L
+
+
+def _check(status):
+    if status != UMI_OK:
+        raise UmiError(status, lib().umi_status_string(status).decode())
+
+
+def umi_status_string(status):
+    return lib().umi_status_string(int(status)).decode()
+
+
+def umi_version():
+    return int(lib().umi_version())
+
+
+def umi_window_len(dt_days):
+    """W = floor(0.5/dt) | 1; 0 for a bad dt."""
+    return int(lib().umi_window_len(float(dt_days)))
+
+
+def umi_launch_geometry(W):
+    """(median_tile, median_sort_n, weight_tile) the library uses for this W."""
+    a, b, c = ctypes.c_int(), ctypes.c_int(), ctypes.c_int()
+    _check(lib().umi_launch_geometry(int(W), ctypes.byref(a), ctypes.byref(b), ctypes.byref(c)))
+    return a.value, b.value, c.value
+
+
+def _cuda_2d(t, dtype, name):
+    import torch
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError("%s must be a CUDA torch.Tensor" % name)
+    if t.dtype != dtype:
+        raise TypeError("%s must be %s" % (name, dtype))
+    if t.dim() == 1:
+        t = t.unsqueeze(0)
+    if t.dim() != 2 or not t.is_contiguous():
+        raise ValueError("%s must be contiguous [n_stars, n_cadences]" % name)
+    return t
+
+
+def umi_detrend(time, flux, W, alpha=2.0, n_iter=5, out=None, stream=None, c=None, min_valid=None):
+    """Device path.  `flux`: CUDA fp32 [S, N] (or [N]); `time`: None or CUDA fp64 of the
+    same shape.  Enqueues on `stream` (default: torch's current stream) and returns the
+    CUDA fp32 trend tensor without synchronising.  `c` / `min_valid` route through
+    umi_detrend_ex (Table 4)."""
+    import torch
+    f = _cuda_2d(flux, torch.float32, "flux")
+    tptr = None
+    if time is not None:
+        tt = _cuda_2d(time, torch.float64, "time")
+        if tt.shape != f.shape or tt.device != f.device:
+            raise ValueError("time must have flux's shape and device")
+        tptr = tt.data_ptr()
+    if out is None:
+        out = torch.empty_like(f)
+    else:
+        out = _cuda_2d(out, torch.float32, "out")
+        if out.shape != f.shape or out.device != f.device:
+            raise ValueError("out must have flux's shape and device")
+    S, N = f.shape
+    with torch.cuda.device(f.device):
+        if stream is None:
+            stream = torch.cuda.current_stream(f.device)
+        sptr = stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+        fptr = f.data_ptr() if f.numel() else None
+        optr = out.data_ptr() if out.numel() else None
+        if S == 0 or N == 0:
+            return out.view(flux.shape)
+        if c is None and min_valid is None:
+            st = lib().umi_detrend(tptr, fptr, S, N, int(W), float(alpha), int(n_iter), optr, sptr)
+        else:
+            st = lib().umi_detrend_ex(tptr, fptr, S, N, int(W), float(alpha),
+                                      5.0 if c is None else float(c), int(n_iter),
+                                      -1 if min_valid is None else int(min_valid), optr, sptr)
+    _check(st)
+    return out.view(flux.shape)
+
+
+def umi_detrend_host(time, flux, W, alpha=2.0, n_iter=5, out=None, stars_per_batch=0, n_streams=0):
+    """Host path (batch driver).  `flux`: C-contiguous fp32 numpy array or CPU tensor
+    [S, N]; `time`: None or fp64 of the same shape; pinned memory makes the copies
+    overlap.  Returns `out` (same kind as `flux`) after all batches are back."""
+    import numpy as np
+    try:
+        import torch
+    except ImportError:  # pragma: no cover
+        torch = None
+    is_torch = torch is not None and isinstance(flux, torch.Tensor)
+
+    def as_np(a, dtype, name):
+        if torch is not None and isinstance(a, torch.Tensor):
+            if a.is_cuda:
+                raise TypeError("%s must be a host array" % name)
+            a = a.numpy()
+        if not isinstance(a, np.ndarray) or a.dtype != dtype or not a.flags.c_contiguous:
+            raise TypeError("%s must be a C-contiguous %s host array" % (name, np.dtype(dtype).name))
+        return a
+
+    f = as_np(flux, np.float32, "flux")
+    f2 = f.reshape(1, -1) if f.ndim == 1 else f
+    if f2.ndim != 2:
+        raise ValueError("flux must be [n_stars, n_cadences]")
+    tptr = None
+    if time is not None:
+        t = as_np(time, np.float64, "time")
+        if t.size != f.size:
+            raise ValueError("time must have flux's shape")
+        tptr = t.ctypes.data
+    if out is None:
+        out = torch.empty_like(flux) if is_torch else np.empty_like(f)
+    o = as_np(out, np.float32, "out")
+    if o.size != f.size:
+        raise ValueError("out must have flux's shape")
+    S, N = f2.shape
+    if S and N:
+        _check(lib().umi_detrend_host(tptr, f.ctypes.data, S, N, int(W), float(alpha), int(n_iter),
+                                      o.ctypes.data, int(stars_per_batch), int(n_streams)))
+    return out

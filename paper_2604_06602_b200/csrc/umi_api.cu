@@ -1,0 +1,235 @@
+/*
+ * umi_api.cu -- the C ABI of include/umi.h: argument validation, launch
+ * geometry, kernel launches and the host-buffer batch driver.
+ */
+#include <cuda_runtime.h>
+#include <math.h>
+#include <stdint.h>
+
+#include <algorithm>
+#include <vector>
+
+#include "umi.h"
+#include "umi_internal.h"
+
+namespace {
+
+constexpr int64_t MAX_GRID = 0x7FFFFFFF;
+
+struct Geometry {
+    int T1, NS;            /* median kernel: positions per tile, sort length */
+    size_t smem1;
+    size_t smem2;          /* reweighting kernel */
+};
+
+/* DESIGN.md, "Launch geometry": the sort length is the smallest power of two
+   (>= 1024) that leaves at least (W-1)/2 positions per tile. */
+Geometry geometry_for(int W)
+{
+    Geometry g;
+    int ns = umi::K1_MIN_SORT;
+    while (ns < (W - 1) + (W - 1) / 2) ns <<= 1;
+    g.NS = ns;
+    g.T1 = ns - (W - 1);
+    g.smem1 = (size_t)ns * umi::K1_BYTES_PER_SLOT;
+    const int h = (W - 1) / 2;
+    const int hal = (h + 3) & ~3;
+    const int G = (3 + (hal - h) + 2 * h) / 4 + 1;
+    g.smem2 = (size_t)(umi::K2_TILE + 4 * G) * sizeof(float);
+    return g;
+}
+
+int check_window(int W)
+{
+    if (W < 1 || (W & 1) == 0) return UMI_ERR_INVALID_ARG;
+    if (W > UMI_MAX_WINDOW) return UMI_ERR_UNSUPPORTED;
+    return UMI_OK;
+}
+
+int cuda_failed(cudaError_t e)
+{
+    if (e == cudaSuccess) return 0;
+    (void)cudaGetLastError(); /* clear */
+    return 1;
+}
+
+int validate(const float* flux, int64_t n_stars, int64_t n_cadences, int W, float alpha, float c,
+             int n_iter, const float* trend_out)
+{
+    if (flux == nullptr || trend_out == nullptr) return UMI_ERR_INVALID_ARG;
+    if (n_stars < 0 || n_cadences < 0 || n_iter < 0) return UMI_ERR_INVALID_ARG;
+    if (!(alpha > 0.f) || !isfinite(alpha) || !(c > 0.f) || !isfinite(c)) return UMI_ERR_INVALID_ARG;
+    return check_window(W);
+}
+
+/* Enqueue both kernels for device-resident buffers. */
+int launch_device(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
+                  int W, float alpha, float c, int n_iter, int min_valid, float* trend_out,
+                  cudaStream_t stream)
+{
+    if (n_stars == 0 || n_cadences == 0) return UMI_OK;
+    const Geometry g = geometry_for(W);
+    if (min_valid < 0) min_valid = std::max(1, W / 3);      /* PAPER.md:192 (R4) */
+
+    umi::MedianParams mp;
+    mp.time = time;
+    mp.flux = flux;
+    mp.out = trend_out;
+    mp.N = n_cadences;
+    mp.tiles_per_star = (n_cadences + g.T1 - 1) / g.T1;
+    mp.n_blocks = n_stars * mp.tiles_per_star;
+    mp.W = W;
+    mp.T = g.T1;
+    mp.NS = g.NS;
+    mp.min_valid = min_valid;
+    if (g.smem1 > 48 * 1024) {
+        if (cuda_failed(cudaFuncSetAttribute(umi::umi_median_kernel,
+                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem1)))
+            return UMI_ERR_CUDA;
+    }
+    const unsigned grid1 = (unsigned)std::min<int64_t>(mp.n_blocks, MAX_GRID);
+    umi::umi_median_kernel<<<grid1, umi::K1_THREADS, g.smem1, stream>>>(mp);
+    if (cuda_failed(cudaGetLastError())) return UMI_ERR_CUDA;
+
+    if (n_iter > 0) {
+        umi::ReweightParams rp;
+        rp.time = time;
+        rp.flux = flux;
+        rp.out = trend_out;
+        rp.N = n_cadences;
+        rp.tiles_per_star = (n_cadences + umi::K2_TILE - 1) / umi::K2_TILE;
+        rp.n_blocks = n_stars * rp.tiles_per_star;
+        rp.W = W;
+        rp.n_iter = n_iter;
+        rp.alpha = alpha;
+        rp.c = c;
+        const unsigned grid2 = (unsigned)std::min<int64_t>(rp.n_blocks, MAX_GRID);
+        umi::umi_reweight_kernel<<<grid2, umi::K2_THREADS, g.smem2, stream>>>(rp);
+        if (cuda_failed(cudaGetLastError())) return UMI_ERR_CUDA;
+    }
+    return UMI_OK;
+}
+
+} // namespace
+
+extern "C" {
+
+int umi_window_len(double dt_days)
+{
+    if (!(dt_days > 0.0) || !isfinite(dt_days)) return 0;
+    const double q = (0.5 / dt_days) * (1.0 + 1.0 / 1048576.0);     /* (R15) */
+    if (!(q < 2147483646.0)) return 0;
+    return (int)floor(q) | 1;
+}
+
+int umi_detrend_ex(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
+                   int W, float alpha, float c, int n_iter, int min_valid,
+                   float* trend_out, void* stream)
+{
+    const int st = validate(flux, n_stars, n_cadences, W, alpha, c, n_iter, trend_out);
+    if (st != UMI_OK) return st;
+    return launch_device(time, flux, n_stars, n_cadences, W, alpha, c, n_iter, min_valid, trend_out,
+                         static_cast<cudaStream_t>(stream));
+}
+
+int umi_detrend(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
+                int W, float alpha, int n_iter, float* trend_out, void* stream)
+{
+    return umi_detrend_ex(time, flux, n_stars, n_cadences, W, alpha, 5.0f /* PAPER.md:63 */, n_iter, -1,
+                          trend_out, stream);
+}
+
+int umi_detrend_host(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
+                     int W, float alpha, int n_iter, float* trend_out,
+                     int64_t stars_per_batch, int n_streams)
+{
+    const int st = validate(flux, n_stars, n_cadences, W, alpha, 5.0f, n_iter, trend_out);
+    if (st != UMI_OK) return st;
+    if (n_stars == 0 || n_cadences == 0) return UMI_OK;
+    if (n_streams <= 0) n_streams = 3;
+    if (n_streams > 16) n_streams = 16;
+    if (stars_per_batch <= 0) {
+        const int64_t row_bytes = n_cadences * (int64_t)sizeof(float);
+        stars_per_batch = std::max<int64_t>(1, (64ll << 20) / std::max<int64_t>(row_bytes, 1));
+    }
+    stars_per_batch = std::min(stars_per_batch, n_stars);
+    const int64_t n_batches = (n_stars + stars_per_batch - 1) / stars_per_batch;
+    if ((int64_t)n_streams > n_batches) n_streams = (int)n_batches;
+
+    struct Slot {
+        cudaStream_t stream = nullptr;
+        float* d_flux = nullptr;
+        float* d_trend = nullptr;
+        double* d_time = nullptr;
+    };
+    std::vector<Slot> slots((size_t)n_streams);
+    const size_t elems = (size_t)stars_per_batch * (size_t)n_cadences;
+    int status = UMI_OK;
+
+    for (auto& s : slots) {
+        if (cuda_failed(cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking)) ||
+            cuda_failed(cudaMalloc(&s.d_flux, elems * sizeof(float))) ||
+            cuda_failed(cudaMalloc(&s.d_trend, elems * sizeof(float))) ||
+            (time != nullptr && cuda_failed(cudaMalloc(&s.d_time, elems * sizeof(double))))) {
+            status = UMI_ERR_CUDA;
+            break;
+        }
+    }
+
+    for (int64_t b = 0; status == UMI_OK && b < n_batches; ++b) {
+        Slot& s = slots[(size_t)(b % n_streams)];
+        const int64_t s0 = b * stars_per_batch;
+        const int64_t ns = std::min(stars_per_batch, n_stars - s0);
+        const size_t off = (size_t)s0 * (size_t)n_cadences;
+        const size_t cnt = (size_t)ns * (size_t)n_cadences;
+        /* the slot's stream serialises reuse of its buffers */
+        if (cuda_failed(cudaMemcpyAsync(s.d_flux, flux + off, cnt * sizeof(float), cudaMemcpyHostToDevice, s.stream)) ||
+            (time != nullptr &&
+             cuda_failed(cudaMemcpyAsync(s.d_time, time + off, cnt * sizeof(double), cudaMemcpyHostToDevice, s.stream)))) {
+            status = UMI_ERR_CUDA;
+            break;
+        }
+        status = launch_device(s.d_time, s.d_flux, ns, n_cadences, W, alpha, 5.0f, n_iter, -1, s.d_trend, s.stream);
+        if (status != UMI_OK) break;
+        if (cuda_failed(cudaMemcpyAsync(trend_out + off, s.d_trend, cnt * sizeof(float), cudaMemcpyDeviceToHost, s.stream)))
+            status = UMI_ERR_CUDA;
+    }
+
+    for (auto& s : slots) {
+        if (s.stream != nullptr && cuda_failed(cudaStreamSynchronize(s.stream))) status = UMI_ERR_CUDA;
+    }
+    for (auto& s : slots) {
+        if (s.d_flux) (void)cudaFree(s.d_flux);
+        if (s.d_trend) (void)cudaFree(s.d_trend);
+        if (s.d_time) (void)cudaFree(s.d_time);
+        if (s.stream) (void)cudaStreamDestroy(s.stream);
+    }
+    (void)cudaGetLastError();
+    return status;
+}
+
+int umi_launch_geometry(int W, int* median_tile, int* median_sort_n, int* weight_tile)
+{
+    const int st = check_window(W);
+    if (st != UMI_OK) return st;
+    const Geometry g = geometry_for(W);
+    if (median_tile) *median_tile = g.T1;
+    if (median_sort_n) *median_sort_n = g.NS;
+    if (weight_tile) *weight_tile = umi::K2_TILE;
+    return UMI_OK;
+}
+
+const char* umi_status_string(int status)
+{
+    switch (status) {
+    case UMI_OK: return "UMI_OK";
+    case UMI_ERR_INVALID_ARG: return "UMI_ERR_INVALID_ARG: null pointer, negative size, even or < 1 window, or bad alpha/c/n_iter";
+    case UMI_ERR_UNSUPPORTED: return "UMI_ERR_UNSUPPORTED: window longer than UMI_MAX_WINDOW";
+    case UMI_ERR_CUDA: return "UMI_ERR_CUDA: a CUDA launch, copy or allocation failed";
+    default: return "UMI: unknown status";
+    }
+}
+
+int umi_version(void) { return 100; /* 0.1.0 */ }
+
+} /* extern "C" */

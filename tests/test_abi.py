@@ -1,0 +1,100 @@
+"""CPU checks of the C-ABI boundary (include/umi.h): the library loads, exports every
+declared symbol, and its host-only logic (window rule, validation, geometry) behaves
+as the header says.  No kernel is launched here."""
+import ctypes
+import os
+import re
+
+import pytest
+
+import paper_2604_06602_b200 as umi
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+HEADER = os.path.join(ROOT, "include", "umi.h")
+
+
+def _declared_symbols():
+    src = open(HEADER).read()
+    src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
+    return sorted(set(re.findall(r"\b(umi_[a-z_]+)\s*\(", src)))
+
+
+def test_library_builds_loads_and_exports_every_declared_symbol():
+    from paper_2604_06602_b200 import build
+    path = build.build()
+    assert os.path.exists(path)
+    L = ctypes.CDLL(path)
+    declared = _declared_symbols()
+    assert set(declared) == set(umi.EXPORTS), (declared, umi.EXPORTS)
+    for name in declared:
+        assert hasattr(L, name), name
+    assert umi.umi_version() >= 100
+
+
+def test_window_len_paper_values_and_guard():
+    # PAPER.md:35 (TESS 2 min -> 361), PAPER.md:192 (Kepler 30 min -> 25); BASELINE.json configs
+    assert umi.umi_window_len(2.0 / 1440) == 361
+    assert umi.umi_window_len(30.0 / 1440) == 25
+    assert umi.umi_window_len(29.4 / 1440) == 25
+    assert umi.umi_window_len(20.0 / 86400) == 2161
+    assert umi.umi_window_len(200.0 / 86400) == 217
+    # (R15) a cadence that went through fp32 must not lose the last sample
+    import numpy as np
+    assert umi.umi_window_len(float(np.float32(2.0 / 1440))) == 361
+    assert umi.umi_window_len(float(np.float32(200.0 / 86400))) == 217
+    for bad in (0.0, -1.0, float("nan"), float("inf"), 1e-300):
+        assert umi.umi_window_len(bad) == 0
+    assert umi.umi_window_len(10.0) == 1   # floor(0.05) | 1
+    for dt in (0.001, 0.0137, 0.02, 0.3):
+        W = umi.umi_window_len(dt)
+        assert W % 2 == 1 and W >= 1
+
+
+def test_validation_happens_on_the_host():
+    L = umi.lib()
+    one = ctypes.c_void_p(16)   # never dereferenced: validation fails first or sizes are 0
+    call = lambda **k: L.umi_detrend(k.get("time"), k.get("flux", one), k.get("S", 1), k.get("N", 10),
+                                     k.get("W", 5), k.get("alpha", 2.0), k.get("n_iter", 5),
+                                     k.get("out", one), None)
+    assert call(flux=None) == umi.UMI_ERR_INVALID_ARG
+    assert call(out=None) == umi.UMI_ERR_INVALID_ARG
+    assert call(S=-1) == umi.UMI_ERR_INVALID_ARG
+    assert call(N=-1) == umi.UMI_ERR_INVALID_ARG
+    assert call(W=4) == umi.UMI_ERR_INVALID_ARG
+    assert call(W=0) == umi.UMI_ERR_INVALID_ARG
+    assert call(W=-3) == umi.UMI_ERR_INVALID_ARG
+    assert call(alpha=0.0) == umi.UMI_ERR_INVALID_ARG
+    assert call(alpha=-2.0) == umi.UMI_ERR_INVALID_ARG
+    assert call(alpha=float("nan")) == umi.UMI_ERR_INVALID_ARG
+    assert call(alpha=float("inf")) == umi.UMI_ERR_INVALID_ARG
+    assert call(n_iter=-1) == umi.UMI_ERR_INVALID_ARG
+    assert call(W=umi.UMI_MAX_WINDOW + 2) == umi.UMI_ERR_UNSUPPORTED
+    assert call(S=0) == umi.UMI_OK      # empty batch: nothing enqueued
+    assert call(N=0) == umi.UMI_OK
+    assert L.umi_detrend_ex(None, one, 1, 10, 5, 2.0, 0.0, 5, -1, one, None) == umi.UMI_ERR_INVALID_ARG
+    assert L.umi_detrend_host(None, None, 1, 10, 5, 2.0, 5, one, 0, 0) == umi.UMI_ERR_INVALID_ARG
+    assert L.umi_detrend_host(None, one, 0, 10, 5, 2.0, 5, one, 0, 0) == umi.UMI_OK
+    for s in range(5):
+        assert umi.umi_status_string(s)
+    assert "UMI_OK" in umi.umi_status_string(0)
+
+
+def test_launch_geometry():
+    for W in (1, 3, 25, 217, 361, 513, 1081, 2161, 4097):
+        T, NS, T2 = umi.umi_launch_geometry(W)
+        assert NS & (NS - 1) == 0 and NS >= 1024
+        assert T + W - 1 == NS
+        assert T >= max(1, (W - 1) // 2)
+        assert NS * 14 <= 227 * 1024
+        assert T2 == 512
+    assert umi.umi_launch_geometry(361)[:2] == (664, 1024)
+    with pytest.raises(umi.UmiError):
+        umi.umi_launch_geometry(4)
+    with pytest.raises(umi.UmiError):
+        umi.umi_launch_geometry(5001)
+
+
+def test_binding_rejects_host_tensors_on_the_device_path():
+    import torch
+    with pytest.raises(TypeError):
+        umi.umi_detrend(None, torch.zeros(2, 8), 3)
