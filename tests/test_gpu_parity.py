@@ -1,0 +1,135 @@
+"""GPU parity tests: the CUDA path, called through the C ABI (include/umi.h) via the
+thin binding, against the fp64 oracle, element by element on the same seeded inputs.
+Bars: median bit-exact, trend within 1e-5 relative, NaN pattern equal.
+"""
+import numpy as np
+import pytest
+
+from oracle import umi_oracle as orc
+from tests import parity
+from workloads import lightcurves as lc
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def umi():
+    import paper_2604_06602_b200 as m
+    m.lib()   # fail loudly if the CUDA library is missing: no fallback
+    return m
+
+
+def _gpu(umi, flux, W, n_iter=5, alpha=2.0, time=None, **kw):
+    import torch
+    f = torch.from_numpy(np.ascontiguousarray(flux, dtype=np.float32)).cuda()
+    t = None if time is None else torch.from_numpy(np.ascontiguousarray(time, dtype=np.float64)).cuda()
+    out = umi.umi_detrend(t, f, W, alpha=alpha, n_iter=n_iter, **kw)
+    torch.cuda.synchronize()
+    return out.cpu().numpy()
+
+
+def _both(umi, flux, W, alpha=2.0, n_iter=5, time=None, c=None, min_valid=None):
+    """Median (n_iter = 0) bit-exact and trend within tolerance, all positions."""
+    kw = {}
+    okw = {}
+    if c is not None:
+        kw["c"] = c
+        okw["c"] = c
+    if min_valid is not None:
+        kw["min_valid"] = min_valid
+        okw["min_valid"] = min_valid
+    ref = orc.detrend(flux, W, alpha=alpha, n_iter=n_iter, time=time, **okw)
+    med = _gpu(umi, flux, W, n_iter=0, alpha=alpha, time=time, **kw)
+    parity.compare_median(med, ref.median)
+    if n_iter == 0:
+        return None
+    got = _gpu(umi, flux, W, n_iter=n_iter, alpha=alpha, time=time, **kw)
+    return parity.compare_trend(got, ref)
+
+
+# ------------------------------------------------------------------ small, every position
+@pytest.mark.parametrize("W", [1, 3, 5, 7, 9, 25, 51, 217, 361, 513, 515, 1081])
+def test_random_series_with_gaps_and_inf(umi, W):
+    # 3 stars x 3001 cadences: several tiles of both kernels and a ragged tail
+    x = lc.random_series(W, 3, 3001)
+    _both(umi, x, W)
+
+
+@pytest.mark.parametrize("W", [3, 25, 361])
+def test_heavy_ties(umi, W):
+    x = lc.random_series(100 + W, 2, 2500, nan_frac=0.02, inf_frac=0.0, ties=True)
+    _both(umi, x, W)
+
+
+@pytest.mark.parametrize("N", [1, 2, 3, 4, 5, 31, 32, 33, 511, 512, 513, 663, 664, 665, 1327, 1329])
+def test_ragged_lengths(umi, N):
+    x = lc.random_series(N, 2, N, nan_frac=0.03 if N > 8 else 0.0, inf_frac=0.0)
+    for W in (1, 5, 361):
+        _both(umi, x, W)   # W > N is legal: the window is clipped (R2)
+
+
+def test_large_windows(umi):
+    x = lc.random_series(7, 2, 9000, nan_frac=0.02)
+    for W in (2161, 4097):
+        _both(umi, x, W)
+
+
+def test_alpha_and_c_presets(umi):
+    # PAPER.md:79 (alpha = 3 Kepler, 1 variable stars), Table 4 (alpha = 10, c = 2.5)
+    x = lc.random_series(11, 2, 2000, nan_frac=0.02)
+    _both(umi, x, 25, alpha=3.0)
+    _both(umi, x, 361, alpha=1.0)
+    _both(umi, x, 361, alpha=0.5)
+    _both(umi, x, 361, alpha=10.0, c=2.5)
+    _both(umi, x, 51, alpha=2.0, n_iter=1)
+    _both(umi, x, 51, alpha=2.0, n_iter=12)
+    _both(umi, x, 51, alpha=2.0, min_valid=1)
+    _both(umi, x, 51, alpha=2.0, min_valid=40)
+
+
+def test_time_marks_cadences_invalid(umi):
+    x = lc.random_series(21, 2, 1500, nan_frac=0.01, inf_frac=0.0)
+    t = np.tile(np.arange(1500, dtype=np.float64) * (2.0 / 1440), (2, 1))
+    t[0, 100:180] = np.nan
+    t[1, 700] = np.inf
+    t[1, 1499] = -np.inf
+    _both(umi, x, 25, time=t)
+    _both(umi, x, 361, time=t)
+
+
+def test_degenerate_inputs(umi):
+    import torch
+    # constant series returns itself bit for bit (R8)
+    x = np.full((2, 1000), 1.2345678, np.float32)
+    for W in (5, 361):
+        got = _gpu(umi, x, W)
+        assert np.array_equal(got, x)
+    # all invalid -> all NaN
+    x = np.full((1, 700), np.nan, np.float32)
+    assert np.isnan(_gpu(umi, x, 25)).all()
+    # a lone valid sample with min_valid = 1
+    x = np.full((1, 700), np.nan, np.float32)
+    x[0, 350] = 3.0
+    got = _gpu(umi, x, 25, min_valid=1)
+    assert got[0, 350] == 3.0 and np.isnan(np.delete(got[0], 350)).all()
+    # two levels: n_plus > 0 but many ties with the median
+    x = np.ones((1, 900), np.float32)
+    x[0, ::3] = 1.5
+    _both(umi, x, 25)
+    # signed zeros and negative values
+    x = lc.random_series(5, 1, 800, nan_frac=0.0, inf_frac=0.0) - 1.0
+    x[0, ::7] = -0.0
+    x[0, 1::7] = 0.0
+    _both(umi, x, 9, n_iter=0)   # values straddle 0: only the median has a relative bar
+    # empty batch: OK, nothing enqueued
+    e = umi.umi_detrend(None, torch.empty((0, 100), dtype=torch.float32, device="cuda"), 5)
+    assert e.shape == (0, 100)
+    with pytest.raises(umi.UmiError):
+        umi.umi_detrend(None, torch.zeros((1, 10), device="cuda"), 4)
+
+
+def test_extreme_magnitudes(umi):
+    # large offsets and tiny scales: fp32 arithmetic must stay within tolerance
+    base = lc.random_series(31, 1, 1500, nan_frac=0.01, inf_frac=0.0)
+    for scale, offset in ((1.0, 0.0), (1e4, 0.0), (1e-3, 0.0), (1.0, 100.0)):
+        _both(umi, (base * scale + offset).astype(np.float32), 51)
