@@ -1,0 +1,325 @@
+#!/usr/bin/env python
+"""bench.py -- detrended cadences/s of the UMI hot path on B200 (BASELINE.json metric).
+
+  python bench.py --gpus N --steps K --warmup W            # this repo's CUDA path
+  python bench.py --impl reference ...                     # the fp64 oracle on host cores
+
+A "step" is one pass of the whole hot path (median kernel + reweighting kernel,
+SURVEY.md 8(a) rows a1-a5) over one synthetic batch.  Default workload = config 2,
+the one the metric is quoted on: 1,000 stars x 19,440 cadences, W = 361, alpha = 2,
+5 iterations (workloads/lightcurves.py, seeded; stands in for TESS sector data).
+N > 1 (torchrun): stars are independent, each rank detrends its own 1,000
+separately seeded stars, no collective on the data path -> "scaling": "weak".
+
+Prints ONE JSON line ("Measurement", for every field).
+"""
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from workloads import lightcurves as lc  # noqa: E402
+
+METRIC = "detrended cadences/sec on 1 B200 (TESS W=361 batch) + fraction of roofline"
+UNIT = "cadences/s"
+
+# DESIGN.md, "Roofline": algorithmic lane-operations per window-sample
+#   Phase 2: 4 (sub, compare, predicated fma, count); Phase 3: 9 per pass
+#   (sub, setp, sel, mul, fma, max, mul, add, fma)  -> 4 + 9 * n_iter = 49 at n_iter = 5.
+OPS_PHASE2 = 4
+OPS_PER_PASS = 9
+SM_COUNT = 148
+LANES_PER_SM = 128          # 4 schedulers x 32 lanes, one warp instruction per clock each
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--config", type=int, default=2, choices=sorted(lc.CONFIGS))
+    ap.add_argument("--stars", type=int, default=None, help="override the star count (debug)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    return ap.parse_args()
+
+
+def exact_window_samples(flux, W, min_valid):
+    """Sum over evaluated positions (own sample valid, >= min_valid valid samples in the
+    window) of the number of valid samples in the window.  Host-side bookkeeping for the
+    roofline numerator: a validity prefix sum, none of the method's arithmetic."""
+    S, N = flux.shape
+    h = W // 2
+    lo = np.clip(np.arange(N) - h, 0, N)
+    hi = np.clip(np.arange(N) + h + 1, 0, N)
+    total = 0
+    for s0 in range(0, S, 256):
+        valid = np.isfinite(flux[s0:s0 + 256])
+        csum = np.zeros((valid.shape[0], N + 1), np.int64)
+        np.cumsum(valid, axis=1, out=csum[:, 1:])
+        n = csum[:, hi] - csum[:, lo]
+        ev = valid & (n >= min_valid)
+        total += int(n[ev].sum())
+    return total
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons with NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.05):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.samples, self.reasons, self.max_mhz = [], set(), None
+        self._stop_evt = threading.Event()
+        self.ok = False
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.h, pynvml.NVML_CLOCK_SM)
+            self.ok = True
+        except Exception:
+            self.ok = False
+
+    def run(self):
+        if not self.ok:
+            return
+        nv = self.nv
+        names = {
+            getattr(nv, "nvmlClocksThrottleReasonHwSlowdown", 0x8): "hw_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonHwThermalSlowdown", 0x40): "hw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwThermalSlowdown", 0x20): "sw_thermal_slowdown",
+            getattr(nv, "nvmlClocksThrottleReasonSwPowerCap", 0x4): "sw_power_cap",
+            getattr(nv, "nvmlClocksThrottleReasonHwPowerBrakeSlowdown", 0x80): "hw_power_brake",
+        }
+        while not self._stop_evt.is_set():
+            try:
+                self.samples.append(nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM))
+                mask = nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                for bit, name in names.items():
+                    if mask & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def stop(self):
+        self._stop_evt.set()
+        if self.is_alive():
+            self.join(timeout=2)
+        med = float(np.median(self.samples)) if self.samples else None
+        return {"sm_mhz": med, "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons),
+                "samples": len(self.samples)}
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return json.load(f), "measured"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
+
+
+def oracle_sample(cfg, flux, n_stars):
+    """Times the fp64 oracle, as it stands, on the first n_stars stars of the workload."""
+    from oracle import umi_oracle as orc
+    sub = np.ascontiguousarray(flux[:n_stars])
+    orc.detrend(sub[:1, :2000], cfg.W)                       # load + thread pool warm-up
+    t0 = time.perf_counter()
+    orc.detrend(sub, cfg.W, alpha=cfg.alpha, n_iter=cfg.n_iter)
+    dt = time.perf_counter() - t0
+    return sub.size / dt, dt, orc.num_threads()
+
+
+def run_reference(args, cfg, rank):
+    """--impl reference: the oracle on the box's host cores, each step a bounded sample."""
+    if rank != 0:
+        return
+    n_sample = min(cfg.n_stars if args.stars is None else args.stars,
+                   max(1, int(600_000 // cfg.n_cadences) or 1))       # ~0.6 M cadences per step
+    flux = lc.stars(args.config, range(n_sample))
+    from oracle import umi_oracle as orc
+    for _ in range(max(args.warmup, 1)):
+        orc.detrend(flux[:1], cfg.W, alpha=cfg.alpha, n_iter=cfg.n_iter)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        orc.detrend(flux, cfg.W, alpha=cfg.alpha, n_iter=cfg.n_iter)
+    dt = time.perf_counter() - t0
+    value = flux.size * args.steps / dt
+    sample = "first %d of %d stars per step, all cadences, fp64, OpenMP" % (n_sample, cfg.n_stars)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "gpu_launches": 0,
+        "config": {"workload": "config%d %s: %d stars x %d cadences, W=%d, alpha=%g, n_iter=%d"
+                   % (args.config, cfg.name, cfg.n_stars, cfg.n_cadences, cfg.W, cfg.alpha, cfg.n_iter)},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+                         "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line))
+
+
+def run_ours(args, cfg, rank, world, local_rank):
+    import torch
+    import paper_2604_06602_b200 as umi
+    umi.lib()                                            # no fallback: raises if the .so is missing
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py --impl ours needs a CUDA device (no CPU fallback)")
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+
+    S = cfg.n_stars if args.stars is None else args.stars
+    N, W = cfg.n_cadences, cfg.W
+    flux_np = lc.stars(args.config, range(rank * S, (rank + 1) * S))     # weak scaling: own stars
+    min_valid = max(1, W // 3)
+    ws_exact = exact_window_samples(flux_np, W, min_valid)
+    h_flux = torch.from_numpy(flux_np).pin_memory()
+    h_out = torch.empty_like(h_flux).pin_memory()
+    d_flux = h_flux.to(dev, non_blocking=True)
+    d_out = torch.empty_like(d_flux)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)        # > 126 MB L2
+    stream = torch.cuda.Stream(dev)
+    torch.cuda.synchronize()
+
+    def step():
+        umi.umi_detrend(None, d_flux, W, alpha=cfg.alpha, n_iter=cfg.n_iter, out=d_out, stream=stream)
+
+    with torch.cuda.stream(stream):
+        for _ in range(max(args.warmup, 3)):
+            flush.zero_()
+            step()
+    torch.cuda.synchronize()
+    if dist is not None:
+        dist.barrier()
+
+    # ---- timed region: K steps, device time per step from CUDA events on the launch stream
+    sampler = ClockSampler(local_rank, period=0.01)
+    sampler.start()
+    ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    torch.cuda.synchronize()
+    with torch.cuda.stream(stream):
+        for a, b in ev:
+            flush.zero_()                                # L2 flush between timed iterations (untimed)
+            a.record(stream)
+            step()
+            b.record(stream)
+    torch.cuda.synchronize()
+    step_ms = [a.elapsed_time(b) for a, b in ev]
+    # ---- same steps again through umi_detrend_profile: per-kernel device times (events
+    #      recorded by the library on the same stream), for the roofline of the dominant kernel
+    k_ms = []
+    with torch.cuda.stream(stream):
+        for _ in range(args.steps):
+            flush.zero_()
+            _, m1, m2 = umi.umi_detrend_profile(None, d_flux, W, alpha=cfg.alpha, n_iter=cfg.n_iter,
+                                                out=d_out, stream=stream)
+            k_ms.append((m1, m2))
+    clocks = sampler.stop()
+    if dist is not None:
+        dist.barrier()
+    total_ms = float(sum(step_ms))
+    if dist is not None:
+        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+
+    # ---- end to end through the public host API: pinned host buffers in, pinned host out
+    e2e = None
+    if not args.no_e2e:
+        for _ in range(2):
+            umi.umi_detrend_host(None, h_flux, W, alpha=cfg.alpha, n_iter=cfg.n_iter, out=h_out)
+        if dist is not None:
+            dist.barrier()
+        t0 = time.perf_counter()
+        for _ in range(args.steps):
+            umi.umi_detrend_host(None, h_flux, W, alpha=cfg.alpha, n_iter=cfg.n_iter, out=h_out)
+        e2e_s = time.perf_counter() - t0
+        if dist is not None:
+            t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_s = float(t.item())
+        e2e = {"value": world * S * N * args.steps / e2e_s, "unit": UNIT,
+               "h2d_bytes_per_step": int(h_flux.numel() * 4), "d2h_bytes_per_step": int(h_out.numel() * 4),
+               "ms_per_step": 1e3 * e2e_s / args.steps,
+               "api": "umi_detrend_host (C ABI, pinned host buffers, 3 streams)"}
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    pk, pk_kind = peaks()
+    ms_per_step = total_ms / args.steps
+    value = world * S * N / (ms_per_step * 1e-3)
+    med_ms = float(np.mean([a for a, _ in k_ms]))
+    rw_ms = float(np.mean([b for _, b in k_ms]))
+    ops_per_ws = OPS_PHASE2 + OPS_PER_PASS * cfg.n_iter
+    sm_max = float(clocks["sm_max_mhz"] or pk.get("sm_max_mhz", 1965.0))
+    sm_now = float(clocks["sm_mhz"] or sm_max)
+    peak = SM_COUNT * LANES_PER_SM * sm_max * 1e6 / 1e12                 # Tlane-op/s at max clock
+    achieved = ops_per_ws * ws_exact / (rw_ms * 1e-3) / 1e12
+    roofline = {
+        "bound": "alu", "kernel": "umi_reweight_kernel",
+        "achieved": achieved, "peak": peak, "unit": "Tlane-op/s", "frac": achieved / peak,
+        "peak_def": "148 SMs x 4 schedulers x 32 lanes x 1 warp-instr/clk x sm_max_mhz (%s clocks)" % pk_kind,
+        "frac_at_measured_clock": achieved / (peak * sm_now / sm_max),
+        "ops_per_window_sample": ops_per_ws, "window_samples_per_launch": ws_exact,
+        "window_samples_nominal": S * N * W,
+        "kernel_ms": rw_ms, "median_kernel_ms": med_ms, "kernel_share_of_step": rw_ms / (rw_ms + med_ms),
+        "window_samples_per_s": ws_exact / (ms_per_step * 1e-3),
+        "hbm_algorithmic_GBps": 8.0 * S * N / (ms_per_step * 1e-3) / 1e9, "hbm_peak_GBps": pk.get("hbm_gbs"),
+        "traffic": None,
+    }
+    cpu = None
+    if not args.no_cpu_baseline:
+        rate, _, cores = oracle_sample(cfg, flux_np, min(S, 16))
+        n_s = int(min(S, max(16, rate * 15.0 / N)))                      # ~15 s of host work
+        rate, secs, cores = oracle_sample(cfg, flux_np, n_s)
+        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": "first %d of %d stars, all cadences, %.1f s" % (n_s, S, secs)}
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": ms_per_step, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": "config%d %s: %d stars x %d cadences per GPU, W=%d, alpha=%g, n_iter=%d"
+                   % (args.config, cfg.name, S, N, W, cfg.alpha, cfg.n_iter),
+                   "l2": "256 MiB buffer written between timed iterations",
+                   "timing": "CUDA events on the launch stream, per step, summed; max over ranks"},
+        "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * args.steps,
+        "roofline": roofline, "cpu_baseline": cpu,
+        "paper_context": "PAPER.md:147: 3.4 ms/star on AMD RX 9060 XT (~5.7e6 cadences/s at N=19440); not a target",
+    }
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    args = parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    cfg = lc.CONFIGS[args.config]
+    if args.impl == "reference":
+        run_reference(args, cfg, rank)
+    else:
+        run_ours(args, cfg, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

@@ -112,6 +112,18 @@ int umi_detrend_host(const double* time, const float* flux,
                      int64_t stars_per_batch, int n_streams);
 
 /*
+ * Measurement aid: umi_detrend_ex, plus the device time of each of its two
+ * kernels taken with CUDA events recorded on `stream` around each launch.
+ *   kernel_ms  HOST, float[2]: [0] Phase-1 median kernel, [1] Phase-2/3
+ *              reweighting kernel (0 when n_iter == 0), milliseconds.
+ * Unlike umi_detrend this call SYNCHRONISES `stream` before returning.
+ */
+int umi_detrend_profile(const double* time, const float* flux,
+                        int64_t n_stars, int64_t n_cadences,
+                        int W, float alpha, float c, int n_iter, int min_valid,
+                        float* trend_out, void* stream, float* kernel_ms);
+
+/*
  * Launch geometry the library uses for this W (for reports and roofline
  * arithmetic; host only).  Any pointer may be NULL.
  *   median_tile    positions per CTA of the Phase-1 (median) kernel

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libumi_b200.so")
 UMI_OK, UMI_ERR_INVALID_ARG, UMI_ERR_UNSUPPORTED, UMI_ERR_CUDA = 0, 1, 2, 3
 UMI_MAX_WINDOW = 4097
 
-EXPORTS = ("umi_window_len", "umi_detrend", "umi_detrend_ex", "umi_detrend_host",
+EXPORTS = ("umi_window_len", "umi_detrend", "umi_detrend_ex", "umi_detrend_host", "umi_detrend_profile",
            "umi_launch_geometry", "umi_status_string", "umi_version")
 
 _lib = None
@@ -47,6 +47,8 @@ def lib():
     L.umi_detrend.argtypes = [vp, vp, i64, i64, ci, cf, ci, vp, vp]
     L.umi_detrend_ex.restype = ci
     L.umi_detrend_ex.argtypes = [vp, vp, i64, i64, ci, cf, cf, ci, ci, vp, vp]
+    L.umi_detrend_profile.restype = ci
+    L.umi_detrend_profile.argtypes = [vp, vp, i64, i64, ci, cf, cf, ci, ci, vp, vp, ctypes.POINTER(cf)]
     L.umi_detrend_host.restype = ci
     L.umi_detrend_host.argtypes = [vp, vp, i64, i64, ci, cf, ci, vp, i64, ci]
     L.umi_launch_geometry.restype = ci
@@ -133,6 +135,30 @@ def umi_detrend(time, flux, W, alpha=2.0, n_iter=5, out=None, stream=None, c=Non
                                       -1 if min_valid is None else int(min_valid), optr, sptr)
     _check(st)
     return out.view(flux.shape)
+
+
+def umi_detrend_profile(time, flux, W, alpha=2.0, n_iter=5, out=None, stream=None, c=5.0, min_valid=-1):
+    """umi_detrend plus per-kernel device times: returns (trend, median_ms, reweight_ms).
+    Synchronises the stream (measurement aid)."""
+    import torch
+    f = _cuda_2d(flux, torch.float32, "flux")
+    tptr = None
+    if time is not None:
+        tt = _cuda_2d(time, torch.float64, "time")
+        if tt.shape != f.shape:
+            raise ValueError("time must have flux's shape")
+        tptr = tt.data_ptr()
+    if out is None:
+        out = torch.empty_like(f)
+    o = _cuda_2d(out, torch.float32, "out")
+    S, N = f.shape
+    ms = (ctypes.c_float * 2)()
+    with torch.cuda.device(f.device):
+        if stream is None:
+            stream = torch.cuda.current_stream(f.device)
+        _check(lib().umi_detrend_profile(tptr, f.data_ptr(), S, N, int(W), float(alpha), float(c),
+                                         int(n_iter), int(min_valid), o.data_ptr(), stream.cuda_stream, ms))
+    return out.view(flux.shape), float(ms[0]), float(ms[1])
 
 
 def umi_detrend_host(time, flux, W, alpha=2.0, n_iter=5, out=None, stars_per_batch=0, n_streams=0):

@@ -65,7 +65,7 @@ int validate(const float* flux, int64_t n_stars, int64_t n_cadences, int W, floa
 /* Enqueue both kernels for device-resident buffers. */
 int launch_device(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
                   int W, float alpha, float c, int n_iter, int min_valid, float* trend_out,
-                  cudaStream_t stream)
+                  cudaStream_t stream, cudaEvent_t* ev = nullptr /* [3] or null */)
 {
     if (n_stars == 0 || n_cadences == 0) return UMI_OK;
     const Geometry g = geometry_for(W);
@@ -88,8 +88,10 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
             return UMI_ERR_CUDA;
     }
     const unsigned grid1 = (unsigned)std::min<int64_t>(mp.n_blocks, MAX_GRID);
+    if (ev && cuda_failed(cudaEventRecord(ev[0], stream))) return UMI_ERR_CUDA;
     umi::umi_median_kernel<<<grid1, umi::K1_THREADS, g.smem1, stream>>>(mp);
     if (cuda_failed(cudaGetLastError())) return UMI_ERR_CUDA;
+    if (ev && cuda_failed(cudaEventRecord(ev[1], stream))) return UMI_ERR_CUDA;
 
     if (n_iter > 0) {
         umi::ReweightParams rp;
@@ -107,6 +109,7 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         umi::umi_reweight_kernel<<<grid2, umi::K2_THREADS, g.smem2, stream>>>(rp);
         if (cuda_failed(cudaGetLastError())) return UMI_ERR_CUDA;
     }
+    if (ev && cuda_failed(cudaEventRecord(ev[2], stream))) return UMI_ERR_CUDA;
     return UMI_OK;
 }
 
@@ -130,6 +133,31 @@ int umi_detrend_ex(const double* time, const float* flux, int64_t n_stars, int64
     if (st != UMI_OK) return st;
     return launch_device(time, flux, n_stars, n_cadences, W, alpha, c, n_iter, min_valid, trend_out,
                          static_cast<cudaStream_t>(stream));
+}
+
+int umi_detrend_profile(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
+                        int W, float alpha, float c, int n_iter, int min_valid,
+                        float* trend_out, void* stream, float* kernel_ms)
+{
+    if (kernel_ms == nullptr) return UMI_ERR_INVALID_ARG;
+    kernel_ms[0] = kernel_ms[1] = 0.f;
+    int st = validate(flux, n_stars, n_cadences, W, alpha, c, n_iter, trend_out);
+    if (st != UMI_OK) return st;
+    if (n_stars == 0 || n_cadences == 0) return UMI_OK;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    cudaEvent_t ev[3] = {nullptr, nullptr, nullptr};
+    for (auto& e : ev)
+        if (cuda_failed(cudaEventCreate(&e))) st = UMI_ERR_CUDA;
+    if (st == UMI_OK)
+        st = launch_device(time, flux, n_stars, n_cadences, W, alpha, c, n_iter, min_valid, trend_out, s, ev);
+    if (st == UMI_OK && cuda_failed(cudaEventSynchronize(ev[2]))) st = UMI_ERR_CUDA;
+    if (st == UMI_OK &&
+        (cuda_failed(cudaEventElapsedTime(&kernel_ms[0], ev[0], ev[1])) ||
+         cuda_failed(cudaEventElapsedTime(&kernel_ms[1], ev[1], ev[2]))))
+        st = UMI_ERR_CUDA;
+    for (auto& e : ev)
+        if (e) (void)cudaEventDestroy(e);
+    return st;
 }
 
 int umi_detrend(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
