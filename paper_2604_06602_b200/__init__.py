@@ -13,7 +13,8 @@ import ctypes
 import os
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(_HERE, "libumi_b200.so")
+# UMI_B200_LIB selects another build of the same library (kernel experiments); default: in-tree.
+LIB_PATH = os.environ.get("UMI_B200_LIB") or os.path.join(_HERE, "libumi_b200.so")
 
 UMI_OK, UMI_ERR_INVALID_ARG, UMI_ERR_UNSUPPORTED, UMI_ERR_CUDA = 0, 1, 2, 3
 UMI_MAX_WINDOW = 4097

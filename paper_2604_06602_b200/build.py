@@ -9,8 +9,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = [os.path.join(CSRC, "umi_api.cu"), os.path.join(CSRC, "umi_kernels.cu")]
-HEADERS = [os.path.join(CSRC, "umi_internal.h"), os.path.join(ROOT, "include", "umi.h")]
+SOURCES = [os.path.join(CSRC, "umi_api.cu"), os.path.join(CSRC, "umi_median.cu"), os.path.join(CSRC, "umi_reweight.cu")]
+HEADERS = [os.path.join(CSRC, "umi_internal.h"), os.path.join(CSRC, "umi_device.cuh"), os.path.join(ROOT, "include", "umi.h")]
 LIB = os.path.join(HERE, "libumi_b200.so")
 
 NVCC_FLAGS = [

@@ -1,0 +1,320 @@
+/*
+ * umi_reweight.cu -- Phase 2 + Phase 3 (Eq. 1-4): upper-RMS scale and
+ * n_iter asymmetric Tukey-bisquare passes, starting from the Phase-1 median.
+ *
+ * CTA = one star x 512 positions; a thread owns 4 consecutive positions and streams
+ * the W+3 samples they share from shared memory with one 128-bit load per 16
+ * (sample, position) evaluations; all accumulators stay in registers, there are no
+ * reductions.  Invalid samples are replaced in shared memory by a finite per-tile
+ * sentinel far below the tile minimum, which Eq. 1 never counts and Eq. 3 always
+ * gives weight 0, so the inner loop carries no validity predicate.
+ *
+ * Inner loop ("Reweighting kernel"): per (sample, position)
+ *     u  = x*k + c0                 k = 1/(c s), c0 = -mu*k
+ *     e  = max(u, -alpha*u)         = |u_eff| of Eq. 2 for any alpha > 0
+ *     t  = sat(1 - e*e)             Eq. 3 (R12): 0 outside the cut-off
+ *     w  = t*t;  S += w;  R += w*u  Eq. 4 in centred form: mu <- mu + c s R/S
+ * With UMI_K2_PACKED the fma/mul/add steps run as sm_100a packed fp32x2
+ * instructions (FFMA2/FMUL2/FADD2) on two consecutive samples at a time.
+ * Nothing here is shared with oracle/.
+ */
+#include "umi_device.cuh"
+
+#ifndef UMI_K2_PACKED
+#define UMI_K2_PACKED 1
+#endif
+#ifndef UMI_K2_MIN_CTAS
+#define UMI_K2_MIN_CTAS 8
+#endif
+#ifndef UMI_K2_UNROLL
+#define UMI_K2_UNROLL 2
+#endif
+
+namespace umi {
+
+namespace {
+
+constexpr int K2_UNROLL = UMI_K2_UNROLL;
+
+/* Phase 2, Eq. 1: strictly-above-median residuals (R7). */
+__device__ __forceinline__ void eval_scale(float x, float med, float& ss, float& cnt)
+{
+    const float d = x - med;
+    const float dp = fmaxf(d, 0.f);
+    ss = fmaf(dp, dp, ss);
+    cnt += (d > 0.f) ? 1.f : 0.f;
+}
+
+/* Phase 3, one (sample, position): accumulates sum w and sum w*u. */
+__device__ __forceinline__ void eval_weight(float x, float k, float c0, float nalpha,
+                                            float& S, float& R)
+{
+    const float a = fmaf(x, k, c0);                  /* u */
+    const float b = a * nalpha;                      /* -alpha*u */
+    const float e = fmaxf(a, b);                     /* |u_eff| */
+    const float t = __saturatef(fmaf(-e, e, 1.f));   /* FFMA.SAT */
+    const float w = t * t;
+    S += w;
+    R = fmaf(w, a, R);
+}
+
+#if UMI_K2_PACKED
+typedef unsigned long long f32x2;                    /* two fp32 in one 64-bit register pair */
+
+__device__ __forceinline__ f32x2 pack2(float lo, float hi)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 ffma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 fmul2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 fadd2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
+/* Phase 3 on one 128-bit group: 4 samples (two fp32x2 pairs) x 4 positions = 8 pair
+   evaluations, written stage by stage so that the 8 dependency chains interleave. */
+__device__ __forceinline__ void eval_weight_group(f32x2 x01, f32x2 x23, const f32x2 (&k2)[K2_NPOS],
+                                                  const f32x2 (&c02)[K2_NPOS], f32x2 nalpha2,
+                                                  f32x2 (&S2)[K2_NPOS], f32x2 (&R2)[K2_NPOS])
+{
+    f32x2 a2[2 * K2_NPOS], w2[2 * K2_NPOS];
+    float e[4 * K2_NPOS];
+#pragma unroll
+    for (int q = 0; q < K2_NPOS; ++q) {
+        a2[2 * q] = ffma2(x01, k2[q], c02[q]);
+        a2[2 * q + 1] = ffma2(x23, k2[q], c02[q]);
+    }
+#pragma unroll
+    for (int i = 0; i < 2 * K2_NPOS; ++i) {
+        const f32x2 b2 = fmul2(a2[i], nalpha2);
+        float a0, a1, b0, b1;
+        unpack2(a2[i], a0, a1);
+        unpack2(b2, b0, b1);
+        e[2 * i] = fmaxf(a0, b0);
+        e[2 * i + 1] = fmaxf(a1, b1);
+    }
+    const f32x2 mone2 = pack2(-1.f, -1.f);
+#pragma unroll
+    for (int i = 0; i < 2 * K2_NPOS; ++i) {
+        /* e*e - 1 packed; the clamp max(1 - e*e, 0) runs on the ALU pipe (FMNMX, negated source),
+           so the FMA pipe only ever sees packed instructions */
+        const f32x2 n2 = ffma2(pack2(e[2 * i], e[2 * i + 1]), pack2(e[2 * i], e[2 * i + 1]), mone2);
+        float n0, n1;
+        unpack2(n2, n0, n1);
+        const f32x2 t2 = pack2(fmaxf(-n0, 0.f), fmaxf(-n1, 0.f));
+        w2[i] = fmul2(t2, t2);
+    }
+#pragma unroll
+    for (int q = 0; q < K2_NPOS; ++q) {
+        S2[q] = fadd2(S2[q], fadd2(w2[2 * q], w2[2 * q + 1]));
+        R2[q] = ffma2(w2[2 * q], a2[2 * q], R2[q]);
+        R2[q] = ffma2(w2[2 * q + 1], a2[2 * q + 1], R2[q]);
+    }
+}
+#endif
+
+} // namespace
+
+__global__ void __launch_bounds__(K2_THREADS, UMI_K2_MIN_CTAS)
+umi_reweight_kernel(ReweightParams prm)
+{
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    float* xs = reinterpret_cast<float*>(smem_raw);
+    __shared__ float s_red[2 * (K2_THREADS / 32)];
+
+    const int tid = threadIdx.x;
+    const int W = prm.W;
+    const int h = (W - 1) >> 1;
+    const int hal = (h + 3) & ~3;
+    const int delta = hal - h;
+    const int G = (3 + delta + 2 * h) / 4 + 1;          /* float4 groups per thread */
+    const int nx = K2_TILE + 4 * G;                     /* staged floats */
+    const int g_lo = (3 + delta + 3) >> 2;              /* first group fully inside all 4 windows */
+    const int g_hi = (delta + 2 * h - 3) >= 0 ? ((delta + 2 * h - 3) >> 2) : -1;   /* last such group */
+    const float nalpha = -prm.alpha;
+    const float qnan = __int_as_float(0x7FC00000);
+
+    for (int64_t bid = blockIdx.x; bid < prm.n_blocks; bid += gridDim.x) {
+        const int64_t star = bid / prm.tiles_per_star;
+        const int64_t tile = bid - star * prm.tiles_per_star;
+        const int64_t j0 = tile * K2_TILE;
+        const int64_t jbase = j0 - hal;                 /* cadence of staged index 0 */
+        const float* frow = prm.flux + star * prm.N;
+        const double* trow = prm.time ? prm.time + star * prm.N : nullptr;
+        float* orow = prm.out + star * prm.N;
+
+        /* stage the union, NaN marks invalid; tile min / max of the valid samples */
+        float tmin = INFINITY, tmax = -INFINITY;
+        for (int u = tid; u < nx; u += K2_THREADS) {
+            float x = 0.f;
+            const bool ok = load_sample(trow, frow, prm.N, jbase + u, x);
+            if (ok) { tmin = fminf(tmin, x); tmax = fmaxf(tmax, x); }
+            xs[u] = ok ? x : qnan;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            tmin = fminf(tmin, __shfl_xor_sync(0xFFFFFFFFu, tmin, o));
+            tmax = fmaxf(tmax, __shfl_xor_sync(0xFFFFFFFFu, tmax, o));
+        }
+        if ((tid & 31) == 0) { s_red[(tid >> 5) * 2] = tmin; s_red[(tid >> 5) * 2 + 1] = tmax; }
+        __syncthreads();
+#pragma unroll
+        for (int w = 0; w < K2_THREADS / 32; ++w) {
+            tmin = fminf(tmin, s_red[2 * w]);
+            tmax = fmaxf(tmax, s_red[2 * w + 1]);
+        }
+        /* sentinel: alpha*(mu - x)/(c s) >= 2 for every window of the tile, since
+           mu >= tmin and s <= 0.6745 (tmax - tmin)  ("Sentinel") */
+        float sent = 0.f;
+        if (tmin <= tmax) {
+            sent = tmin - 2.f * (prm.c * SCALE_CONST / prm.alpha) * (tmax - tmin);
+            sent = fmaxf(sent, -3.0e38f);
+        }
+        for (int u = tid; u < nx; u += K2_THREADS) {
+            const float x = xs[u];
+            if (x != x) xs[u] = sent;
+        }
+        __syncthreads();
+
+        /* per-position state: 4 consecutive positions, local index 4*tid + q */
+        float med[K2_NPOS], mu[K2_NPOS], kk[K2_NPOS], cs[K2_NPOS];
+        bool act[K2_NPOS];
+        bool any_act = false;
+#pragma unroll
+        for (int q = 0; q < K2_NPOS; ++q) {
+            const int64_t j = j0 + 4 * tid + q;
+            med[q] = (j < prm.N) ? orow[j] : qnan;
+            act[q] = (med[q] == med[q]);
+            any_act = any_act || act[q];
+            mu[q] = act[q] ? med[q] : 0.f;
+            kk[q] = 0.f;
+            cs[q] = 0.f;
+        }
+        const float4* xs4 = reinterpret_cast<const float4*>(xs) + tid;
+
+        if (__any_sync(0xFFFFFFFFu, any_act)) {
+            /* ---- Phase 2 (Eq. 1) ---- */
+            float ss[K2_NPOS], cnt[K2_NPOS];
+#pragma unroll
+            for (int q = 0; q < K2_NPOS; ++q) { ss[q] = 0.f; cnt[q] = 0.f; }
+            for (int g = 0; g < G; ++g) {
+                const float4 v = xs4[g];
+                const float xv[4] = {v.x, v.y, v.z, v.w};
+                if (g >= g_lo && g <= g_hi) {
+#pragma unroll
+                    for (int q = 0; q < K2_NPOS; ++q)
+#pragma unroll
+                        for (int r = 0; r < 4; ++r) eval_scale(xv[r], mu[q], ss[q], cnt[q]);
+                } else {
+#pragma unroll
+                    for (int q = 0; q < K2_NPOS; ++q)
+#pragma unroll
+                        for (int r = 0; r < 4; ++r) {
+                            const int o = 4 * g + r - delta - q;
+                            if (o >= 0 && o <= 2 * h) eval_scale(xv[r], mu[q], ss[q], cnt[q]);
+                        }
+                }
+            }
+#pragma unroll
+            for (int q = 0; q < K2_NPOS; ++q) {
+                bool on = act[q] && cnt[q] > 0.f;                   /* (R8) */
+                float s = 0.f;
+                if (on) {
+                    s = SCALE_CONST * sqrtf(ss[q] / cnt[q]);
+                    on = s > 0.f;
+                }
+                act[q] = on;
+                cs[q] = on ? prm.c * s : 0.f;
+                kk[q] = on ? 1.f / cs[q] : 0.f;
+            }
+
+            /* ---- Phase 3 (Eq. 2-4), s held fixed (R9), exactly n_iter passes (R10) ---- */
+            for (int it = 0; it < prm.n_iter; ++it) {
+                float S[K2_NPOS], R[K2_NPOS], c0[K2_NPOS];
+#pragma unroll
+                for (int q = 0; q < K2_NPOS; ++q) { S[q] = 0.f; R[q] = 0.f; c0[q] = -mu[q] * kk[q]; }
+#if UMI_K2_PACKED
+                f32x2 S2[K2_NPOS], R2[K2_NPOS], k2[K2_NPOS], c02[K2_NPOS];
+                const f32x2 nalpha2 = pack2(nalpha, nalpha);
+#pragma unroll
+                for (int q = 0; q < K2_NPOS; ++q) {
+                    S2[q] = pack2(0.f, 0.f);
+                    R2[q] = pack2(0.f, 0.f);
+                    k2[q] = pack2(kk[q], kk[q]);
+                    c02[q] = pack2(c0[q], c0[q]);
+                }
+#endif
+                /* edge groups: samples that belong to some but not all of the 4 windows */
+                for (int g = 0; g < G; ++g) {
+                    if (g >= g_lo && g <= g_hi) { g = g_hi; continue; }
+                    const float4 v = xs4[g];
+                    const float xv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                    for (int q = 0; q < K2_NPOS; ++q)
+#pragma unroll
+                        for (int r = 0; r < 4; ++r) {
+                            const int o = 4 * g + r - delta - q;
+                            if (o >= 0 && o <= 2 * h) eval_weight(xv[r], kk[q], c0[q], nalpha, S[q], R[q]);
+                        }
+                }
+                /* interior groups: every sample belongs to all 4 windows */
+#if UMI_K2_PACKED
+#pragma unroll K2_UNROLL
+                for (int g = g_lo; g <= g_hi; ++g) {
+                    const ulonglong2 v2 = reinterpret_cast<const ulonglong2*>(xs4)[g];
+                    eval_weight_group(v2.x, v2.y, k2, c02, nalpha2, S2, R2);
+                }
+#else
+#pragma unroll 2
+                for (int g = g_lo; g <= g_hi; ++g) {
+                    const float4 v = xs4[g];
+                    const float xv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                    for (int q = 0; q < K2_NPOS; ++q)
+#pragma unroll
+                        for (int r = 0; r < 4; ++r) eval_weight(xv[r], kk[q], c0[q], nalpha, S[q], R[q]);
+                }
+#endif
+#pragma unroll
+                for (int q = 0; q < K2_NPOS; ++q) {
+#if UMI_K2_PACKED
+                    float s0, s1, r0, r1;
+                    unpack2(S2[q], s0, s1);
+                    unpack2(R2[q], r0, r1);
+                    S[q] += s0 + s1;
+                    R[q] += r0 + r1;
+#endif
+                    if (act[q] && S[q] > 0.f) mu[q] = fmaf(R[q] / S[q], cs[q], mu[q]);   /* Eq. 4; (R11) */
+                }
+            }
+        }
+
+#pragma unroll
+        for (int q = 0; q < K2_NPOS; ++q) {
+            const int64_t j = j0 + 4 * tid + q;
+            if (j < prm.N && med[q] == med[q]) orow[j] = mu[q];
+        }
+        __syncthreads();
+    }
+}
+
+} // namespace umi
