@@ -31,7 +31,7 @@ Geometry geometry_for(int W)
     while (ns < (W - 1) + (W - 1) / 2) ns <<= 1;
     g.NS = ns;
     g.T1 = ns - (W - 1);
-    g.smem1 = (size_t)ns * umi::K1_BYTES_PER_SLOT;
+    g.smem1 = umi::k1_smem_bytes(ns);
     const int h = (W - 1) / 2;
     const int hal = (h + 3) & ~3;
     const int G = (3 + (hal - h) + 2 * h) / 4 + 1;
@@ -82,15 +82,9 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
     mp.T = g.T1;
     mp.NS = g.NS;
     mp.min_valid = min_valid;
-    if (g.smem1 > 48 * 1024) {
-        if (cuda_failed(cudaFuncSetAttribute(umi::umi_median_kernel,
-                                             cudaFuncAttributeMaxDynamicSharedMemorySize, (int)g.smem1)))
-            return UMI_ERR_CUDA;
-    }
     const unsigned grid1 = (unsigned)std::min<int64_t>(mp.n_blocks, MAX_GRID);
     if (ev && cuda_failed(cudaEventRecord(ev[0], stream))) return UMI_ERR_CUDA;
-    umi::umi_median_kernel<<<grid1, umi::K1_THREADS, g.smem1, stream>>>(mp);
-    if (cuda_failed(cudaGetLastError())) return UMI_ERR_CUDA;
+    if (cuda_failed(umi::launch_median(mp, grid1, g.smem1, stream))) return UMI_ERR_CUDA;
     if (ev && cuda_failed(cudaEventRecord(ev[1], stream))) return UMI_ERR_CUDA;
 
     if (n_iter > 0) {
@@ -106,8 +100,7 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.alpha = alpha;
         rp.c = c;
         const unsigned grid2 = (unsigned)std::min<int64_t>(rp.n_blocks, MAX_GRID);
-        umi::umi_reweight_kernel<<<grid2, umi::K2_THREADS, g.smem2, stream>>>(rp);
-        if (cuda_failed(cudaGetLastError())) return UMI_ERR_CUDA;
+        if (cuda_failed(umi::launch_reweight(rp, grid2, g.smem2, stream))) return UMI_ERR_CUDA;
     }
     if (ev && cuda_failed(cudaEventRecord(ev[2], stream))) return UMI_ERR_CUDA;
     return UMI_OK;

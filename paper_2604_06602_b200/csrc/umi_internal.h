@@ -2,13 +2,24 @@
 #ifndef UMI_INTERNAL_H
 #define UMI_INTERNAL_H
 
+#include <cuda_runtime.h>
+#include <stddef.h>
 #include <stdint.h>
 
 namespace umi {
 
 constexpr int K1_THREADS = 256;                  /* median kernel */
 constexpr int K1_MIN_SORT = 1024;                /* smallest per-tile sort length */
-constexpr int K1_BYTES_PER_SLOT = 14;            /* u64 sort entry + f32 median + u16 rank */
+/* walkers per tile of the median kernel and its dynamic shared memory (bytes) */
+__host__ __device__ constexpr int k1_walkers(int ns) { return (131072 / ns) > 32 ? (131072 / ns) : 32; }
+__host__ __device__ constexpr size_t k1_smem_bytes(int ns)
+{
+    /* u64 sort entries + u16 ranks + max(rank bitsets [NW][NS/32+1] + scan offsets [NW/32][NS/32], f32 medians) */
+    const size_t bw = (size_t)ns / 32, nw = (size_t)k1_walkers(ns);
+    const size_t bits = 4 * (nw * (bw + 1) + (nw / 32) * bw);
+    const size_t med = 4 * (size_t)ns;
+    return (size_t)ns * 10 + (bits > med ? bits : med);
+}
 
 constexpr int K2_THREADS = 128;                  /* reweighting kernel */
 constexpr int K2_NPOS = 4;                       /* consecutive positions per thread */
@@ -35,8 +46,9 @@ struct ReweightParams {
     float alpha, c;
 };
 
-__global__ void umi_median_kernel(MedianParams prm);
-__global__ void umi_reweight_kernel(ReweightParams prm);
+/* Enqueue one kernel; return the launch status (cudaGetLastError). */
+cudaError_t launch_median(const MedianParams& prm, unsigned grid, size_t smem, cudaStream_t stream);
+cudaError_t launch_reweight(const ReweightParams& prm, unsigned grid, size_t smem, cudaStream_t stream);
 
 } // namespace umi
 

@@ -2,33 +2,134 @@
  * umi_median.cu -- Phase 1: exact sliding-window sample median.
  *
  * CTA = one star x one tile of T consecutive positions.  The T windows of a tile
- * live inside one union of U = T + W - 1 = NS samples.  The union is sorted ONCE
- * per tile (bitonic, 64-bit key|index), then each lane of one warp walks T/32
- * consecutive positions, keeping the union-rank of the current window's median:
- * a slide removes one sample and adds one, so the median moves by at most a
- * couple of included ranks.  Exact (the result is a selected sample);
- * O(log^2 U) per position for the sort plus O(1) expected per slide, instead of
- * O(W) per position for a per-thread quickselect (the paper's kernel).
- * Readings R1-R6, R16, R18 of DESIGN.md.  Nothing here is shared with oracle/.
+ * live inside one union of U = T + W - 1 = NS samples (NS a power of two).
+ *   1. sort the union ONCE per tile: bitonic network on 64-bit (key << 32 | index)
+ *      entries, E = NS/256 per thread -- strides < E in registers, strides < 32 E
+ *      with warp shuffles, only the top three strides through shared memory;
+ *   2. NW "walkers" (one thread each) own T/NW consecutive positions.  A walker's
+ *      first window is selected from a bitset of the union ranks it holds; the NW
+ *      bitsets are built together as an exclusive-or prefix scan over the entries
+ *      that leave / enter between consecutive walkers (2 T atomicXor per tile
+ *      instead of NW W), and the median is the k-th set bit (popcount + fns);
+ *   3. each walker then slides: one sample leaves, one enters, so the union rank of
+ *      the median moves by at most a couple of included ranks (O(1) expected).
+ * Exact: the result is a selected input sample.  O(log^2 U) per position for the
+ * sort instead of O(W) per position for a per-thread quickselect (the paper's
+ * kernel).  Readings R1-R6, R16, R18 of DESIGN.md.
+ * Nothing here is shared with oracle/.
  */
 #include "umi_device.cuh"
 
 namespace umi {
 
+namespace {
+
+
+__device__ __forceinline__ uint64_t shfl_xor_u64(uint64_t v, int mask)
+{
+    const uint32_t lo = __shfl_xor_sync(0xFFFFFFFFu, (uint32_t)v, mask);
+    const uint32_t hi = __shfl_xor_sync(0xFFFFFFFFu, (uint32_t)(v >> 32), mask);
+    return ((uint64_t)hi << 32) | lo;
+}
+
+__device__ __forceinline__ void cmp_swap(uint64_t& a, uint64_t& b, bool up)
+{
+    const bool sw = (a > b) == up;
+    const uint64_t lo = sw ? b : a, hi = sw ? a : b;
+    a = lo;
+    b = hi;
+}
+
+/* One bitonic stage (merge size K, stride J) on entries i = tid*E + e held in v[e] (blocked). */
+template <int E, int K, int J>
+__device__ __forceinline__ void bitonic_stage(uint64_t (&v)[E], uint64_t* srt, int tid)
+{
+    if constexpr (J < E) {
+        /* partner inside the thread */
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            if ((e & J) == 0) {
+                const bool up = (K < E) ? ((e & K) == 0) : (((tid * E) & K) == 0);
+                cmp_swap(v[e], v[e | J], up);
+            }
+        }
+    } else if constexpr (J < 32 * E) {
+        /* partner in another lane of the warp */
+        constexpr int LM = J / E;
+        const bool up = ((tid * E) & K) == 0;
+        const bool low = (tid & LM) == 0;
+        const bool keep_min = (low == up);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const uint64_t o = shfl_xor_u64(v[e], LM);
+            const bool take = (o < v[e]) == keep_min;               /* entries are unique: o != v[e] */
+            v[e] = take ? o : v[e];
+        }
+    } else {
+        /* partner in another warp: exchange through shared memory */
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < E; e += 2)
+            *reinterpret_cast<ulonglong2*>(srt + tid * E + e) = make_ulonglong2(v[e], v[e + 1]);
+        __syncthreads();
+        const bool up = ((tid * E) & K) == 0;
+        const bool low = ((tid * E) & J) == 0;
+        const bool keep_min = (low == up);
+        const uint64_t* other = srt + ((tid * E) ^ J);
+#pragma unroll
+        for (int e = 0; e < E; e += 2) {
+            const ulonglong2 o2 = *reinterpret_cast<const ulonglong2*>(other + e);
+            const bool t0 = (o2.x < v[e]) == keep_min;
+            const bool t1 = (o2.y < v[e + 1]) == keep_min;
+            v[e] = t0 ? o2.x : v[e];
+            v[e + 1] = t1 ? o2.y : v[e + 1];
+        }
+    }
+}
+
+template <int E, int K, int J>
+__device__ __forceinline__ void bitonic_merge(uint64_t (&v)[E], uint64_t* srt, int tid)
+{
+    if constexpr (J > 0) {
+        bitonic_stage<E, K, J>(v, srt, tid);
+        bitonic_merge<E, K, J / 2>(v, srt, tid);
+    }
+}
+
+/* Bitonic sort of NS = 256*E entries, ascending. */
+template <int E, int K = 2>
+__device__ __forceinline__ void bitonic_sort_blocked(uint64_t (&v)[E], uint64_t* srt, int tid)
+{
+    if constexpr (K <= K1_THREADS * E) {
+        bitonic_merge<E, K, K / 2>(v, srt, tid);
+        bitonic_sort_blocked<E, K * 2>(v, srt, tid);
+    }
+}
+
+} // namespace
+
+template <int E>
 __global__ void __launch_bounds__(K1_THREADS)
 umi_median_kernel(MedianParams prm)
 {
+    constexpr int NS = K1_THREADS * E;
+    constexpr int BW = NS / 32;                                     /* bitset words per walker */
+    constexpr int BWP = BW + 1;                                     /* padded row stride: conflict-free both ways */
+    constexpr int NW = k1_walkers(NS);                              /* walkers per tile */
+    constexpr int NWB = NW / 32;                                    /* walker blocks of 32 */
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    const int NS = prm.NS;
+    uint64_t* srt = reinterpret_cast<uint64_t*>(smem_raw);          /* [NS] key<<32 | union index, sorted */
+    uint16_t* rank = reinterpret_cast<uint16_t*>(srt + NS);         /* [NS] union index -> rank           */
+    uint32_t* bits = reinterpret_cast<uint32_t*>(rank + NS);        /* [NW][BWP] rank bitsets, then ...   */
+    uint32_t* boff = bits + NW * BWP;                               /* [NWB][BW] block offsets of the scan */
+    float* medbuf = reinterpret_cast<float*>(bits);                 /* ... aliased: [T] medians of the tile */
+    __shared__ int s_nvu;
+
     const int W = prm.W;
     const int T = prm.T;
     const int h = (W - 1) >> 1;
-    uint64_t* srt = reinterpret_cast<uint64_t*>(smem_raw);          /* [NS] key<<32 | union index */
-    float* medbuf = reinterpret_cast<float*>(srt + NS);             /* [NS] (first T used) */
-    uint16_t* rank = reinterpret_cast<uint16_t*>(medbuf + NS);      /* [NS] union index -> rank */
-    __shared__ int s_nvu;
-
     const int tid = threadIdx.x;
+    const int lane = tid & 31;
 
     for (int64_t bid = blockIdx.x; bid < prm.n_blocks; bid += gridDim.x) {
         const int64_t star = bid / prm.tiles_per_star;
@@ -41,114 +142,168 @@ umi_median_kernel(MedianParams prm)
         const double* trow = prm.time ? prm.time + star * prm.N : nullptr;
 
         if (tid == 0) s_nvu = 0;
-
-        /* stage: union index u <-> cadence jbase + u; U = T + W - 1 == NS */
-        for (int u = tid; u < NS; u += K1_THREADS) {
-            float x = 0.f;
-            bool ok = load_sample(trow, frow, prm.N, jbase + u, x);
-            uint32_t key = ok ? float_to_key(x) : KEY_INVALID;
-            srt[u] = ((uint64_t)key << 32) | (uint32_t)u;
-        }
+        for (int i = tid; i < NW * BWP + NWB * BW; i += K1_THREADS) bits[i] = 0u;
         __syncthreads();
 
-        /* bitonic sort, ascending; keys are unique because the index is part of them */
-        for (int k = 2; k <= NS; k <<= 1) {
-            for (int j = k >> 1; j > 0; j >>= 1) {
-                for (int t = tid; t < (NS >> 1); t += K1_THREADS) {
-                    const int i = ((t & ~(j - 1)) << 1) | (t & (j - 1));
-                    const int p = i | j;
-                    const bool up = ((i & k) == 0);
-                    const uint64_t a = srt[i], b = srt[p];
-                    if ((a > b) == up) { srt[i] = b; srt[p] = a; }
+        /* 1. load E consecutive union entries, sort */
+        uint64_t v[E];
+        int nvalid = 0;
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int u = tid * E + e;
+            float x = 0.f;
+            const bool ok = load_sample(trow, frow, prm.N, jbase + u, x);
+            nvalid += ok ? 1 : 0;
+            v[e] = ((uint64_t)(ok ? float_to_key(x) : KEY_INVALID) << 32) | (uint32_t)u;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) nvalid += __shfl_xor_sync(0xFFFFFFFFu, nvalid, o);
+        if (lane == 0 && nvalid) atomicAdd(&s_nvu, nvalid);
+
+        bitonic_sort_blocked<E>(v, srt, tid);
+
+        __syncthreads();
+#pragma unroll
+        for (int e = 0; e < E; e += 2)
+            *reinterpret_cast<ulonglong2*>(srt + tid * E + e) = make_ulonglong2(v[e], v[e + 1]);
+#pragma unroll
+        for (int e = 0; e < E; ++e) rank[(uint32_t)v[e]] = (uint16_t)(tid * E + e);
+        __syncthreads();
+        const int nvu = s_nvu;                                      /* valid entries = ranks [0, nvu) */
+
+        /* 2. walker w owns positions [w*Ts, (w+1)*Ts).  Bitset of the ranks in its first window:
+              row 0 = window of position 0; row w = (entries leaving) xor (entries entering) between the
+              starts of walkers w-1 and w; an exclusive-or prefix scan over w turns rows into bitsets. */
+        const int Ts = (Tact + NW - 1) / NW;
+        const int nwa = (Tact + Ts - 1) / Ts;                       /* active walkers */
+        const int span = (nwa - 1) * Ts;                            /* start of the last active walker */
+        const float inv_ts = 1.0f / (float)Ts;
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int u = tid * E + e;
+            const int r = rank[u];
+            if (r < nvu) {
+                const uint32_t bit = 1u << (r & 31);
+                const int wi = r >> 5;
+                if (u < W) atomicXor(&bits[wi], bit);
+                if (u < span) {
+                    int w = (int)((float)u * inv_ts);
+                    w += ((w + 1) * Ts <= u) ? 1 : 0;
+                    w -= (w * Ts > u) ? 1 : 0;
+                    atomicXor(&bits[(w + 1) * BWP + wi], bit);
                 }
-                __syncthreads();
+                const int ue = u - W;
+                if (ue >= 0 && ue < span) {
+                    int w = (int)((float)ue * inv_ts);
+                    w += ((w + 1) * Ts <= ue) ? 1 : 0;
+                    w -= (w * Ts > ue) ? 1 : 0;
+                    atomicXor(&bits[(w + 1) * BWP + wi], bit);
+                }
             }
         }
-
-        /* ranks and the number of valid samples in the union */
-        for (int r = tid; r < NS; r += K1_THREADS) {
-            const uint64_t e = srt[r];
-            rank[(uint32_t)e] = (uint16_t)r;
-            const bool v = (uint32_t)(e >> 32) != KEY_INVALID;
-            const bool vnext = (r + 1 < NS) && ((uint32_t)(srt[r + 1] >> 32) != KEY_INVALID);
-            if (v && !vnext) s_nvu = r + 1;
+        __syncthreads();
+        /* scan over walkers, one (block of 32 walkers, word column) pair per work item */
+        for (int item = tid; item < NWB * BW; item += K1_THREADS) {
+            const int col = item % BW, blk = item / BW;
+            uint32_t acc = 0u;
+            uint32_t* pcol = bits + (blk * 32) * BWP + col;
+#pragma unroll 8
+            for (int i = 0; i < 32; ++i) {
+                acc ^= pcol[i * BWP];
+                pcol[i * BWP] = acc;
+            }
+            boff[item] = acc;                                       /* block total, made exclusive below */
         }
         __syncthreads();
-        const int nvu = s_nvu;
+        if (NWB > 1) {
+            for (int col = tid; col < BW; col += K1_THREADS) {
+                uint32_t acc = 0u;
+                for (int blk = 0; blk < NWB; ++blk) {
+                    const uint32_t t = boff[blk * BW + col];
+                    boff[blk * BW + col] = acc;
+                    acc ^= t;
+                }
+            }
+        } else {
+            for (int col = tid; col < BW; col += K1_THREADS) boff[col] = 0u;
+        }
+        __syncthreads();
 
-        /* walk: one warp, lane w owns positions [w*Ts, (w+1)*Ts) of the tile */
-        if (tid < 32) {
-            const int Ts = (Tact + 31) >> 5;
-            int pbeg = tid * Ts;
+        /* first window of each walker: n = population of its bitset, median = k-th set bit */
+        int n = 0, rho = -1;
+        if (tid < nwa) {
+            const uint32_t* row = bits + tid * BWP;
+            const uint32_t* off = boff + (tid >> 5) * BW;
+#pragma unroll 4
+            for (int i = 0; i < BW; ++i) n += __popc(row[i] ^ off[i]);
+            if (n > 0) {
+                int need = (n - 1) >> 1;                            /* (R6) lower median */
+                for (int i = 0; i < BW; ++i) {
+                    const uint32_t word = row[i] ^ off[i];
+                    const int pc = __popc(word);
+                    if (need < pc) {
+                        rho = i * 32 + (int)__fns(word, 0, need + 1);
+                        break;
+                    }
+                    need -= pc;
+                }
+            }
+        }
+        __syncthreads();                                            /* bitsets are dead: medbuf reuses them */
+
+        /* 3. walk: a slide removes one entry and adds one */
+        if (tid < nwa) {
+            const int pbeg = tid * Ts;
             int pend = pbeg + Ts;
             if (pend > Tact) pend = Tact;
-            const bool lane_on = pbeg < pend;
-            if (!lane_on) pbeg = 0;
             const uint32_t uW = (uint32_t)W;
-
-            /* n = valid samples in window pbeg = union [pbeg, pbeg + W) */
-            int n = 0;
-            for (int t = 0; t < W; ++t) n += (rank[pbeg + t] < nvu) ? 1 : 0;
-            const int k0 = (n - 1) >> 1;                            /* (R6) lower median */
-            int rho = -1;
-            {
-                int acc = 0;
-                for (int r = 0; r < nvu; ++r) {
-                    const uint32_t u = (uint32_t)srt[r];
-                    const bool inc = (u - (uint32_t)pbeg) < uW;
-                    acc += inc ? 1 : 0;
-                    if (inc && acc == k0 + 1) rho = r;
-                }
-            }
-            if (lane_on) {
-                int p = pbeg;
-                for (;;) {
-                    /* emit position p (R4, R5) */
-                    const bool own = rank[p + h] < nvu;
-                    float m = __int_as_float(0x7FC00000);
-                    if (own && n >= prm.min_valid && n > 0)
-                        m = key_to_float((uint32_t)(srt[rho] >> 32));
-                    medbuf[p] = m;
-                    if (++p >= pend) break;
-                    /* slide to window p: union index p-1 leaves, p+W-1 enters */
-                    const int ro = rank[p - 1], ri = rank[p + W - 1];
-                    const bool vo = ro < nvu, vi = ri < nvu;
-                    const int n2 = n - (vo ? 1 : 0) + (vi ? 1 : 0);
-                    if (n2 == 0) {
-                        rho = -1;
-                    } else if (n == 0) {
-                        rho = ri;
-                    } else {
-                        const int k2 = (n2 - 1) >> 1;
-                        int below = ((n - 1) >> 1) - ((vo && ro < rho) ? 1 : 0) + ((vi && ri < rho) ? 1 : 0);
-                        const uint32_t up = (uint32_t)p;
-                        if (vo && ro == rho) {
-                            int r = rho + 1;
-                            while (r < nvu && ((uint32_t)srt[r] - up) >= uW) ++r;
-                            if (r < nvu) {
-                                rho = r;
-                            } else {
-                                r = rho - 1;
-                                while (r > 0 && ((uint32_t)srt[r] - up) >= uW) --r;
-                                rho = r;
-                                --below;
-                            }
-                        }
-                        while (below > k2) {
-                            int r = rho - 1;
+            int p = pbeg;
+            for (;;) {
+                /* emit position p (R4, R5) */
+                const bool own = rank[p + h] < nvu;
+                float m = __int_as_float(0x7FC00000);
+                if (own && n >= prm.min_valid && n > 0)
+                    m = key_to_float((uint32_t)(srt[rho] >> 32));
+                medbuf[p] = m;
+                if (++p >= pend) break;
+                /* slide to window p: union index p-1 leaves, p+W-1 enters */
+                const int ro = rank[p - 1], ri = rank[p + W - 1];
+                const bool vo = ro < nvu, vi = ri < nvu;
+                const int n2 = n - (vo ? 1 : 0) + (vi ? 1 : 0);
+                if (n2 == 0) {
+                    rho = -1;
+                } else if (n == 0) {
+                    rho = ri;
+                } else {
+                    const int k2 = (n2 - 1) >> 1;
+                    int below = ((n - 1) >> 1) - ((vo && ro < rho) ? 1 : 0) + ((vi && ri < rho) ? 1 : 0);
+                    const uint32_t up = (uint32_t)p;
+                    if (vo && ro == rho) {                          /* the median itself left */
+                        int r = rho + 1;
+                        while (r < nvu && ((uint32_t)srt[r] - up) >= uW) ++r;
+                        if (r < nvu) {
+                            rho = r;
+                        } else {
+                            r = rho - 1;
                             while (r > 0 && ((uint32_t)srt[r] - up) >= uW) --r;
                             rho = r;
                             --below;
                         }
-                        while (below < k2) {
-                            int r = rho + 1;
-                            while (r < nvu - 1 && ((uint32_t)srt[r] - up) >= uW) ++r;
-                            rho = r;
-                            ++below;
-                        }
                     }
-                    n = n2;
+                    while (below > k2) {
+                        int r = rho - 1;
+                        while (r > 0 && ((uint32_t)srt[r] - up) >= uW) --r;
+                        rho = r;
+                        --below;
+                    }
+                    while (below < k2) {
+                        int r = rho + 1;
+                        while (r < nvu - 1 && ((uint32_t)srt[r] - up) >= uW) ++r;
+                        rho = r;
+                        ++below;
+                    }
                 }
+                n = n2;
             }
         }
         __syncthreads();
@@ -157,6 +312,24 @@ umi_median_kernel(MedianParams prm)
         for (int p = tid; p < Tact; p += K1_THREADS) orow[p] = medbuf[p];
         __syncthreads();
     }
+}
+
+cudaError_t launch_median(const MedianParams& prm, unsigned grid, size_t smem, cudaStream_t stream)
+{
+    void (*k1)(MedianParams) = nullptr;
+    switch (prm.NS / K1_THREADS) {
+    case 4: k1 = umi_median_kernel<4>; break;
+    case 8: k1 = umi_median_kernel<8>; break;
+    case 16: k1 = umi_median_kernel<16>; break;
+    case 32: k1 = umi_median_kernel<32>; break;
+    default: return cudaErrorInvalidValue;
+    }
+    if (smem > 48 * 1024) {
+        const cudaError_t e = cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    k1<<<grid, K1_THREADS, smem, stream>>>(prm);
+    return cudaGetLastError();
 }
 
 } // namespace umi

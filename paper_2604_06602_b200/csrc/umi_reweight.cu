@@ -317,4 +317,10 @@ umi_reweight_kernel(ReweightParams prm)
     }
 }
 
+cudaError_t launch_reweight(const ReweightParams& prm, unsigned grid, size_t smem, cudaStream_t stream)
+{
+    umi_reweight_kernel<<<grid, K2_THREADS, smem, stream>>>(prm);
+    return cudaGetLastError();
+}
+
 } // namespace umi

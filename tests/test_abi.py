@@ -85,7 +85,7 @@ def test_launch_geometry():
         assert NS & (NS - 1) == 0 and NS >= 1024
         assert T + W - 1 == NS
         assert T >= max(1, (W - 1) // 2)
-        assert NS * 14 <= 227 * 1024
+        assert NS * 14 <= 227 * 1024  # sort entries + ranks + bitsets
         assert T2 == 512
     assert umi.umi_launch_geometry(361)[:2] == (664, 1024)
     with pytest.raises(umi.UmiError):
