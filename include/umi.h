@@ -97,10 +97,13 @@ int umi_detrend_ex(const double* time, const float* flux,
 /*
  * Batch driver (the paper streams 50-star batches): the same
  * computation with HOST buffers.  Stars are cut into batches of
- * `stars_per_batch` (<= 0: chosen so that a batch is about 64 MiB of flux),
- * and host->device copy, kernels and device->host copy of successive batches
- * are pipelined over `n_streams` CUDA streams (<= 0: 3) with one device buffer
- * set per stream, allocated and freed inside the call.
+ * `stars_per_batch` (<= 0: at most ~16 MiB of flux per batch and at least 4
+ * batches per stream when the job is large enough), and host->device copy,
+ * kernels and device->host copy of successive batches are pipelined over
+ * `n_streams` CUDA streams (<= 0: 3) with one device buffer set per stream,
+ * allocated and freed inside the call with cudaMallocAsync / cudaFreeAsync
+ * (the call raises the release threshold of the device's default memory pool
+ * to 1 GiB so that repeated calls reuse the buffers).
  *
  *   time, flux, trend_out   HOST pointers, same shapes as above; time may be NULL.
  * The call returns after every batch has been copied back (it synchronises).

@@ -171,7 +171,11 @@ int umi_detrend_host(const double* time, const float* flux, int64_t n_stars, int
     if (n_streams > 16) n_streams = 16;
     if (stars_per_batch <= 0) {
         const int64_t row_bytes = n_cadences * (int64_t)sizeof(float);
-        stars_per_batch = std::max<int64_t>(1, (64ll << 20) / std::max<int64_t>(row_bytes, 1));
+        /* ~16 MiB of flux per batch, but at least 4 batches per stream when the job allows it */
+        stars_per_batch = std::max<int64_t>(1, (16ll << 20) / std::max<int64_t>(row_bytes, 1));
+        const int64_t by_count = (n_stars + 4 * n_streams - 1) / (4 * n_streams);
+        const int64_t floor_b = std::max<int64_t>(1, (2ll << 20) / std::max<int64_t>(row_bytes, 1));
+        stars_per_batch = std::max(floor_b, std::min(stars_per_batch, by_count));
     }
     stars_per_batch = std::min(stars_per_batch, n_stars);
     const int64_t n_batches = (n_stars + stars_per_batch - 1) / stars_per_batch;
@@ -184,14 +188,29 @@ int umi_detrend_host(const double* time, const float* flux, int64_t n_stars, int
         double* d_time = nullptr;
     };
     std::vector<Slot> slots((size_t)n_streams);
+    {
+        /* keep the per-call buffers in the driver's stream-ordered pool between calls (up to 1 GiB) */
+        int dev = 0;
+        cudaMemPool_t pool = nullptr;
+        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            uint64_t thr = 0;
+            if (cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr) == cudaSuccess &&
+                thr < (1ull << 30)) {
+                thr = 1ull << 30;
+                (void)cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+            }
+        }
+        (void)cudaGetLastError();
+    }
     const size_t elems = (size_t)stars_per_batch * (size_t)n_cadences;
     int status = UMI_OK;
 
     for (auto& s : slots) {
         if (cuda_failed(cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking)) ||
-            cuda_failed(cudaMalloc(&s.d_flux, elems * sizeof(float))) ||
-            cuda_failed(cudaMalloc(&s.d_trend, elems * sizeof(float))) ||
-            (time != nullptr && cuda_failed(cudaMalloc(&s.d_time, elems * sizeof(double))))) {
+            /* stream-ordered allocations: served from the driver's pool after the first call */
+            cuda_failed(cudaMallocAsync((void**)&s.d_flux, elems * sizeof(float), s.stream)) ||
+            cuda_failed(cudaMallocAsync((void**)&s.d_trend, elems * sizeof(float), s.stream)) ||
+            (time != nullptr && cuda_failed(cudaMallocAsync((void**)&s.d_time, elems * sizeof(double), s.stream)))) {
             status = UMI_ERR_CUDA;
             break;
         }
@@ -217,12 +236,13 @@ int umi_detrend_host(const double* time, const float* flux, int64_t n_stars, int
     }
 
     for (auto& s : slots) {
-        if (s.stream != nullptr && cuda_failed(cudaStreamSynchronize(s.stream))) status = UMI_ERR_CUDA;
+        if (s.stream == nullptr) continue;
+        if (s.d_flux) (void)cudaFreeAsync(s.d_flux, s.stream);
+        if (s.d_trend) (void)cudaFreeAsync(s.d_trend, s.stream);
+        if (s.d_time) (void)cudaFreeAsync(s.d_time, s.stream);
+        if (cuda_failed(cudaStreamSynchronize(s.stream))) status = UMI_ERR_CUDA;
     }
     for (auto& s : slots) {
-        if (s.d_flux) (void)cudaFree(s.d_flux);
-        if (s.d_trend) (void)cudaFree(s.d_trend);
-        if (s.d_time) (void)cudaFree(s.d_time);
         if (s.stream) (void)cudaStreamDestroy(s.stream);
     }
     (void)cudaGetLastError();
