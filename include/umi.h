@@ -118,7 +118,9 @@ int umi_detrend_host(const double* time, const float* flux,
  * Measurement aid: umi_detrend_ex, plus the device time of each of its two
  * kernels taken with CUDA events recorded on `stream` around each launch.
  *   kernel_ms  HOST, float[2]: [0] Phase-1 median kernel, [1] Phase-2/3
- *              reweighting kernel (0 when n_iter == 0), milliseconds.
+ *              reweighting kernel (0 when n_iter == 0), milliseconds.  Windows of
+ *              at most 49 samples run all phases in one fused kernel: its time is
+ *              reported in [1] and [0] is ~0.
  * Unlike umi_detrend this call SYNCHRONISES `stream` before returning.
  */
 int umi_detrend_profile(const double* time, const float* flux,

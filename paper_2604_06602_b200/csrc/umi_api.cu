@@ -71,6 +71,28 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
     const Geometry g = geometry_for(W);
     if (min_valid < 0) min_valid = std::max(1, W / 3);      /* PAPER.md:192 (R4) */
 
+    if (W <= umi::KS_MAX_WINDOW) {
+        /* short windows: all three phases in one register-resident kernel (umi_small.cu) */
+        umi::ReweightParams rp;
+        rp.time = time;
+        rp.flux = flux;
+        rp.out = trend_out;
+        rp.N = n_cadences;
+        rp.tiles_per_star = (n_cadences + umi::KS_THREADS - 1) / umi::KS_THREADS;
+        rp.n_blocks = n_stars * rp.tiles_per_star;
+        rp.W = W;
+        rp.n_iter = n_iter;
+        rp.alpha = alpha;
+        rp.c = c;
+        const int wt = W <= 9 ? 9 : W <= 17 ? 17 : W <= 25 ? 25 : W <= 33 ? 33 : 49;
+        const unsigned grid = (unsigned)std::min<int64_t>(rp.n_blocks, MAX_GRID);
+        if (ev && (cuda_failed(cudaEventRecord(ev[0], stream)) || cuda_failed(cudaEventRecord(ev[1], stream))))
+            return UMI_ERR_CUDA;
+        if (cuda_failed(umi::launch_small(rp, min_valid, wt, grid, stream))) return UMI_ERR_CUDA;
+        if (ev && cuda_failed(cudaEventRecord(ev[2], stream))) return UMI_ERR_CUDA;
+        return UMI_OK;
+    }
+
     umi::MedianParams mp;
     mp.time = time;
     mp.flux = flux;

@@ -21,6 +21,9 @@ __host__ __device__ constexpr size_t k1_smem_bytes(int ns)
     return (size_t)ns * 10 + (bits > med ? bits : med);
 }
 
+constexpr int KS_THREADS = 256;                  /* fused small-window kernel: one position per thread */
+constexpr int KS_MAX_WINDOW = 49;                /* windows up to this length take the fused kernel */
+
 constexpr int K2_THREADS = 128;                  /* reweighting kernel */
 constexpr int K2_NPOS = 4;                       /* consecutive positions per thread */
 constexpr int K2_TILE = K2_THREADS * K2_NPOS;    /* positions per CTA */
@@ -49,6 +52,8 @@ struct ReweightParams {
 /* Enqueue one kernel; return the launch status (cudaGetLastError). */
 cudaError_t launch_median(const MedianParams& prm, unsigned grid, size_t smem, cudaStream_t stream);
 cudaError_t launch_reweight(const ReweightParams& prm, unsigned grid, size_t smem, cudaStream_t stream);
+/* fused kernel for W <= KS_MAX_WINDOW; wt = compiled wire count (9, 17, 25, 33 or 49) >= W */
+cudaError_t launch_small(const ReweightParams& prm, int min_valid, int wt, unsigned grid, cudaStream_t stream);
 
 } // namespace umi
 

@@ -48,7 +48,7 @@ def _both(umi, flux, W, alpha=2.0, n_iter=5, time=None, c=None, min_valid=None):
 
 
 # ------------------------------------------------------------------ small, every position
-@pytest.mark.parametrize("W", [1, 3, 5, 7, 9, 25, 51, 217, 361, 513, 515, 1081])
+@pytest.mark.parametrize("W", [1, 3, 5, 7, 9, 11, 17, 19, 25, 27, 33, 35, 49, 51, 217, 361, 513, 515, 1081])
 def test_random_series_with_gaps_and_inf(umi, W):
     # 3 stars x 3001 cadences: several tiles of both kernels and a ragged tail
     x = lc.random_series(W, 3, 3001)
