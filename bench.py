@@ -130,6 +130,17 @@ def peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
+def ncu_traffic(config_id, n_stars):
+    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the
+    committed ncu --set full capture (profiles/traffic_r01.json); None for any other workload."""
+    path = os.path.join(ROOT, "profiles", "traffic_r01.json")
+    if config_id != 2 or n_stars != 1000 or not os.path.exists(path):
+        return None
+    with open(path) as f:
+        k = json.load(f)["kernels"].get("umi_reweight_kernel")
+    return None if k is None else k["dram_bytes_read"] + k["dram_bytes_write"]
+
+
 def oracle_sample(cfg, flux, n_stars):
     """Times the fp64 oracle, as it stands, on the first n_stars stars of the workload."""
     from oracle import umi_oracle as orc
@@ -283,8 +294,10 @@ def run_ours(args, cfg, rank, world, local_rank):
         "kernel_ms": rw_ms, "median_kernel_ms": med_ms, "kernel_share_of_step": rw_ms / (rw_ms + med_ms),
         "window_samples_per_s": ws_exact / (ms_per_step * 1e-3),
         "hbm_algorithmic_GBps": 8.0 * S * N / (ms_per_step * 1e-3) / 1e9, "hbm_peak_GBps": pk.get("hbm_gbs"),
-        "traffic": None,
+        "traffic": ncu_traffic(args.config, S),
     }
+    if W <= 49:
+        roofline["kernel"] = "umi_small_kernel (fused phases 1-3)"
     cpu = None
     if not args.no_cpu_baseline:
         rate, _, cores = oracle_sample(cfg, flux_np, min(S, 16))
