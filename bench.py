@@ -122,6 +122,21 @@ class ClockSampler(threading.Thread):
                 "samples": len(self.samples)}
 
 
+def shard_stars(rank, world, stars_per_rank):
+    """Weak scaling: rank r owns the separately seeded stars [r*S, (r+1)*S); no data-path collective."""
+    return range(rank * stars_per_rank, (rank + 1) * stars_per_rank)
+
+
+def max_over_ranks(value, dist, device=None):
+    """Max over ranks of a host scalar (timings); identity when not distributed."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([float(value)], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
 def peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -197,7 +212,7 @@ def run_ours(args, cfg, rank, world, local_rank):
 
     S = cfg.n_stars if args.stars is None else args.stars
     N, W = cfg.n_cadences, cfg.W
-    flux_np = lc.stars(args.config, range(rank * S, (rank + 1) * S))     # weak scaling: own stars
+    flux_np = lc.stars(args.config, shard_stars(rank, world, S))          # weak scaling: own stars
     min_valid = max(1, W // 3)
     ws_exact = exact_window_samples(flux_np, W, min_valid)
     h_flux = torch.from_numpy(flux_np).pin_memory()
@@ -244,11 +259,7 @@ def run_ours(args, cfg, rank, world, local_rank):
     clocks = sampler.stop()
     if dist is not None:
         dist.barrier()
-    total_ms = float(sum(step_ms))
-    if dist is not None:
-        t = torch.tensor([total_ms], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(sum(step_ms), dist, dev)
 
     # ---- end to end through the public host API: pinned host buffers in, pinned host out
     e2e = None
@@ -260,11 +271,7 @@ def run_ours(args, cfg, rank, world, local_rank):
         t0 = time.perf_counter()
         for _ in range(args.steps):
             umi.umi_detrend_host(None, h_flux, W, alpha=cfg.alpha, n_iter=cfg.n_iter, out=h_out)
-        e2e_s = time.perf_counter() - t0
-        if dist is not None:
-            t = torch.tensor([e2e_s], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_s = float(t.item())
+        e2e_s = max_over_ranks(time.perf_counter() - t0, dist, dev)
         e2e = {"value": world * S * N * args.steps / e2e_s, "unit": UNIT,
                "h2d_bytes_per_step": int(h_flux.numel() * 4), "d2h_bytes_per_step": int(h_out.numel() * 4),
                "ms_per_step": 1e3 * e2e_s / args.steps,

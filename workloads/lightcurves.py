@@ -145,7 +145,8 @@ def stars(config_id, indices, workers=None):
     if workers <= 1 or total < 4_000_000:
         return _stars_chunk((config_id, indices))
     chunks = [c for c in np.array_split(np.asarray(indices), min(len(indices), workers * 4)) if len(c)]
-    with concurrent.futures.ProcessPoolExecutor(max_workers=workers) as ex:
+    import multiprocessing
+    with concurrent.futures.ProcessPoolExecutor(max_workers=workers, mp_context=multiprocessing.get_context("spawn")) as ex:
         parts = list(ex.map(_stars_chunk, [(config_id, c.tolist()) for c in chunks]))
     return np.concatenate(parts, axis=0)
 
