@@ -74,3 +74,34 @@ def detrend(flux, W, alpha=2.0, n_iter=5, c=5.0, time=None, min_valid=None):
                 continue
             trend[b, i], median[b, i], scale[b, i] = location(x, alpha, c, n_iter)
     return trend, median, scale
+
+
+def detrend_gapped(time, flux, t0, dt, n_grid, W, alpha=2.0, n_iter=5, c=5.0, min_valid=None):
+    """Brute force for compacted rows with time stamps (PAPER.md:155 gap handling, reading
+    R20): slot = rint((t - t0)/dt); a sample is valid iff time and flux are finite, its slot is
+    inside [0, n_grid) and the next sample of the row has a different slot; its window is the
+    valid samples whose slot differs from its own by at most h.  Whole-row boolean masks."""
+    time = np.atleast_2d(np.asarray(time, dtype=np.float64))
+    flux = np.atleast_2d(np.asarray(flux, dtype=np.float32))
+    S, M = flux.shape
+    h = (W - 1) // 2
+    if min_valid is None:
+        min_valid = max(1, W // 3)
+    trend = np.full((S, M), np.nan)
+    median = np.full((S, M), np.nan)
+    for b in range(S):
+        with np.errstate(invalid="ignore"):
+            k = np.rint((time[b] - t0) / dt)
+        ok = np.isfinite(time[b]) & (k >= 0) & (k < n_grid)
+        same_as_next = np.zeros(M, dtype=bool)
+        same_as_next[:-1] = np.isfinite(time[b, :-1]) & np.isfinite(time[b, 1:]) & (k[:-1] == k[1:])
+        ok &= ~same_as_next
+        ok &= np.isfinite(flux[b])
+        for i in range(M):
+            if not ok[i]:
+                continue
+            x = flux[b][ok & (np.abs(k - k[i]) <= h)].astype(np.float64)
+            if x.size < min_valid:
+                continue
+            trend[b, i], median[b, i], _ = location(x, alpha, c, n_iter)
+    return trend, median

@@ -77,32 +77,25 @@ static int slot_valid(const double *time, const float *flux, int64_t N, int64_t 
 }
 
 /*
- * One window: star row (time, flux) of length N, position i.
- * Outputs (any may be NULL): trend (double), median (float), scale s, n valid,
- * n_plus, near_cutoff flag.  work[] must hold 2*W doubles.
- * Returns 1 if a trend value was produced, 0 if the output is NaN.
+ * The estimator on the n valid samples x[0..n) of one window.
+ * own_valid = the position's own slot is valid.  Outputs (any may be NULL): trend
+ * (double), median (float), scale s, n_plus, near_cutoff flag.  sorted[] must
+ * hold n doubles.  Returns 1 if a trend value was produced, 0 if the output is NaN.
  */
-static int oracle_window(const double *time, const float *flux, int64_t N, int64_t i,
-                         int W, double alpha, double c, int n_iter, int min_valid,
-                         double cutoff_tol, double *work,
-                         double *trend, float *median, double *scale,
-                         int32_t *n_valid, int32_t *n_plus_out, uint8_t *near_cutoff)
+static int oracle_location(const double *x, int n, int own_valid,
+                           double alpha, double c, int n_iter, int min_valid,
+                           double cutoff_tol, double *sorted,
+                           double *trend, float *median, double *scale,
+                           int32_t *n_plus_out, uint8_t *near_cutoff)
 {
-    const int64_t h = (W - 1) / 2;                    /* (R1) centred window [i-h, i+h] */
-    double *x = work, *sorted = work + W;
-    int n = 0;
-    for (int64_t j = i - h; j <= i + h; ++j)
-        if (slot_valid(time, flux, N, j)) x[n++] = (double)flux[j];   /* exact widening */
-
     if (trend) *trend = NAN;
     if (median) *median = NAN;
     if (scale) *scale = NAN;
-    if (n_valid) *n_valid = n;
     if (n_plus_out) *n_plus_out = 0;
     if (near_cutoff) *near_cutoff = 0;
 
     /* (R4) PAPER.md:192 minimum length W/3; (R5) invalid own slot -> NaN */
-    if (!slot_valid(time, flux, N, i) || n < min_valid) return 0;
+    if (!own_valid || n < min_valid || n < 1) return 0;
 
     /* Phase 1: the exact sample median.  Definition written out:
      * sort ascending, take rank k = (n-1)/2 (R6: lower middle when n is even). */
@@ -152,6 +145,28 @@ static int oracle_window(const double *time, const float *flux, int64_t N, int64
     if (trend) *trend = mu;
     if (near_cutoff) *near_cutoff = (uint8_t)flagged;
     return 1;
+}
+
+/*
+ * One window: star row (time, flux) of length N, position i.
+ * Outputs (any may be NULL): trend (double), median (float), scale s, n valid,
+ * n_plus, near_cutoff flag.  work[] must hold 2*W doubles.
+ * Returns 1 if a trend value was produced, 0 if the output is NaN.
+ */
+static int oracle_window(const double *time, const float *flux, int64_t N, int64_t i,
+                         int W, double alpha, double c, int n_iter, int min_valid,
+                         double cutoff_tol, double *work,
+                         double *trend, float *median, double *scale,
+                         int32_t *n_valid, int32_t *n_plus_out, uint8_t *near_cutoff)
+{
+    const int64_t h = (W - 1) / 2;                    /* (R1) centred window [i-h, i+h] */
+    double *x = work, *sorted = work + W;
+    int n = 0;
+    for (int64_t j = i - h; j <= i + h; ++j)
+        if (slot_valid(time, flux, N, j)) x[n++] = (double)flux[j];   /* exact widening */
+    if (n_valid) *n_valid = n;
+    return oracle_location(x, n, slot_valid(time, flux, N, i), alpha, c, n_iter, min_valid,
+                           cutoff_tol, sorted, trend, median, scale, n_plus_out, near_cutoff);
 }
 
 static int resolve_min_valid(int W, int min_valid)
@@ -246,6 +261,106 @@ int umi_oracle_detrend(const double *time, const float *flux,
         }
         free(work);
     }
+    return bad;
+}
+
+/*
+ * Normalisation stage ("detrending, normalization"): flat = flux / trend,
+ * one division per cadence in fp64 (fp32 flux widened exactly); NaN where trend is NaN.
+ */
+int umi_oracle_normalize(const float *flux, const double *trend64, int64_t count, double *flat64)
+{
+    if (!flux || !trend64 || !flat64 || count < 0) return 1;
+    for (int64_t q = 0; q < count; ++q) flat64[q] = (double)flux[q] / trend64[q];
+    return 0;
+}
+
+/*
+ * Gap handling by time stamps ("gap handling"; reading R20): the
+ * rows are COMPACTED series (cadences were removed, so time jumps) of n_samples samples
+ * with real time stamps.  Sample (b, i) sits in slot k_i = rint((time[i] - t0) / dt)
+ * (round half to even) of a uniform grid of n_grid slots; it is valid iff time and flux
+ * are finite, 0 <= k_i < n_grid, and the NEXT sample of the row does not map to the same
+ * slot.  Its window is the valid samples j of the same row with |k_j - k_i| <= h: W slots
+ * of fixed duration W*dt, exactly what the positional window of PAPER.md:35 spans on an
+ * uncompacted series.  Times are assumed non-decreasing along a row, so only samples
+ * j in [i-h, i+h] can qualify.  Outputs as umi_oracle_detrend, [n_stars, n_samples].
+ */
+int umi_oracle_gapped(const double *time, const float *flux,
+                      int64_t n_stars, int64_t n_samples,
+                      double t0, double dt, int64_t n_grid,
+                      int W, double alpha, double c, int n_iter, int min_valid,
+                      double cutoff_tol,
+                      double *trend64, float *trend32, float *median,
+                      double *scale, int32_t *n_valid, int32_t *n_plus,
+                      uint8_t *near_cutoff)
+{
+    if (!time || !flux || n_stars < 0 || n_samples < 0 || n_grid < 0 || W < 1 || (W & 1) == 0 ||
+        n_iter < 0 || !(alpha > 0.0) || !(c > 0.0) || !(dt > 0.0) || !isfinite(dt) || !isfinite(t0))
+        return 1;
+    const int mv = resolve_min_valid(W, min_valid);
+    const int64_t h = (W - 1) / 2;
+    const int64_t total = n_stars * n_samples;
+    int64_t *slot = (int64_t *)malloc((size_t)(total > 0 ? total : 1) * sizeof(int64_t));
+    if (!slot) return 1;
+    /* slot of every sample, -1 = invalid */
+    for (int64_t b = 0; b < n_stars; ++b) {
+        const double *trow = time + b * n_samples;
+        const float *frow = flux + b * n_samples;
+        int64_t *srow = slot + b * n_samples;
+        for (int64_t i = 0; i < n_samples; ++i) {
+            srow[i] = -1;
+            if (!isfinite(trow[i])) continue;
+            double k = rint((trow[i] - t0) / dt);
+            if (!(k >= 0.0) || !(k < (double)n_grid)) continue;
+            srow[i] = (int64_t)k;
+        }
+        for (int64_t i = 0; i < n_samples; ++i) {
+            int64_t k = srow[i];
+            /* a sample that shares its slot with its successor is dropped */
+            if (k >= 0 && i + 1 < n_samples && isfinite(trow[i + 1])) {
+                double kn = rint((trow[i + 1] - t0) / dt);
+                if (kn == (double)k) srow[i] = -1;
+            }
+        }
+        for (int64_t i = 0; i < n_samples; ++i)
+            if (!isfinite(frow[i])) srow[i] = -1;
+    }
+    int bad = 0;
+#pragma omp parallel
+    {
+        double *work = (double *)malloc((size_t)2 * (size_t)W * sizeof(double));
+#pragma omp for schedule(dynamic, 256)
+        for (int64_t q = 0; q < total; ++q) {
+            if (!work) {
+#pragma omp atomic write
+                bad = 1;
+                continue;
+            }
+            const int64_t b = q / n_samples, i = q % n_samples;
+            const float *frow = flux + b * n_samples;
+            const int64_t *srow = slot + b * n_samples;
+            const int64_t ki = srow[i];
+            int n = 0;
+            if (ki >= 0) {
+                for (int64_t j = i - h; j <= i + h; ++j) {
+                    if (j < 0 || j >= n_samples || srow[j] < 0) continue;
+                    int64_t d = srow[j] - ki;
+                    if (d < 0) d = -d;
+                    if (d <= h) work[n++] = (double)frow[j];
+                }
+            }
+            if (n_valid) n_valid[q] = n;
+            double t64;
+            oracle_location(work, n, ki >= 0, alpha, c, n_iter, mv, cutoff_tol, work + W,
+                            &t64, median ? median + q : NULL, scale ? scale + q : NULL,
+                            n_plus ? n_plus + q : NULL, near_cutoff ? near_cutoff + q : NULL);
+            if (trend64) trend64[q] = t64;
+            if (trend32) trend32[q] = (float)t64;
+        }
+        free(work);
+    }
+    free(slot);
     return bad;
 }
 

@@ -57,6 +57,14 @@ def lib():
             _c_i64_p, _c_i64_p, ctypes.c_int64,
             ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
             ctypes.c_double] + outs
+        L.umi_oracle_normalize.restype = ctypes.c_int
+        L.umi_oracle_normalize.argtypes = [_c_float_p, _c_double_p, ctypes.c_int64, _c_double_p]
+        L.umi_oracle_gapped.restype = ctypes.c_int
+        L.umi_oracle_gapped.argtypes = [
+            _c_double_p, _c_float_p, ctypes.c_int64, ctypes.c_int64,
+            ctypes.c_double, ctypes.c_double, ctypes.c_int64,
+            ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
+            ctypes.c_double] + outs
         _lib = L
     return _lib
 
@@ -136,4 +144,35 @@ def positions(flux, star_idx, pos_idx, W, alpha=2.0, n_iter=5, c=5.0, time=None,
         *_out_ptrs(r))
     if rc != 0:
         raise ValueError("umi_oracle_positions: invalid arguments")
+    return r
+
+
+def normalize(flux, trend64):
+    """PAPER.md:155 normalisation stage: flat = flux / trend in fp64, flux's shape."""
+    flux = np.ascontiguousarray(flux, dtype=np.float32)
+    trend64 = np.ascontiguousarray(trend64, dtype=np.float64)
+    if flux.size != trend64.size:
+        raise ValueError("flux and trend must have the same size")
+    flat = np.empty(flux.shape, np.float64)
+    rc = lib().umi_oracle_normalize(flux.ctypes.data_as(_c_float_p), trend64.ctypes.data_as(_c_double_p),
+                                    flux.size, flat.ctypes.data_as(_c_double_p))
+    if rc != 0:
+        raise ValueError("umi_oracle_normalize: invalid arguments")
+    return flat
+
+
+def gapped(time, flux, t0, dt, n_grid, W, alpha=2.0, n_iter=5, c=5.0, min_valid=-1,
+           cutoff_tol=1e-5) -> OracleResult:
+    """Compacted rows with real time stamps (gap handling; reading R20):
+    the window of a sample is the valid samples within +-h grid slots of its own slot."""
+    flux, time, tp = _prep(flux, time)
+    if tp is None:
+        raise ValueError("time is required")
+    S, M = flux.shape
+    r = _alloc((S, M))
+    rc = lib().umi_oracle_gapped(
+        tp, flux.ctypes.data_as(_c_float_p), S, M, float(t0), float(dt), int(n_grid),
+        int(W), float(alpha), float(c), int(n_iter), int(min_valid), float(cutoff_tol), *_out_ptrs(r))
+    if rc != 0:
+        raise ValueError("umi_oracle_gapped: invalid arguments")
     return r

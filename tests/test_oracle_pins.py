@@ -405,3 +405,66 @@ def test_near_cutoff_flag():
     assert r.near_cutoff[0] == 0
     r = orc.positions(x, [0], [2], W=5, cutoff_tol=0.3)   # pass-1 u_eff = -0.75 is within 0.3 of -1
     assert r.near_cutoff[0] == 1
+
+
+# ---------------------------------------------------------------- next rows: F1 normalisation, F2 gap handling
+def test_normalize_is_flux_over_trend():
+    # PAPER.md:155 "normalization": flat * trend = flux; a constant series flattens to exactly 1
+    from workloads import lightcurves as lc
+    x = lc.random_series(3, 2, 400)
+    r = orc.detrend(x, 25)
+    flat = orc.normalize(x, r.trend64)
+    ok = ~np.isnan(r.trend64)
+    assert np.array_equal(np.isnan(flat), ~ok | np.isnan(x))
+    np.testing.assert_allclose(flat[ok] * r.trend64[ok], x[ok].astype(np.float64), rtol=4e-16)
+    cst = np.full((1, 300), 0.75, np.float32)
+    assert np.array_equal(orc.normalize(cst, orc.detrend(cst, 9).trend64), np.ones((1, 300)))
+
+
+@pytest.mark.parametrize("W,jitter", [(5, 0.0), (25, 0.3), (51, 0.45)])
+def test_gapped_equals_base_oracle_on_the_nan_filled_grid(W, jitter):
+    # R20: removing the invalid slots and giving real time stamps must not change anything:
+    # the base oracle on the uniform NaN-filled grid (pinned above) fixes every value.
+    from workloads import lightcurves as lc
+    dt = 2.0 / 1440
+    grid = lc.random_series(40 + W, 3, 900, nan_frac=0.04, inf_frac=0.0)
+    grid[1, 300:420] = np.nan                         # a gap wider than the window
+    t, f, slot = lc.compact(grid, dt, t0=1234.5, jitter=jitter, seed=W)
+    base = orc.detrend(grid, W)
+    got = orc.gapped(t, f, 1234.5, dt, grid.shape[1], W)
+    for b in range(grid.shape[0]):
+        m = slot[b] >= 0
+        np.testing.assert_array_equal(got.trend64[b, m], base.trend64[b, slot[b, m]])
+        np.testing.assert_array_equal(got.median[b, m], base.median[b, slot[b, m]])
+        np.testing.assert_array_equal(got.n_valid[b, m], base.n_valid[b, slot[b, m]])
+        assert np.isnan(got.trend64[b, ~m]).all()     # padding (NaN time) -> NaN
+
+
+def test_gapped_brute_force_out_of_range_and_colliding_slots():
+    from workloads import lightcurves as lc
+    dt = 0.02
+    grid = lc.random_series(77, 2, 260, nan_frac=0.05, inf_frac=0.0)
+    t, f, slot = lc.compact(grid, dt, t0=10.0, jitter=0.2, seed=1)
+    t[0, 50] = t[0, 51] - 1e-9 * dt                   # two samples in one slot: the first is dropped
+    t[1, 5] = np.inf
+    f[1, 9] = np.nan
+    n_grid = 240                                      # slots >= 240 fall outside the grid
+    for W, mv in ((7, -1), (31, 3)):
+        got = orc.gapped(t, f, 10.0, dt, n_grid, W, min_valid=mv)
+        bt, bm = brute.detrend_gapped(t, f, 10.0, dt, n_grid, W, min_valid=None if mv < 0 else mv)
+        assert np.array_equal(np.isnan(got.trend64), np.isnan(bt))
+        ok = ~np.isnan(bt)
+        np.testing.assert_allclose(got.trend64[ok], bt[ok], rtol=1e-13)
+        np.testing.assert_array_equal(got.median[ok].astype(np.float64), bm[ok])
+        assert np.isnan(got.trend64[0, 50]) and not np.isnan(got.trend64[0, 51])
+        for b in range(2):
+            assert np.isnan(got.trend64[b, slot[b] >= n_grid]).all()
+
+
+def test_gapped_on_uniform_times_is_the_positional_window():
+    from workloads import lightcurves as lc
+    x = lc.random_series(9, 2, 500, nan_frac=0.0, inf_frac=0.0)
+    t = np.tile(5.0 + np.arange(500) * 0.01, (2, 1))
+    a = orc.gapped(t, x, 5.0, 0.01, 500, 21)
+    b = orc.detrend(x, 21)
+    np.testing.assert_array_equal(a.trend64, b.trend64)

@@ -185,3 +185,25 @@ def random_series(seed, n_stars, n_cadences, nan_frac=0.05, inf_frac=0.01, ties=
         m = rng.random(x.shape) < inf_frac
         x[m] = np.where(rng.random(m.sum()) < 0.5, np.inf, -np.inf).astype(np.float32)
     return x
+
+
+def compact(flux_grid, dt_days, t0=0.0, jitter=0.0, seed=0):
+    """Compacted rows with real time stamps, as a mission pipeline delivers them after
+    quality filtering: the non-finite slots of a uniform-grid array are
+    REMOVED, so time jumps across gaps.  Returns (time[S, M] fp64, flux[S, M] fp32,
+    slot[S, M] int64) with M = the longest row; shorter rows are padded at the end with
+    NaN time / NaN flux / slot -1.  time = t0 + slot*dt + U(-jitter, jitter)*dt (inputs
+    only: no method arithmetic here; `slot` is what the caller started from, for tests)."""
+    flux_grid = np.atleast_2d(np.asarray(flux_grid, dtype=np.float32))
+    S, N = flux_grid.shape
+    rng = np.random.Generator(np.random.PCG64(np.random.SeedSequence([4242, int(seed)])))
+    keep = [np.flatnonzero(np.isfinite(flux_grid[b])) for b in range(S)]
+    M = max([k.size for k in keep] + [1])
+    time = np.full((S, M), np.nan, np.float64)
+    flux = np.full((S, M), np.nan, np.float32)
+    slot = np.full((S, M), -1, np.int64)
+    for b, k in enumerate(keep):
+        slot[b, :k.size] = k
+        flux[b, :k.size] = flux_grid[b, k]
+        time[b, :k.size] = t0 + (k + rng.uniform(-jitter, jitter, k.size)) * dt_days
+    return time, flux, slot
