@@ -32,6 +32,7 @@
 #ifndef UMI_B200_H
 #define UMI_B200_H
 
+#include <stddef.h>
 #include <stdint.h>
 
 #ifdef __cplusplus
@@ -93,6 +94,52 @@ int umi_detrend_ex(const double* time, const float* flux,
                    int64_t n_stars, int64_t n_cadences,
                    int W, float alpha, float c, int n_iter, int min_valid,
                    float* trend_out, void* stream);
+
+/*
+ * Detrend + normalise ("detrending, normalization"): umi_detrend_ex, and in the
+ * same kernels' epilogue flat_out[b, i] = flux[b, i] / trend_out[b, i] (one IEEE fp32
+ * division; NaN wherever trend_out is NaN).  With n_iter = 0 the divisor is the median.
+ *   flat_out  DEVICE, float [n_stars*n_cadences]; must not overlap the other buffers;
+ *             NULL -> UMI_ERR_INVALID_ARG (use umi_detrend_ex).
+ * trend_out is still required (it is the scratch between the kernels).
+ */
+int umi_flatten(const double* time, const float* flux,
+                int64_t n_stars, int64_t n_cadences,
+                int W, float alpha, float c, int n_iter, int min_valid,
+                float* trend_out, float* flat_out, void* stream);
+
+/*
+ * Gap handling by time stamps ("gap handling", the stage in front of the
+ * detrender; reading R20).  The rows are COMPACTED series: cadences were removed
+ * upstream, so time jumps.  Sample (b, i) sits in slot k = rint((time[b, i] - t0) / dt)
+ * (fp64, round half to even) of a uniform grid of n_grid slots, and its window is the valid
+ * samples of its row whose slot differs from k by at most h = (W-1)/2 -- the same W*dt of
+ * time the positional window of PAPER.md:35 spans on an uncompacted row.  A sample is
+ * invalid (NaN out, in no window) iff its time or flux is not finite, k is outside
+ * [0, n_grid), or the next sample of its row lands in the same slot.  Rows must be
+ * non-decreasing in time (otherwise the result is unspecified but memory-safe); rows
+ * shorter than n_samples are padded with NaN time.
+ *
+ * Implementation: NaN-fill + scatter onto the grid, the hot path on [n_stars, n_grid],
+ * gather back (csrc/umi_regrid.cu).
+ *   time       DEVICE, const double [n_stars*n_samples]; required.
+ *   flux       DEVICE, const float  [n_stars*n_samples].
+ *   t0, dt     grid origin and cadence in the unit of `time`; dt > 0, both finite.
+ *   n_grid     >= 0 slots per row (e.g. 1 + rint((t_last - t0)/dt)).
+ *   trend_out  DEVICE, float [n_stars*n_samples].
+ *   flat_out   DEVICE, float [n_stars*n_samples] or NULL: flux / trend.
+ *   workspace  DEVICE, at least umi_gapped_workspace_bytes(n_stars, n_grid) bytes, owned by
+ *              the caller, free to reuse once the stream has passed the call; too small or
+ *              NULL -> UMI_ERR_INVALID_ARG.  The library allocates nothing.
+ * Enqueues on `stream`; does not synchronise.
+ */
+size_t umi_gapped_workspace_bytes(int64_t n_stars, int64_t n_grid);
+int umi_detrend_gapped(const double* time, const float* flux,
+                       int64_t n_stars, int64_t n_samples,
+                       double t0, double dt, int64_t n_grid,
+                       int W, float alpha, float c, int n_iter, int min_valid,
+                       float* trend_out, float* flat_out,
+                       void* workspace, size_t workspace_bytes, void* stream);
 
 /*
  * Batch driver (the paper streams 50-star batches): the same

@@ -20,6 +20,7 @@ UMI_OK, UMI_ERR_INVALID_ARG, UMI_ERR_UNSUPPORTED, UMI_ERR_CUDA = 0, 1, 2, 3
 UMI_MAX_WINDOW = 4097
 
 EXPORTS = ("umi_window_len", "umi_detrend", "umi_detrend_ex", "umi_detrend_host", "umi_detrend_profile",
+           "umi_flatten", "umi_detrend_gapped", "umi_gapped_workspace_bytes",
            "umi_launch_geometry", "umi_status_string", "umi_version")
 
 _lib = None
@@ -52,6 +53,13 @@ def lib():
     L.umi_detrend_profile.argtypes = [vp, vp, i64, i64, ci, cf, cf, ci, ci, vp, vp, ctypes.POINTER(cf)]
     L.umi_detrend_host.restype = ci
     L.umi_detrend_host.argtypes = [vp, vp, i64, i64, ci, cf, ci, vp, i64, ci]
+    L.umi_flatten.restype = ci
+    L.umi_flatten.argtypes = [vp, vp, i64, i64, ci, cf, cf, ci, ci, vp, vp, vp]
+    L.umi_gapped_workspace_bytes.restype = ctypes.c_size_t
+    L.umi_gapped_workspace_bytes.argtypes = [i64, i64]
+    L.umi_detrend_gapped.restype = ci
+    L.umi_detrend_gapped.argtypes = [vp, vp, i64, i64, ctypes.c_double, ctypes.c_double, i64,
+                                     ci, cf, cf, ci, ci, vp, vp, vp, ctypes.c_size_t, vp]
     L.umi_launch_geometry.restype = ci
     L.umi_launch_geometry.argtypes = [ci] + [ctypes.POINTER(ci)] * 3
     L.umi_status_string.restype = ctypes.c_char_p
@@ -136,6 +144,66 @@ def umi_detrend(time, flux, W, alpha=2.0, n_iter=5, out=None, stream=None, c=Non
                                       -1 if min_valid is None else int(min_valid), optr, sptr)
     _check(st)
     return out.view(flux.shape)
+
+
+def _stream_ptr(stream, device):
+    import torch
+    if stream is None:
+        stream = torch.cuda.current_stream(device)
+    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+
+
+def umi_flatten(time, flux, W, alpha=2.0, n_iter=5, c=5.0, min_valid=-1, stream=None):
+    """Detrend + normalise (PAPER.md:155): returns (trend, flat) with flat = flux / trend
+    computed in the kernels' epilogue.  Same argument rules as umi_detrend."""
+    import torch
+    f = _cuda_2d(flux, torch.float32, "flux")
+    tptr = None
+    if time is not None:
+        tt = _cuda_2d(time, torch.float64, "time")
+        if tt.shape != f.shape or tt.device != f.device:
+            raise ValueError("time must have flux's shape and device")
+        tptr = tt.data_ptr()
+    trend, flat = torch.empty_like(f), torch.empty_like(f)
+    S, N = f.shape
+    if S and N:
+        with torch.cuda.device(f.device):
+            _check(lib().umi_flatten(tptr, f.data_ptr(), S, N, int(W), float(alpha), float(c), int(n_iter),
+                                     int(min_valid), trend.data_ptr(), flat.data_ptr(),
+                                     _stream_ptr(stream, f.device)))
+    return trend.view(flux.shape), flat.view(flux.shape)
+
+
+def umi_gapped_workspace_bytes(n_stars, n_grid):
+    return int(lib().umi_gapped_workspace_bytes(int(n_stars), int(n_grid)))
+
+
+def umi_detrend_gapped(time, flux, t0, dt, n_grid, W, alpha=2.0, n_iter=5, c=5.0, min_valid=-1,
+                       flat=False, workspace=None, stream=None):
+    """Compacted rows with real time stamps (gap handling; include/umi.h).
+    `time` CUDA fp64 [S, M], `flux` CUDA fp32 [S, M].  Returns trend, or (trend, flat).
+    `workspace`: optional CUDA uint8 tensor of at least umi_gapped_workspace_bytes bytes."""
+    import torch
+    f = _cuda_2d(flux, torch.float32, "flux")
+    tt = _cuda_2d(time, torch.float64, "time")
+    if tt.shape != f.shape or tt.device != f.device:
+        raise ValueError("time must have flux's shape and device")
+    S, M = f.shape
+    need = umi_gapped_workspace_bytes(S, n_grid)
+    if workspace is None:
+        workspace = torch.empty(max(need, 1), dtype=torch.uint8, device=f.device)
+    elif not (isinstance(workspace, torch.Tensor) and workspace.is_cuda and workspace.is_contiguous()):
+        raise TypeError("workspace must be a contiguous CUDA tensor")
+    wbytes = workspace.numel() * workspace.element_size()
+    trend = torch.empty_like(f)
+    fl = torch.empty_like(f) if flat else None
+    if S and M:
+        with torch.cuda.device(f.device):
+            _check(lib().umi_detrend_gapped(tt.data_ptr(), f.data_ptr(), S, M, float(t0), float(dt), int(n_grid),
+                                            int(W), float(alpha), float(c), int(n_iter), int(min_valid),
+                                            trend.data_ptr(), fl.data_ptr() if flat else None,
+                                            workspace.data_ptr(), wbytes, _stream_ptr(stream, f.device)))
+    return (trend.view(flux.shape), fl.view(flux.shape)) if flat else trend.view(flux.shape)
 
 
 def umi_detrend_profile(time, flux, W, alpha=2.0, n_iter=5, out=None, stream=None, c=5.0, min_valid=-1):

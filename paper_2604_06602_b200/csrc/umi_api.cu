@@ -65,7 +65,8 @@ int validate(const float* flux, int64_t n_stars, int64_t n_cadences, int W, floa
 /* Enqueue both kernels for device-resident buffers. */
 int launch_device(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
                   int W, float alpha, float c, int n_iter, int min_valid, float* trend_out,
-                  cudaStream_t stream, cudaEvent_t* ev = nullptr /* [3] or null */)
+                  cudaStream_t stream, cudaEvent_t* ev = nullptr /* [3] or null */,
+                  float* flat_out = nullptr)
 {
     if (n_stars == 0 || n_cadences == 0) return UMI_OK;
     const Geometry g = geometry_for(W);
@@ -77,6 +78,7 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.time = time;
         rp.flux = flux;
         rp.out = trend_out;
+        rp.flat = flat_out;
         rp.N = n_cadences;
         rp.tiles_per_star = (n_cadences + umi::KS_THREADS - 1) / umi::KS_THREADS;
         rp.n_blocks = n_stars * rp.tiles_per_star;
@@ -97,6 +99,7 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
     mp.time = time;
     mp.flux = flux;
     mp.out = trend_out;
+    mp.flat = (n_iter == 0) ? flat_out : nullptr;
     mp.N = n_cadences;
     mp.tiles_per_star = (n_cadences + g.T1 - 1) / g.T1;
     mp.n_blocks = n_stars * mp.tiles_per_star;
@@ -114,6 +117,7 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.time = time;
         rp.flux = flux;
         rp.out = trend_out;
+        rp.flat = flat_out;
         rp.N = n_cadences;
         rp.tiles_per_star = (n_cadences + umi::K2_TILE - 1) / umi::K2_TILE;
         rp.n_blocks = n_stars * rp.tiles_per_star;
@@ -148,6 +152,59 @@ int umi_detrend_ex(const double* time, const float* flux, int64_t n_stars, int64
     if (st != UMI_OK) return st;
     return launch_device(time, flux, n_stars, n_cadences, W, alpha, c, n_iter, min_valid, trend_out,
                          static_cast<cudaStream_t>(stream));
+}
+
+int umi_flatten(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
+                int W, float alpha, float c, int n_iter, int min_valid,
+                float* trend_out, float* flat_out, void* stream)
+{
+    if (flat_out == nullptr) return UMI_ERR_INVALID_ARG;
+    const int st = validate(flux, n_stars, n_cadences, W, alpha, c, n_iter, trend_out);
+    if (st != UMI_OK) return st;
+    return launch_device(time, flux, n_stars, n_cadences, W, alpha, c, n_iter, min_valid, trend_out,
+                         static_cast<cudaStream_t>(stream), nullptr, flat_out);
+}
+
+size_t umi_gapped_workspace_bytes(int64_t n_stars, int64_t n_grid)
+{
+    if (n_stars <= 0 || n_grid <= 0) return 0;
+    return (size_t)2 * (size_t)n_stars * (size_t)n_grid * sizeof(float);
+}
+
+int umi_detrend_gapped(const double* time, const float* flux, int64_t n_stars, int64_t n_samples,
+                       double t0, double dt, int64_t n_grid,
+                       int W, float alpha, float c, int n_iter, int min_valid,
+                       float* trend_out, float* flat_out,
+                       void* workspace, size_t workspace_bytes, void* stream)
+{
+    if (time == nullptr || n_grid < 0 || !(dt > 0.0) || !isfinite(dt) || !isfinite(t0)) return UMI_ERR_INVALID_ARG;
+    const int st = validate(flux, n_stars, n_samples, W, alpha, c, n_iter, trend_out);
+    if (st != UMI_OK) return st;
+    if (n_stars == 0 || n_samples == 0) return UMI_OK;
+    const size_t need = umi_gapped_workspace_bytes(n_stars, n_grid);
+    if (need > 0 && (workspace == nullptr || workspace_bytes < need)) return UMI_ERR_INVALID_ARG;
+    cudaStream_t s = static_cast<cudaStream_t>(stream);
+    umi::RegridParams gp;
+    gp.time = time;
+    gp.flux = flux;
+    gp.n_stars = n_stars;
+    gp.M = n_samples;
+    gp.n_grid = n_grid;
+    gp.t0 = t0;
+    gp.dt = dt;
+    float* grid_flux = static_cast<float*>(workspace);
+    float* grid_trend = grid_flux + (size_t)n_stars * (size_t)n_grid;
+    if (n_grid > 0) {
+        /* 0xFFFFFFFF is a NaN: every slot starts invalid */
+        if (cuda_failed(cudaMemsetAsync(grid_flux, 0xFF, (size_t)n_stars * (size_t)n_grid * sizeof(float), s)))
+            return UMI_ERR_CUDA;
+        if (cuda_failed(umi::launch_regrid_scatter(gp, grid_flux, s))) return UMI_ERR_CUDA;
+        const int st2 = launch_device(nullptr, grid_flux, n_stars, n_grid, W, alpha, c, n_iter, min_valid,
+                                      grid_trend, s);
+        if (st2 != UMI_OK) return st2;
+    }
+    if (cuda_failed(umi::launch_regrid_gather(gp, grid_trend, trend_out, flat_out, s))) return UMI_ERR_CUDA;
+    return UMI_OK;
 }
 
 int umi_detrend_profile(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
@@ -293,6 +350,6 @@ const char* umi_status_string(int status)
     }
 }
 
-int umi_version(void) { return 100; /* 0.1.0 */ }
+int umi_version(void) { return 200; /* 0.2.0 */ }
 
 } /* extern "C" */

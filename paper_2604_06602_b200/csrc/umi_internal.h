@@ -32,6 +32,7 @@ struct MedianParams {
     const double* time;      /* may be null */
     const float* flux;
     float* out;              /* median, NaN where the position has no trend */
+    float* flat;             /* null, or flux / median (only set when the call stops after Phase 1) */
     int64_t N;               /* cadences per star */
     int64_t tiles_per_star;
     int64_t n_blocks;        /* n_stars * tiles_per_star */
@@ -42,6 +43,7 @@ struct ReweightParams {
     const double* time;
     const float* flux;
     float* out;              /* in: median from the median kernel; out: trend */
+    float* flat;             /* null, or flux / trend (PAPER.md:155 normalisation), NaN where trend is NaN */
     int64_t N;
     int64_t tiles_per_star;
     int64_t n_blocks;
@@ -54,6 +56,19 @@ cudaError_t launch_median(const MedianParams& prm, unsigned grid, size_t smem, c
 cudaError_t launch_reweight(const ReweightParams& prm, unsigned grid, size_t smem, cudaStream_t stream);
 /* fused kernel for W <= KS_MAX_WINDOW; wt = compiled wire count (9, 17, 25, 33 or 49) >= W */
 cudaError_t launch_small(const ReweightParams& prm, int min_valid, int wt, unsigned grid, cudaStream_t stream);
+
+/* umi_regrid.cu: gap handling by time stamps (R20) */
+struct RegridParams {
+    const double* time;      /* [n_stars, M] compacted rows */
+    const float* flux;       /* [n_stars, M] */
+    int64_t n_stars, M, n_grid;
+    double t0, dt;
+};
+/* grid_flux[n_stars, n_grid] must already be NaN-filled */
+cudaError_t launch_regrid_scatter(const RegridParams& prm, float* grid_flux, cudaStream_t stream);
+/* trend_out[b, i] = grid_trend[b, slot] (NaN for invalid samples); flat_out (nullable) = flux / trend */
+cudaError_t launch_regrid_gather(const RegridParams& prm, const float* grid_trend, float* trend_out,
+                                 float* flat_out, cudaStream_t stream);
 
 } // namespace umi
 

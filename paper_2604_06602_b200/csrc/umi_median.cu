@@ -310,6 +310,13 @@ umi_median_kernel(MedianParams prm)
 
         float* orow = prm.out + star * prm.N + j0;
         for (int p = tid; p < Tact; p += K1_THREADS) orow[p] = medbuf[p];
+        if (prm.flat != nullptr) {                                  /* PAPER.md:155 normalisation, n_iter = 0 */
+            float* flrow = prm.flat + star * prm.N + j0;
+            for (int p = tid; p < Tact; p += K1_THREADS) {
+                const float m = medbuf[p];
+                flrow[p] = (m == m) ? __ldg(frow + j0 + p) / m : m;
+            }
+        }
         __syncthreads();
     }
 }

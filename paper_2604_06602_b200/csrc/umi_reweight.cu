@@ -313,6 +313,15 @@ umi_reweight_kernel(ReweightParams prm)
             const int64_t j = j0 + 4 * tid + q;
             if (j < prm.N && med[q] == med[q]) orow[j] = mu[q];
         }
+        if (prm.flat != nullptr) {                                  /* PAPER.md:155 normalisation */
+            float* flrow = prm.flat + star * prm.N;
+#pragma unroll
+            for (int q = 0; q < K2_NPOS; ++q) {
+                const int64_t j = j0 + 4 * tid + q;
+                /* own sample = staged index hal + 4*tid + q (valid whenever the median is not NaN) */
+                if (j < prm.N) flrow[j] = (med[q] == med[q]) ? xs[hal + 4 * tid + q] / mu[q] : qnan;
+            }
+        }
         __syncthreads();
     }
 }

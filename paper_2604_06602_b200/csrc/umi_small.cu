@@ -205,7 +205,11 @@ umi_small_kernel(ReweightParams prm, int min_valid)
                 if (on && S > 0.f) mu = fmaf(R / S, cs, mu);        /* Eq. 4; (R11) */
             }
         }
-        if (in_row) orow[j] = has ? mu : qnan;
+        if (in_row) {
+            orow[j] = has ? mu : qnan;
+            if (prm.flat != nullptr)                                /* PAPER.md:155 normalisation */
+                prm.flat[star * prm.N + j] = has ? xs[tid + h] / mu : qnan;
+        }
         __syncthreads();
     }
 }

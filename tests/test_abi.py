@@ -28,7 +28,7 @@ def test_library_builds_loads_and_exports_every_declared_symbol():
     assert set(declared) == set(umi.EXPORTS), (declared, umi.EXPORTS)
     for name in declared:
         assert hasattr(L, name), name
-    assert umi.umi_version() >= 100
+    assert umi.umi_version() >= 200
 
 
 def test_window_len_paper_values_and_guard():
@@ -74,6 +74,21 @@ def test_validation_happens_on_the_host():
     assert L.umi_detrend_ex(None, one, 1, 10, 5, 2.0, 0.0, 5, -1, one, None) == umi.UMI_ERR_INVALID_ARG
     assert L.umi_detrend_host(None, None, 1, 10, 5, 2.0, 5, one, 0, 0) == umi.UMI_ERR_INVALID_ARG
     assert L.umi_detrend_host(None, one, 0, 10, 5, 2.0, 5, one, 0, 0) == umi.UMI_OK
+    # next rows: normalisation and time-stamped gap handling
+    assert L.umi_flatten(None, one, 1, 10, 5, 2.0, 5.0, 5, -1, one, None, None) == umi.UMI_ERR_INVALID_ARG
+    assert L.umi_flatten(None, one, 0, 10, 5, 2.0, 5.0, 5, -1, one, one, None) == umi.UMI_OK
+    gap = lambda **k: L.umi_detrend_gapped(k.get("time", one), one, k.get("S", 1), 10, 0.0, k.get("dt", 0.5),
+                                           k.get("n_grid", 12), 5, 2.0, 5.0, 5, -1, one, None,
+                                           k.get("ws", one), k.get("wsb", 1 << 20), None)
+    assert gap(time=None) == umi.UMI_ERR_INVALID_ARG
+    assert gap(dt=0.0) == umi.UMI_ERR_INVALID_ARG
+    assert gap(dt=float("nan")) == umi.UMI_ERR_INVALID_ARG
+    assert gap(n_grid=-1) == umi.UMI_ERR_INVALID_ARG
+    assert gap(ws=None) == umi.UMI_ERR_INVALID_ARG
+    assert gap(wsb=95) == umi.UMI_ERR_INVALID_ARG      # 2 * 1 * 12 * 4 = 96 bytes needed
+    assert gap(S=0) == umi.UMI_OK
+    assert umi.umi_gapped_workspace_bytes(3, 100) == 2400
+    assert umi.umi_gapped_workspace_bytes(0, 100) == 0
     for s in range(5):
         assert umi.umi_status_string(s)
     assert "UMI_OK" in umi.umi_status_string(0)

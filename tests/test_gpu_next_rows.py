@@ -1,0 +1,116 @@
+"""GPU parity for the rows SURVEY.md 8(f) marks "next": F1 fused normalisation
+(umi_flatten) and F2 time-stamped gap handling (umi_detrend_gapped,
+PAPER.md:155; R20), through the C ABI, against the fp64 oracle.
+Bars: NaN pattern identical, median bit-exact, trend and flat within 1e-5 relative."""
+import numpy as np
+import pytest
+
+from oracle import umi_oracle as orc
+from tests import parity
+from workloads import lightcurves as lc
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def umi():
+    import paper_2604_06602_b200 as m
+    m.lib()
+    return m
+
+
+def _cuda(a, dtype):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a, dtype=dtype)).cuda()
+
+
+def _check_flat(flat_gpu, flux, ref):
+    want = orc.normalize(flux, ref.trend64)
+    got = flat_gpu.astype(np.float64)
+    assert np.array_equal(np.isnan(got), np.isnan(want))
+    ok = ~np.isnan(want) & ~ref.near_cutoff.astype(bool)
+    if ok.any():
+        rel = np.abs(got[ok] - want[ok]) / np.maximum(np.abs(want[ok]), 1e-30)
+        assert rel.max() <= parity.TOL, rel.max()
+
+
+@pytest.mark.parametrize("W", [1, 9, 25, 49, 51, 361, 1081])
+@pytest.mark.parametrize("n_iter", [0, 5])
+def test_flatten_matches_oracle(umi, W, n_iter):
+    import torch
+    x = lc.random_series(300 + W, 3, 2777)
+    ref = orc.detrend(x, W, n_iter=n_iter)
+    trend, flat = umi.umi_flatten(None, _cuda(x, np.float32), W, n_iter=n_iter)
+    torch.cuda.synchronize()
+    trend, flat = trend.cpu().numpy(), flat.cpu().numpy()
+    if n_iter == 0:
+        parity.compare_median(trend, ref.median)
+    else:
+        parity.compare_trend(trend, ref)
+    _check_flat(flat, x, ref)
+
+
+def test_flatten_constant_series_is_exactly_one(umi):
+    import torch
+    x = np.full((2, 1500), 0.3, np.float32)
+    for W in (25, 361):
+        trend, flat = umi.umi_flatten(None, _cuda(x, np.float32), W)
+        torch.cuda.synchronize()
+        assert np.array_equal(flat.cpu().numpy(), np.ones_like(x))
+        assert np.array_equal(trend.cpu().numpy(), x)
+
+
+@pytest.mark.parametrize("W,jitter", [(5, 0.0), (25, 0.3), (51, 0.45), (361, 0.4), (1081, 0.2)])
+def test_gapped_matches_oracle(umi, W, jitter):
+    import torch
+    dt = 2.0 / 1440
+    grid = lc.random_series(500 + W, 3, 4001, nan_frac=0.04, inf_frac=0.0)
+    grid[1, 1000:1000 + W + 40] = np.nan                  # a gap wider than the window
+    t, f, slot = lc.compact(grid, dt, t0=2458000.25, jitter=jitter, seed=W)
+    t[2, 17] = np.inf                                     # bad time stamp
+    f[0, 33] = np.nan                                     # bad flux that survived compaction
+    n_grid = grid.shape[1] - 7                            # the last slots fall outside the grid
+    ref = orc.gapped(t, f, 2458000.25, dt, n_grid, W)
+    td, fd = _cuda(t, np.float64), _cuda(f, np.float32)
+    med = umi.umi_detrend_gapped(td, fd, 2458000.25, dt, n_grid, W, n_iter=0)
+    trend, flat = umi.umi_detrend_gapped(td, fd, 2458000.25, dt, n_grid, W, flat=True)
+    torch.cuda.synchronize()
+    parity.compare_median(med.cpu().numpy(), ref.median)
+    parity.compare_trend(trend.cpu().numpy(), ref)
+    _check_flat(flat.cpu().numpy(), f, ref)
+
+
+def test_gapped_colliding_slots_and_empty_grid(umi):
+    import torch
+    dt = 0.02
+    grid = lc.random_series(78, 2, 900, nan_frac=0.03, inf_frac=0.0)
+    t, f, slot = lc.compact(grid, dt, t0=10.0, jitter=0.2, seed=2)
+    t[0, 50] = t[0, 51] - 1e-9 * dt                       # two samples in one slot
+    ref = orc.gapped(t, f, 10.0, dt, 900, 31)
+    got = umi.umi_detrend_gapped(_cuda(t, np.float64), _cuda(f, np.float32), 10.0, dt, 900, 31)
+    torch.cuda.synchronize()
+    got = got.cpu().numpy()
+    parity.compare_trend(got, ref)
+    assert np.isnan(got[0, 50]) and not np.isnan(got[0, 51])
+    # n_grid = 0: every sample is outside the grid
+    got = umi.umi_detrend_gapped(_cuda(t, np.float64), _cuda(f, np.float32), 10.0, dt, 0, 31)
+    torch.cuda.synchronize()
+    assert np.isnan(got.cpu().numpy()).all()
+    # a caller-owned workspace that is too small is refused on the host
+    with pytest.raises(umi.UmiError):
+        umi.umi_detrend_gapped(_cuda(t, np.float64), _cuda(f, np.float32), 10.0, dt, 900, 31,
+                               workspace=torch.empty(16, dtype=torch.uint8, device="cuda"))
+
+
+def test_gapped_tess_batch_stars_compacted(umi):
+    # config-2 stars with their 1-day gap removed (PAPER.md:155 pipeline order), full length
+    import torch
+    cfg = lc.CONFIGS[2]
+    grid = lc.stars(2, [3, 4])
+    t, f, slot = lc.compact(grid, cfg.dt_days, t0=1468.27, jitter=0.1, seed=9)
+    ref = orc.gapped(t, f, 1468.27, cfg.dt_days, cfg.n_cadences, cfg.W)
+    trend, flat = umi.umi_detrend_gapped(_cuda(t, np.float64), _cuda(f, np.float32), 1468.27, cfg.dt_days,
+                                         cfg.n_cadences, cfg.W, flat=True)
+    torch.cuda.synchronize()
+    parity.compare_trend(trend.cpu().numpy(), ref)
+    _check_flat(flat.cpu().numpy(), f, ref)
