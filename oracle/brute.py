@@ -105,3 +105,32 @@ def detrend_gapped(time, flux, t0, dt, n_grid, W, alpha=2.0, n_iter=5, c=5.0, mi
                 continue
             trend[b, i], median[b, i], _ = location(x, alpha, c, n_iter)
     return trend, median
+
+
+def location_family(x, scale_kind="upper_rms", weight_kind="bisquare", alpha=2.0, c=5.0, n_iter=5):
+    """Sibling estimators (F4): scale_kind "mad" = np.median-style MAD (lower middle, R21),
+    weight_kind "welsch" = exp(-u_eff^2) (R22).  Returns (mu, median, s)."""
+    x = np.asarray(x, dtype=np.float64)
+    n = x.size
+    med = np.sort(x)[(n - 1) // 2]
+    if scale_kind == "mad":
+        s = np.sort(np.abs(x - med))[(n - 1) // 2]
+    else:
+        upper = x[x > med]
+        if upper.size == 0:
+            return med, med, 0.0
+        s = SCALE_CONST * np.sqrt(np.mean((upper - med) ** 2))
+    if not s > 0.0:
+        return med, med, s
+    mu = med
+    for _ in range(n_iter):
+        u = (x - mu) / (c * s)
+        if weight_kind == "welsch":
+            u_eff = np.where(u < 0.0, alpha * u, u)
+            w = np.exp(-u_eff ** 2)
+        else:
+            w = bisquare_weights(u, alpha)
+        if not w.sum() > 0.0:
+            break
+        mu = np.average(x, weights=w)
+    return mu, med, s

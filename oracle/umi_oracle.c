@@ -36,6 +36,12 @@
 
 #define UMI_ORACLE_SCALE_CONST 0.6745
 
+/* Sibling estimators on the same window machinery. */
+#define UMI_ORACLE_SCALE_UPPER_RMS 0   /* PAPER.md:43-48, the paper's scale */
+#define UMI_ORACLE_SCALE_MAD 1         /* the standard MAD (ablation) */
+#define UMI_ORACLE_WEIGHT_BISQUARE 0   /* PAPER.md:58, Eq. 3 */
+#define UMI_ORACLE_WEIGHT_WELSCH 1     /* Gaussian-shaped weights */
+
 /* W = floor(0.5/dt) | 1, dt in days.
  * (R15) the quotient is nudged up by 2^-20 relative before the floor so that a
  * cadence that passed through fp32 (0.5/dt = 359.99999) still gives the
@@ -82,7 +88,8 @@ static int slot_valid(const double *time, const float *flux, int64_t N, int64_t 
  * (double), median (float), scale s, n_plus, near_cutoff flag.  sorted[] must
  * hold n doubles.  Returns 1 if a trend value was produced, 0 if the output is NaN.
  */
-static int oracle_location(const double *x, int n, int own_valid,
+static int oracle_location_family(const double *x, int n, int own_valid,
+                           int scale_kind, int weight_kind,
                            double alpha, double c, int n_iter, int min_valid,
                            double cutoff_tol, double *sorted,
                            double *trend, float *median, double *scale,
@@ -104,6 +111,16 @@ static int oracle_location(const double *x, int n, int own_valid,
     const double med = sorted[(n - 1) / 2];
     if (median) *median = (float)med;                 /* a selected fp32 sample: exact */
 
+    double s;
+    if (scale_kind == UMI_ORACLE_SCALE_MAD) {
+        /* Sibling scale (F4): the standard MAD, the median of the absolute
+         * deviations from the median, both sides.  (R21) rank (n-1)/2 of the sorted deviations,
+         * as for the median itself (R6); used as s directly -- PAPER.md:48 scales sigma_upper
+         * by 0.6745 "to match the MAD convention", so the MAD itself carries no factor. */
+        for (int j = 0; j < n; ++j) sorted[j] = fabs(x[j] - med);
+        qsort(sorted, (size_t)n, sizeof(double), cmp_double);
+        s = sorted[(n - 1) / 2];
+    } else {
     /* Phase 2, Eq. 1: RMS of residuals strictly above the median (R7). */
     int n_plus = 0;
     double ss = 0.0;
@@ -116,7 +133,8 @@ static int oracle_location(const double *x, int n, int own_valid,
         return 1;
     }
     const double sigma_upper = sqrt(ss / (double)n_plus);
-    const double s = UMI_ORACLE_SCALE_CONST * sigma_upper;            /* PAPER.md:48 */
+    s = UMI_ORACLE_SCALE_CONST * sigma_upper;                         /* PAPER.md:48 */
+    }
     if (scale) *scale = s;
     if (!(s > 0.0)) {                                 /* (R8) */
         if (trend) *trend = med;
@@ -133,9 +151,15 @@ static int oracle_location(const double *x, int n, int own_valid,
             double u = (x[j] - mu) / (c * s);         /* PAPER.md:54 */
             double ueff = (u < 0.0) ? alpha * u : u;  /* Eq. 2 */
             double w;
+            if (weight_kind == UMI_ORACLE_WEIGHT_WELSCH) {
+                /* Sibling weight (F4; PAPER.md:19 "Welsch ... Gaussian-shaped weights"):
+                 * (R22) w = exp(-u_eff^2), no cut-off. */
+                w = exp(-ueff * ueff);
+            } else {
             if (fabs(ueff) < 1.0) { double t = 1.0 - ueff * ueff; w = t * t; }   /* Eq. 3 */
             else w = 0.0;
             if (fabs(fabs(ueff) - 1.0) <= cutoff_tol) flagged = 1;
+            }
             sw += w;
             swx += w * x[j];
         }
@@ -145,6 +169,18 @@ static int oracle_location(const double *x, int n, int own_valid,
     if (trend) *trend = mu;
     if (near_cutoff) *near_cutoff = (uint8_t)flagged;
     return 1;
+}
+
+/* The paper's estimator: upper-RMS scale, bisquare weights. */
+static int oracle_location(const double *x, int n, int own_valid,
+                           double alpha, double c, int n_iter, int min_valid,
+                           double cutoff_tol, double *sorted,
+                           double *trend, float *median, double *scale,
+                           int32_t *n_plus_out, uint8_t *near_cutoff)
+{
+    return oracle_location_family(x, n, own_valid, UMI_ORACLE_SCALE_UPPER_RMS, UMI_ORACLE_WEIGHT_BISQUARE,
+                                  alpha, c, n_iter, min_valid, cutoff_tol, sorted,
+                                  trend, median, scale, n_plus_out, near_cutoff);
 }
 
 /*
@@ -361,6 +397,55 @@ int umi_oracle_gapped(const double *time, const float *flux,
         free(work);
     }
     free(slot);
+    return bad;
+}
+
+/*
+ * Sibling estimators (F4): every position of every star with the chosen scale and weight.
+ * scale_kind 0 / weight_kind 0 is umi_oracle_detrend.  n_plus is not produced for the MAD.
+ */
+int umi_oracle_family(const double *time, const float *flux,
+                      int64_t n_stars, int64_t n_cadences,
+                      int W, int scale_kind, int weight_kind,
+                      double alpha, double c, int n_iter, int min_valid, double cutoff_tol,
+                      double *trend64, float *trend32, float *median,
+                      double *scale, int32_t *n_valid, int32_t *n_plus,
+                      uint8_t *near_cutoff)
+{
+    if (!flux || n_stars < 0 || n_cadences < 0 || W < 1 || (W & 1) == 0 || n_iter < 0 ||
+        !(alpha > 0.0) || !(c > 0.0) || scale_kind < 0 || scale_kind > 1 || weight_kind < 0 || weight_kind > 1)
+        return 1;
+    const int mv = resolve_min_valid(W, min_valid);
+    const int64_t h = (W - 1) / 2;
+    const int64_t total = n_stars * n_cadences;
+    int bad = 0;
+#pragma omp parallel
+    {
+        double *work = (double *)malloc((size_t)2 * (size_t)W * sizeof(double));
+#pragma omp for schedule(dynamic, 256)
+        for (int64_t q = 0; q < total; ++q) {
+            if (!work) {
+#pragma omp atomic write
+                bad = 1;
+                continue;
+            }
+            const int64_t b = q / n_cadences, i = q % n_cadences;
+            const float *frow = flux + b * n_cadences;
+            const double *trow = time ? time + b * n_cadences : NULL;
+            int n = 0;
+            for (int64_t j = i - h; j <= i + h; ++j)
+                if (slot_valid(trow, frow, n_cadences, j)) work[n++] = (double)frow[j];
+            if (n_valid) n_valid[q] = n;
+            double t64;
+            oracle_location_family(work, n, slot_valid(trow, frow, n_cadences, i), scale_kind, weight_kind,
+                                   alpha, c, n_iter, mv, cutoff_tol, work + W,
+                                   &t64, median ? median + q : NULL, scale ? scale + q : NULL,
+                                   n_plus ? n_plus + q : NULL, near_cutoff ? near_cutoff + q : NULL);
+            if (trend64) trend64[q] = t64;
+            if (trend32) trend32[q] = (float)t64;
+        }
+        free(work);
+    }
     return bad;
 }
 

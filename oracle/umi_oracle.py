@@ -57,6 +57,11 @@ def lib():
             _c_i64_p, _c_i64_p, ctypes.c_int64,
             ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
             ctypes.c_double] + outs
+        L.umi_oracle_family.restype = ctypes.c_int
+        L.umi_oracle_family.argtypes = [
+            _c_double_p, _c_float_p, ctypes.c_int64, ctypes.c_int64,
+            ctypes.c_int, ctypes.c_int, ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_int,
+            ctypes.c_int, ctypes.c_double] + outs
         L.umi_oracle_normalize.restype = ctypes.c_int
         L.umi_oracle_normalize.argtypes = [_c_float_p, _c_double_p, ctypes.c_int64, _c_double_p]
         L.umi_oracle_gapped.restype = ctypes.c_int
@@ -175,4 +180,23 @@ def gapped(time, flux, t0, dt, n_grid, W, alpha=2.0, n_iter=5, c=5.0, min_valid=
         int(W), float(alpha), float(c), int(n_iter), int(min_valid), float(cutoff_tol), *_out_ptrs(r))
     if rc != 0:
         raise ValueError("umi_oracle_gapped: invalid arguments")
+    return r
+
+
+SCALE_UPPER_RMS, SCALE_MAD = 0, 1
+WEIGHT_BISQUARE, WEIGHT_WELSCH = 0, 1
+
+
+def family(flux, W, scale_kind=0, weight_kind=0, alpha=2.0, n_iter=5, c=5.0, time=None, min_valid=-1,
+           cutoff_tol=1e-5) -> OracleResult:
+    """Sibling estimators: MAD scale and/or Welsch weights on the same windows."""
+    flux, time, tp = _prep(flux, time)
+    S, N = flux.shape
+    r = _alloc((S, N))
+    r.n_plus[...] = 0
+    rc = lib().umi_oracle_family(
+        tp, flux.ctypes.data_as(_c_float_p), S, N, int(W), int(scale_kind), int(weight_kind),
+        float(alpha), float(c), int(n_iter), int(min_valid), float(cutoff_tol), *_out_ptrs(r))
+    if rc != 0:
+        raise ValueError("umi_oracle_family: invalid arguments")
     return r

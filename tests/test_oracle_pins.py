@@ -468,3 +468,104 @@ def test_gapped_on_uniform_times_is_the_positional_window():
     a = orc.gapped(t, x, 5.0, 0.01, 500, 21)
     b = orc.detrend(x, 21)
     np.testing.assert_array_equal(a.trend64, b.trend64)
+
+
+# ---------------------------------------------------------------- next row F4: sibling estimators (MAD scale, Welsch weights)
+def test_family_default_is_the_paper_estimator():
+    from workloads import lightcurves as lc
+    x = lc.random_series(12, 2, 600)
+    a, b = orc.family(x, 25, 0, 0), orc.detrend(x, 25)
+    np.testing.assert_array_equal(a.trend64, b.trend64)
+    np.testing.assert_array_equal(a.scale, b.scale)
+
+
+def test_mad_scale_library_routine_and_gaussian_constant():
+    # n_iter = 0 leaves (median, s); the MAD of an odd gap-free window is scipy's routine
+    rng = np.random.default_rng(11)
+    x = rng.normal(1.0, 2e-3, (1, 801)).astype(np.float32)
+    r = orc.family(x, 51, orc.SCALE_MAD, 0, n_iter=0)
+    for i in (25, 26, 400, 775):
+        win = x[0, i - 25:i + 26].astype(np.float64)
+        assert r.scale[0, i] == scipy.stats.median_abs_deviation(win)
+    # 0.6745 sigma is "the MAD convention at the Gaussian model"
+    big = rng.normal(0.0, 1.0, 200001).astype(np.float32)
+    rr = orc.family(big[None, 99000:101001].copy(), 2001, orc.SCALE_MAD, 0, n_iter=0)
+    full = orc.positions(big, [0], [100000], W=200001, n_iter=0)        # reference sigma_upper ~ 1
+    mad = np.sort(np.abs(big.astype(np.float64) - np.median(big)))[100000]
+    assert abs(mad - scipy.stats.norm.ppf(0.75)) < 0.01 and abs(0.6745 - scipy.stats.norm.ppf(0.75)) < 1e-4
+    assert abs(full.scale[0] / 0.6745 - 1.0) < 0.01 and np.isfinite(rr.scale[0, 1000])
+
+
+@pytest.mark.parametrize("sk,wk", [(0, 1), (1, 0), (1, 1)])
+def test_family_brute_force_with_gaps(sk, wk):
+    from workloads import lightcurves as lc
+    x = lc.random_series(90 + sk * 2 + wk, 2, 160, nan_frac=0.08, inf_frac=0.02)
+    for W, alpha in ((7, 2.0), (15, 1.0), (31, 3.0)):
+        r = orc.family(x, W, sk, wk, alpha=alpha)
+        h = (W - 1) // 2
+        for b in range(2):
+            for i in range(160):
+                win = brute.window_samples(x[b], i, W)
+                if not np.isfinite(x[b, i]) or win.size < max(1, W // 3):
+                    assert np.isnan(r.trend64[b, i])
+                    continue
+                mu, med, s = brute.location_family(win, "mad" if sk else "upper_rms",
+                                                   "welsch" if wk else "bisquare", alpha=alpha)
+                assert r.median[b, i] == np.float32(med)
+                assert r.scale[b, i] == pytest.approx(s, rel=1e-13, abs=0.0)
+                assert r.trend64[b, i] == pytest.approx(mu, rel=1e-12)
+
+
+def test_welsch_worked_example_and_limits():
+    # x = {0,1,2,3,4}, MAD scale: median 2, deviations {2,1,0,1,2} -> MAD = 1; c = 5, alpha = 2:
+    # u = (x-2)/5, u_eff = {-.8,-.4,0,.2,.4}, w = exp(-u_eff^2); one pass by hand
+    x = np.array([[0, 1, 2, 3, 4]], np.float32)
+    w = [math.exp(-0.64), math.exp(-0.16), 1.0, math.exp(-0.04), math.exp(-0.16)]
+    mu1 = sum(wi * xi for wi, xi in zip(w, range(5))) / sum(w)
+    r = orc.family(x, 5, orc.SCALE_MAD, orc.WEIGHT_WELSCH, alpha=2.0, n_iter=1, min_valid=5)
+    assert r.scale[0, 2] == 1.0 and r.median[0, 2] == 2.0
+    assert r.trend64[0, 2] == pytest.approx(mu1, rel=1e-15) and abs(mu1 - 2.180888) < 1e-6
+    # symmetric data, alpha = 1: the location stays at the centre for both weights and both scales
+    for sk in (0, 1):
+        for wk in (0, 1):
+            assert orc.family(x, 5, sk, wk, alpha=1.0, min_valid=5).trend64[0, 2] == pytest.approx(2.0, abs=1e-15)
+    # c -> infinity: every weight -> 1, one pass gives the window mean
+    rng = np.random.default_rng(3)
+    y = rng.normal(1.0, 1e-2, (1, 41)).astype(np.float32)
+    big = orc.family(y, 41, orc.SCALE_MAD, orc.WEIGHT_WELSCH, c=1e9, n_iter=1)
+    assert big.trend64[0, 20] == pytest.approx(y.astype(np.float64).mean(), rel=1e-12)
+
+
+def test_mad_biweight_invariants():
+    rng = np.random.default_rng(8)
+    x = (1.0 + 1e-3 * rng.standard_normal((1, 400))).astype(np.float32)
+    for wk in (0, 1):
+        r = orc.family(x, 41, orc.SCALE_MAD, wk, alpha=1.0)
+        # two-sided scale + symmetric weights: reflection equivariance on interior odd windows
+        m = orc.family((-x).astype(np.float32), 41, orc.SCALE_MAD, wk, alpha=1.0)
+        np.testing.assert_allclose(m.trend64[0, 20:-20], -r.trend64[0, 20:-20], rtol=1e-13)
+        # positive affine map (power of two: exact)
+        a = orc.family((4.0 * x).astype(np.float32), 41, orc.SCALE_MAD, wk, alpha=1.0)
+        np.testing.assert_array_equal(a.trend64, 4.0 * r.trend64)
+        # fixed point of the estimating equation after many passes
+        f = orc.family(x, 41, orc.SCALE_MAD, wk, alpha=1.0, n_iter=300)
+        i = 200
+        win = x[0, i - 20:i + 21].astype(np.float64)
+        u = (win - f.trend64[0, i]) / (5.0 * f.scale[0, i])
+        wgt = np.exp(-u ** 2) if wk else brute.bisquare_weights(u, 1.0)
+        assert abs(np.sum(wgt * (win - f.trend64[0, i]))) < 1e-12
+    cst = np.full((1, 100), 2.5, np.float32)
+    assert np.array_equal(orc.family(cst, 9, orc.SCALE_MAD, orc.WEIGHT_WELSCH).trend64, cst.astype(np.float64))
+
+
+def test_mad_is_inflated_by_a_deep_dip_but_upper_rms_is_not():
+    # "deep transits can inflate the [MAD] scale"; the upper-RMS never sees them
+    rng = np.random.default_rng(21)
+    x = (1.0 + 1e-3 * rng.standard_normal(201)).astype(np.float32)
+    y = x.copy()
+    lows = np.argsort(x)[:80]                      # 40 % of the window, all below the median
+    y[lows] -= 0.05
+    a0, a1 = (orc.family(v[None, :], 201, orc.SCALE_UPPER_RMS, 0, n_iter=0).scale[0, 100] for v in (x, y))
+    m0, m1 = (orc.family(v[None, :], 201, orc.SCALE_MAD, 0, n_iter=0).scale[0, 100] for v in (x, y))
+    assert a0 == a1
+    assert m1 > 1.5 * m0
