@@ -109,6 +109,33 @@ int umi_flatten(const double* time, const float* flux,
                 float* trend_out, float* flat_out, void* stream);
 
 /*
+ * Sibling estimators on the same window machinery: the scale and the
+ * weight function are selectable; everything else (window, validity, median start, n_iter
+ * passes of Eq. 2 + Eq. 4 with fixed s, c, alpha, min_valid) is umi_detrend_ex.
+ *   scale_kind   UMI_SCALE_UPPER_RMS  Eq. 1, s = 0.6745 sigma_upper (the paper's scale)
+ *                UMI_SCALE_MAD        s = median |x - median| over the window, both sides, the
+ *                                     "standard MAD" of PAPER.md:50 / the ablation of PAPER.md:91;
+ *                                     rank (n-1)/2 of the n deviations (R21), no extra factor
+ *   weight_kind  UMI_WEIGHT_BISQUARE  Eq. 3
+ *                UMI_WEIGHT_WELSCH    w = exp(-u_eff^2) ("Gaussian-shaped weights", R22)
+ * alpha = 1 with the MAD and bisquare weights is the classic symmetric biweight location.
+ *   scale_out  DEVICE, float [n_stars*n_cadences]: receives s per position (NaN where the trend
+ *              is NaN).  REQUIRED for UMI_SCALE_MAD (it carries the MAD from the selection
+ *              kernel to the reweighting kernel), optional (may be NULL) for the upper-RMS.
+ *   flat_out   DEVICE or NULL: flux / trend as in umi_flatten.
+ * Other arguments and errors as umi_detrend_ex; an unknown kind -> UMI_ERR_INVALID_ARG.
+ */
+#define UMI_SCALE_UPPER_RMS 0
+#define UMI_SCALE_MAD 1
+#define UMI_WEIGHT_BISQUARE 0
+#define UMI_WEIGHT_WELSCH 1
+int umi_detrend_family(const double* time, const float* flux,
+                       int64_t n_stars, int64_t n_cadences,
+                       int W, int scale_kind, int weight_kind,
+                       float alpha, float c, int n_iter, int min_valid,
+                       float* trend_out, float* scale_out, float* flat_out, void* stream);
+
+/*
  * Gap handling by time stamps ("gap handling", the stage in front of the
  * detrender; reading R20).  The rows are COMPACTED series: cadences were removed
  * upstream, so time jumps.  Sample (b, i) sits in slot k = rint((time[b, i] - t0) / dt)

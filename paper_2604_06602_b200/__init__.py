@@ -18,9 +18,11 @@ LIB_PATH = os.environ.get("UMI_B200_LIB") or os.path.join(_HERE, "libumi_b200.so
 
 UMI_OK, UMI_ERR_INVALID_ARG, UMI_ERR_UNSUPPORTED, UMI_ERR_CUDA = 0, 1, 2, 3
 UMI_MAX_WINDOW = 4097
+UMI_SCALE_UPPER_RMS, UMI_SCALE_MAD = 0, 1
+UMI_WEIGHT_BISQUARE, UMI_WEIGHT_WELSCH = 0, 1
 
 EXPORTS = ("umi_window_len", "umi_detrend", "umi_detrend_ex", "umi_detrend_host", "umi_detrend_profile",
-           "umi_flatten", "umi_detrend_gapped", "umi_gapped_workspace_bytes",
+           "umi_flatten", "umi_detrend_family", "umi_detrend_gapped", "umi_gapped_workspace_bytes",
            "umi_launch_geometry", "umi_status_string", "umi_version")
 
 _lib = None
@@ -55,6 +57,8 @@ def lib():
     L.umi_detrend_host.argtypes = [vp, vp, i64, i64, ci, cf, ci, vp, i64, ci]
     L.umi_flatten.restype = ci
     L.umi_flatten.argtypes = [vp, vp, i64, i64, ci, cf, cf, ci, ci, vp, vp, vp]
+    L.umi_detrend_family.restype = ci
+    L.umi_detrend_family.argtypes = [vp, vp, i64, i64, ci, ci, ci, cf, cf, ci, ci, vp, vp, vp, vp]
     L.umi_gapped_workspace_bytes.restype = ctypes.c_size_t
     L.umi_gapped_workspace_bytes.argtypes = [i64, i64]
     L.umi_detrend_gapped.restype = ci
@@ -172,6 +176,31 @@ def umi_flatten(time, flux, W, alpha=2.0, n_iter=5, c=5.0, min_valid=-1, stream=
                                      int(min_valid), trend.data_ptr(), flat.data_ptr(),
                                      _stream_ptr(stream, f.device)))
     return trend.view(flux.shape), flat.view(flux.shape)
+
+
+def umi_detrend_family(time, flux, W, scale_kind=0, weight_kind=0, alpha=2.0, n_iter=5, c=5.0, min_valid=-1,
+                       flat=False, stream=None):
+    """Sibling estimators (include/umi.h): MAD or upper-RMS scale, bisquare or Welsch weights.
+    Returns (trend, scale) or (trend, scale, flat)."""
+    import torch
+    f = _cuda_2d(flux, torch.float32, "flux")
+    tptr = None
+    if time is not None:
+        tt = _cuda_2d(time, torch.float64, "time")
+        if tt.shape != f.shape or tt.device != f.device:
+            raise ValueError("time must have flux's shape and device")
+        tptr = tt.data_ptr()
+    trend, scale = torch.empty_like(f), torch.empty_like(f)
+    fl = torch.empty_like(f) if flat else None
+    S, N = f.shape
+    if S and N:
+        with torch.cuda.device(f.device):
+            _check(lib().umi_detrend_family(tptr, f.data_ptr(), S, N, int(W), int(scale_kind), int(weight_kind),
+                                            float(alpha), float(c), int(n_iter), int(min_valid),
+                                            trend.data_ptr(), scale.data_ptr(), fl.data_ptr() if flat else None,
+                                            _stream_ptr(stream, f.device)))
+    out = (trend.view(flux.shape), scale.view(flux.shape))
+    return out + (fl.view(flux.shape),) if flat else out
 
 
 def umi_gapped_workspace_bytes(n_stars, n_grid):

@@ -16,6 +16,13 @@ namespace {
 
 constexpr int64_t MAX_GRID = 0x7FFFFFFF;
 
+/* sibling-estimator selection (F4); the default is the paper's path */
+struct Family {
+    bool on = false;
+    int scale_kind = umi::SCALE_UPPER_RMS, weight_kind = umi::WEIGHT_BISQUARE;
+    float* scale_out = nullptr;
+};
+
 struct Geometry {
     int T1, NS;            /* median kernel: positions per tile, sort length */
     size_t smem1;
@@ -66,10 +73,12 @@ int validate(const float* flux, int64_t n_stars, int64_t n_cadences, int W, floa
 int launch_device(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
                   int W, float alpha, float c, int n_iter, int min_valid, float* trend_out,
                   cudaStream_t stream, cudaEvent_t* ev = nullptr /* [3] or null */,
-                  float* flat_out = nullptr)
+                  float* flat_out = nullptr, const Family& fam = Family())
 {
     if (n_stars == 0 || n_cadences == 0) return UMI_OK;
-    const Geometry g = geometry_for(W);
+    Geometry g = geometry_for(W);
+    const bool mad = fam.on && fam.scale_kind == umi::SCALE_MAD;
+    if (mad) g.smem1 = umi::k1_smem_bytes(g.NS, true);
     if (min_valid < 0) min_valid = std::max(1, W / 3);      /* PAPER.md:192 (R4) */
 
     if (W <= umi::KS_MAX_WINDOW) {
@@ -86,11 +95,15 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.n_iter = n_iter;
         rp.alpha = alpha;
         rp.c = c;
+        rp.scale_in = nullptr;
+        rp.scale_out = fam.scale_out;
+        rp.weight_kind = fam.weight_kind;
+        rp.scale_kind = fam.scale_kind;
         const int wt = W <= 9 ? 9 : W <= 17 ? 17 : W <= 25 ? 25 : W <= 33 ? 33 : 49;
         const unsigned grid = (unsigned)std::min<int64_t>(rp.n_blocks, MAX_GRID);
         if (ev && (cuda_failed(cudaEventRecord(ev[0], stream)) || cuda_failed(cudaEventRecord(ev[1], stream))))
             return UMI_ERR_CUDA;
-        if (cuda_failed(umi::launch_small(rp, min_valid, wt, grid, stream))) return UMI_ERR_CUDA;
+        if (cuda_failed(umi::launch_small(rp, fam.on, min_valid, wt, grid, stream))) return UMI_ERR_CUDA;
         if (ev && cuda_failed(cudaEventRecord(ev[2], stream))) return UMI_ERR_CUDA;
         return UMI_OK;
     }
@@ -100,6 +113,7 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
     mp.flux = flux;
     mp.out = trend_out;
     mp.flat = (n_iter == 0) ? flat_out : nullptr;
+    mp.scale = mad ? fam.scale_out : nullptr;
     mp.N = n_cadences;
     mp.tiles_per_star = (n_cadences + g.T1 - 1) / g.T1;
     mp.n_blocks = n_stars * mp.tiles_per_star;
@@ -112,7 +126,10 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
     if (cuda_failed(umi::launch_median(mp, grid1, g.smem1, stream))) return UMI_ERR_CUDA;
     if (ev && cuda_failed(cudaEventRecord(ev[1], stream))) return UMI_ERR_CUDA;
 
-    if (n_iter > 0) {
+    /* the family path also runs the second kernel with n_iter = 0 when only the upper-RMS scale is wanted */
+    const bool scale_only = fam.on && !mad && fam.scale_out != nullptr && n_iter == 0;
+    if (scale_only) mp.flat = nullptr;
+    if (n_iter > 0 || scale_only) {
         umi::ReweightParams rp;
         rp.time = time;
         rp.flux = flux;
@@ -125,8 +142,12 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.n_iter = n_iter;
         rp.alpha = alpha;
         rp.c = c;
+        rp.scale_in = mad ? fam.scale_out : nullptr;
+        rp.scale_out = mad ? nullptr : fam.scale_out;
+        rp.weight_kind = fam.weight_kind;
+        rp.scale_kind = fam.scale_kind;
         const unsigned grid2 = (unsigned)std::min<int64_t>(rp.n_blocks, MAX_GRID);
-        if (cuda_failed(umi::launch_reweight(rp, grid2, g.smem2, stream))) return UMI_ERR_CUDA;
+        if (cuda_failed(umi::launch_reweight(rp, fam.on, grid2, g.smem2, stream))) return UMI_ERR_CUDA;
     }
     if (ev && cuda_failed(cudaEventRecord(ev[2], stream))) return UMI_ERR_CUDA;
     return UMI_OK;
@@ -163,6 +184,24 @@ int umi_flatten(const double* time, const float* flux, int64_t n_stars, int64_t 
     if (st != UMI_OK) return st;
     return launch_device(time, flux, n_stars, n_cadences, W, alpha, c, n_iter, min_valid, trend_out,
                          static_cast<cudaStream_t>(stream), nullptr, flat_out);
+}
+
+int umi_detrend_family(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
+                       int W, int scale_kind, int weight_kind, float alpha, float c, int n_iter, int min_valid,
+                       float* trend_out, float* scale_out, float* flat_out, void* stream)
+{
+    if (scale_kind != UMI_SCALE_UPPER_RMS && scale_kind != UMI_SCALE_MAD) return UMI_ERR_INVALID_ARG;
+    if (weight_kind != UMI_WEIGHT_BISQUARE && weight_kind != UMI_WEIGHT_WELSCH) return UMI_ERR_INVALID_ARG;
+    if (scale_kind == UMI_SCALE_MAD && scale_out == nullptr) return UMI_ERR_INVALID_ARG;
+    const int st = validate(flux, n_stars, n_cadences, W, alpha, c, n_iter, trend_out);
+    if (st != UMI_OK) return st;
+    Family fam;
+    fam.on = true;
+    fam.scale_kind = scale_kind;
+    fam.weight_kind = weight_kind;
+    fam.scale_out = scale_out;
+    return launch_device(time, flux, n_stars, n_cadences, W, alpha, c, n_iter, min_valid, trend_out,
+                         static_cast<cudaStream_t>(stream), nullptr, flat_out, fam);
 }
 
 size_t umi_gapped_workspace_bytes(int64_t n_stars, int64_t n_grid)

@@ -12,14 +12,19 @@ constexpr int K1_THREADS = 256;                  /* median kernel */
 constexpr int K1_MIN_SORT = 1024;                /* smallest per-tile sort length */
 /* walkers per tile of the median kernel and its dynamic shared memory (bytes) */
 __host__ __device__ constexpr int k1_walkers(int ns) { return (131072 / ns) > 32 ? (131072 / ns) : 32; }
-__host__ __device__ constexpr size_t k1_smem_bytes(int ns)
+__host__ __device__ constexpr size_t k1_smem_bytes(int ns, bool mad = false)
 {
     /* u64 sort entries + u16 ranks + max(rank bitsets [NW][NS/32+1] + scan offsets [NW/32][NS/32], f32 medians) */
     const size_t bw = (size_t)ns / 32, nw = (size_t)k1_walkers(ns);
     const size_t bits = 4 * (nw * (bw + 1) + (nw / 32) * bw);
     const size_t med = 4 * (size_t)ns;
-    return (size_t)ns * 10 + (bits > med ? bits : med);
+    /* the MAD variant stages one more fp32 per position (the scale) behind everything else */
+    return (size_t)ns * 10 + (bits > med ? bits : med) + (mad ? 4 * (size_t)ns : 0);
 }
+
+/* sibling estimators; values match include/umi.h */
+constexpr int SCALE_UPPER_RMS = 0, SCALE_MAD = 1;
+constexpr int WEIGHT_BISQUARE = 0, WEIGHT_WELSCH = 1;
 
 constexpr int KS_THREADS = 256;                  /* fused small-window kernel: one position per thread */
 constexpr int KS_MAX_WINDOW = 49;                /* windows up to this length take the fused kernel */
@@ -33,6 +38,7 @@ struct MedianParams {
     const float* flux;
     float* out;              /* median, NaN where the position has no trend */
     float* flat;             /* null, or flux / median (only set when the call stops after Phase 1) */
+    float* scale;            /* null, or MAD of the window (selects the MAD variant of the kernel) */
     int64_t N;               /* cadences per star */
     int64_t tiles_per_star;
     int64_t n_blocks;        /* n_stars * tiles_per_star */
@@ -44,6 +50,10 @@ struct ReweightParams {
     const float* flux;
     float* out;              /* in: median from the median kernel; out: trend */
     float* flat;             /* null, or flux / trend (PAPER.md:155 normalisation), NaN where trend is NaN */
+    const float* scale_in;   /* family kernels: null, or s per position (replaces Phase 2) */
+    float* scale_out;        /* family kernels: null, or receives s per position */
+    int weight_kind;         /* family kernels: WEIGHT_BISQUARE / WEIGHT_WELSCH */
+    int scale_kind;          /* fused short-window kernel only */
     int64_t N;
     int64_t tiles_per_star;
     int64_t n_blocks;
@@ -53,9 +63,10 @@ struct ReweightParams {
 
 /* Enqueue one kernel; return the launch status (cudaGetLastError). */
 cudaError_t launch_median(const MedianParams& prm, unsigned grid, size_t smem, cudaStream_t stream);
-cudaError_t launch_reweight(const ReweightParams& prm, unsigned grid, size_t smem, cudaStream_t stream);
+/* family = false: the paper's path (scale_in/scale_out/weight_kind ignored); true: the sibling-estimator variants */
+cudaError_t launch_reweight(const ReweightParams& prm, bool family, unsigned grid, size_t smem, cudaStream_t stream);
 /* fused kernel for W <= KS_MAX_WINDOW; wt = compiled wire count (9, 17, 25, 33 or 49) >= W */
-cudaError_t launch_small(const ReweightParams& prm, int min_valid, int wt, unsigned grid, cudaStream_t stream);
+cudaError_t launch_small(const ReweightParams& prm, bool family, int min_valid, int wt, unsigned grid, cudaStream_t stream);
 
 /* umi_regrid.cu: gap handling by time stamps (R20) */
 struct RegridParams {

@@ -108,7 +108,18 @@ __device__ __forceinline__ void bitonic_sort_blocked(uint64_t (&v)[E], uint64_t*
 
 } // namespace
 
-template <int E>
+/*
+ * MAD variant (R21): each walker also keeps the
+ * rank range [L, R] of the cnt = (n-1)/2 + 1 window members with the smallest |x - median|; the
+ * MAD is the larger of the two end deviations.  The range is contiguous in sorted order and
+ * contains the median, so a slide changes it by O(1) members: the leaving / entering sample,
+ * then grow / shrink / exchange steps at the two ends.
+ */
+struct MadRange {
+    int L, R, cnt;
+};
+
+template <int E, bool MAD>
 __global__ void __launch_bounds__(K1_THREADS)
 umi_median_kernel(MedianParams prm)
 {
@@ -123,6 +134,7 @@ umi_median_kernel(MedianParams prm)
     uint32_t* bits = reinterpret_cast<uint32_t*>(rank + NS);        /* [NW][BWP] rank bitsets, then ...   */
     uint32_t* boff = bits + NW * BWP;                               /* [NWB][BW] block offsets of the scan */
     float* medbuf = reinterpret_cast<float*>(bits);                 /* ... aliased: [T] medians of the tile */
+    float* sclbuf = reinterpret_cast<float*>(smem_raw + k1_smem_bytes(NS, false));   /* MAD only: [T] scales */
     __shared__ int s_nvu;
 
     const int W = prm.W;
@@ -258,13 +270,60 @@ umi_median_kernel(MedianParams prm)
             if (pend > Tact) pend = Tact;
             const uint32_t uW = (uint32_t)W;
             int p = pbeg;
+            MadRange mr = {0, 0, 0};
+            float mad = 0.f;
+            /* window members next to rank r, under the window of position q */
+            auto val = [&](int r) { return key_to_float((uint32_t)(srt[r] >> 32)); };
+            auto nextm = [&](int r, int q) {
+                do { ++r; } while (r < nvu && ((uint32_t)srt[r] - (uint32_t)q) >= uW);
+                return r;
+            };
+            auto prevm = [&](int r, int q) {
+                do { --r; } while (r >= 0 && ((uint32_t)srt[r] - (uint32_t)q) >= uW);
+                return r;
+            };
+            /* restore the invariant for window q (median rank rho, n members) and return the MAD */
+            auto mad_fix = [&](int q) {
+                if (n == 0) { mr.cnt = 0; return 0.f; }
+                const int target = ((n - 1) >> 1) + 1;              /* (R21) rank (n-1)/2 of the deviations */
+                if (mr.cnt == 0 || rho < mr.L || rho > mr.R) { mr.L = mr.R = rho; mr.cnt = 1; }
+                const float med = val(rho);
+                const float inf = INFINITY;
+                float dL = med - val(mr.L), dR = val(mr.R) - med;
+                int Lp = prevm(mr.L, q), Rn = nextm(mr.R, q);
+                float dLp = Lp >= 0 ? med - val(Lp) : inf, dRn = Rn < nvu ? val(Rn) - med : inf;
+                while (mr.cnt < target) {                           /* grow towards the nearer neighbour */
+                    if (dLp <= dRn) { mr.L = Lp; dL = dLp; Lp = prevm(mr.L, q); dLp = Lp >= 0 ? med - val(Lp) : inf; }
+                    else            { mr.R = Rn; dR = dRn; Rn = nextm(mr.R, q); dRn = Rn < nvu ? val(Rn) - med : inf; }
+                    ++mr.cnt;
+                }
+                while (mr.cnt > target) {                           /* drop the farther end */
+                    if (dL > dR || (dL == dR && mr.L != rho)) { Lp = mr.L; dLp = dL; mr.L = nextm(mr.L, q); dL = med - val(mr.L); }
+                    else                                      { Rn = mr.R; dRn = dR; mr.R = prevm(mr.R, q); dR = val(mr.R) - med; }
+                    --mr.cnt;
+                }
+                for (;;) {                                          /* exchange while an outside member is nearer */
+                    if (dL > dRn) {
+                        Lp = mr.L; dLp = dL; mr.L = nextm(mr.L, q); dL = med - val(mr.L);
+                        mr.R = Rn; dR = dRn; Rn = nextm(mr.R, q); dRn = Rn < nvu ? val(Rn) - med : inf;
+                    } else if (dR > dLp) {
+                        Rn = mr.R; dRn = dR; mr.R = prevm(mr.R, q); dR = val(mr.R) - med;
+                        mr.L = Lp; dL = dLp; Lp = prevm(mr.L, q); dLp = Lp >= 0 ? med - val(Lp) : inf;
+                    } else {
+                        break;
+                    }
+                }
+                return fmaxf(dL, dR);
+            };
+            if constexpr (MAD) mad = mad_fix(p);
             for (;;) {
                 /* emit position p (R4, R5) */
                 const bool own = rank[p + h] < nvu;
+                const bool has = own && n >= prm.min_valid && n > 0;
                 float m = __int_as_float(0x7FC00000);
-                if (own && n >= prm.min_valid && n > 0)
-                    m = key_to_float((uint32_t)(srt[rho] >> 32));
+                if (has) m = key_to_float((uint32_t)(srt[rho] >> 32));
                 medbuf[p] = m;
+                if constexpr (MAD) sclbuf[p] = has ? mad : __int_as_float(0x7FC00000);
                 if (++p >= pend) break;
                 /* slide to window p: union index p-1 leaves, p+W-1 enters */
                 const int ro = rank[p - 1], ri = rank[p + W - 1];
@@ -304,12 +363,28 @@ umi_median_kernel(MedianParams prm)
                     }
                 }
                 n = n2;
+                if constexpr (MAD) {
+                    /* the leaving / entering sample against the old range, then repair */
+                    /* (the entering one first: moving an end below may land on it) */
+                    if (mr.cnt > 0 && vi && ri > mr.L && ri < mr.R) ++mr.cnt;
+                    if (mr.cnt > 0 && vo && ro >= mr.L && ro <= mr.R) {
+                        if (--mr.cnt > 0) {
+                            if (ro == mr.L) mr.L = nextm(mr.L, p);
+                            if (ro == mr.R) mr.R = prevm(mr.R, p);
+                        }
+                    }
+                    mad = mad_fix(p);
+                }
             }
         }
         __syncthreads();
 
         float* orow = prm.out + star * prm.N + j0;
         for (int p = tid; p < Tact; p += K1_THREADS) orow[p] = medbuf[p];
+        if constexpr (MAD) {
+            float* srow = prm.scale + star * prm.N + j0;
+            for (int p = tid; p < Tact; p += K1_THREADS) srow[p] = sclbuf[p];
+        }
         if (prm.flat != nullptr) {                                  /* PAPER.md:155 normalisation, n_iter = 0 */
             float* flrow = prm.flat + star * prm.N + j0;
             for (int p = tid; p < Tact; p += K1_THREADS) {
@@ -324,11 +399,12 @@ umi_median_kernel(MedianParams prm)
 cudaError_t launch_median(const MedianParams& prm, unsigned grid, size_t smem, cudaStream_t stream)
 {
     void (*k1)(MedianParams) = nullptr;
+    const bool mad = prm.scale != nullptr;
     switch (prm.NS / K1_THREADS) {
-    case 4: k1 = umi_median_kernel<4>; break;
-    case 8: k1 = umi_median_kernel<8>; break;
-    case 16: k1 = umi_median_kernel<16>; break;
-    case 32: k1 = umi_median_kernel<32>; break;
+    case 4: k1 = mad ? umi_median_kernel<4, true> : umi_median_kernel<4, false>; break;
+    case 8: k1 = mad ? umi_median_kernel<8, true> : umi_median_kernel<8, false>; break;
+    case 16: k1 = mad ? umi_median_kernel<16, true> : umi_median_kernel<16, false>; break;
+    case 32: k1 = mad ? umi_median_kernel<32, true> : umi_median_kernel<32, false>; break;
     default: return cudaErrorInvalidValue;
     }
     if (smem > 48 * 1024) {

@@ -58,6 +58,17 @@ __device__ __forceinline__ void eval_weight(float x, float k, float c0, float na
     R = fmaf(w, a, R);
 }
 
+/* Sibling weight (F4; R22): Welsch, w = exp(-u_eff^2), no cut-off. */
+__device__ __forceinline__ void eval_welsch(float x, float k, float c0, float nalpha,
+                                            float& S, float& R)
+{
+    const float a = fmaf(x, k, c0);                  /* u */
+    const float e = fmaxf(a, a * nalpha);            /* |u_eff| */
+    const float w = exp2f(e * e * -1.4426950408889634f);   /* exp(-e^2); 0 for the sentinel (e >= 16) */
+    S += w;
+    R = fmaf(w, a, R);
+}
+
 #if UMI_K2_PACKED
 typedef unsigned long long f32x2;                    /* two fp32 in one 64-bit register pair */
 
@@ -134,6 +145,9 @@ __device__ __forceinline__ void eval_weight_group(f32x2 x01, f32x2 x23, const f3
 
 } // namespace
 
+/* MODE 0: the paper's path.  MODE 1: sibling estimators with bisquare weights (scale from a buffer
+   and / or written out).  MODE 2: the same with Welsch weights. */
+template <int MODE>
 __global__ void __launch_bounds__(K2_THREADS, UMI_K2_MIN_CTAS)
 umi_reweight_kernel(ReweightParams prm)
 {
@@ -186,7 +200,10 @@ umi_reweight_kernel(ReweightParams prm)
            mu >= tmin and s <= 0.6745 (tmax - tmin)  ("Sentinel") */
         float sent = 0.f;
         if (tmin <= tmax) {
-            sent = tmin - 2.f * (prm.c * SCALE_CONST / prm.alpha) * (tmax - tmin);
+            if constexpr (MODE == 0)
+                sent = tmin - 2.f * (prm.c * SCALE_CONST / prm.alpha) * (tmax - tmin);
+            else   /* s <= tmax - tmin for either scale; Welsch needs |u_eff| >= 16 for an exact 0 */
+                sent = tmin - (MODE == 2 ? 24.f : 2.f) * (prm.c / prm.alpha) * (tmax - tmin);
             sent = fmaxf(sent, -3.0e38f);
         }
         for (int u = tid; u < nx; u += K2_THREADS) {
@@ -208,6 +225,10 @@ umi_reweight_kernel(ReweightParams prm)
             mu[q] = act[q] ? med[q] : 0.f;
             kk[q] = 0.f;
             cs[q] = 0.f;
+            if constexpr (MODE != 0) {                              /* no trend, no scale */
+                if (prm.scale_in == nullptr && prm.scale_out != nullptr && j < prm.N && !act[q])
+                    prm.scale_out[star * prm.N + j] = qnan;
+            }
         }
         const float4* xs4 = reinterpret_cast<const float4*>(xs) + tid;
 
@@ -216,7 +237,8 @@ umi_reweight_kernel(ReweightParams prm)
             float ss[K2_NPOS], cnt[K2_NPOS];
 #pragma unroll
             for (int q = 0; q < K2_NPOS; ++q) { ss[q] = 0.f; cnt[q] = 0.f; }
-            for (int g = 0; g < G; ++g) {
+            const bool given = (MODE != 0) && prm.scale_in != nullptr;
+            for (int g = 0; g < (given ? 0 : G); ++g) {
                 const float4 v = xs4[g];
                 const float xv[4] = {v.x, v.y, v.z, v.w};
                 if (g >= g_lo && g <= g_hi) {
@@ -241,6 +263,15 @@ umi_reweight_kernel(ReweightParams prm)
                 if (on) {
                     s = SCALE_CONST * sqrtf(ss[q] / cnt[q]);
                     on = s > 0.f;
+                }
+                if constexpr (MODE != 0) {
+                    const int64_t j = j0 + 4 * tid + q;
+                    if (given) {                                    /* the MAD from the selection kernel */
+                        s = (act[q] && j < prm.N) ? prm.scale_in[star * prm.N + j] : 0.f;
+                        on = act[q] && s > 0.f;
+                    } else if (prm.scale_out != nullptr && j < prm.N && act[q]) {
+                        prm.scale_out[star * prm.N + j] = s;
+                    }
                 }
                 act[q] = on;
                 cs[q] = on ? prm.c * s : 0.f;
@@ -273,10 +304,24 @@ umi_reweight_kernel(ReweightParams prm)
 #pragma unroll
                         for (int r = 0; r < 4; ++r) {
                             const int o = 4 * g + r - delta - q;
-                            if (o >= 0 && o <= 2 * h) eval_weight(xv[r], kk[q], c0[q], nalpha, S[q], R[q]);
+                            if (o >= 0 && o <= 2 * h) {
+                                if constexpr (MODE == 2) eval_welsch(xv[r], kk[q], c0[q], nalpha, S[q], R[q]);
+                                else eval_weight(xv[r], kk[q], c0[q], nalpha, S[q], R[q]);
+                            }
                         }
                 }
                 /* interior groups: every sample belongs to all 4 windows */
+                if constexpr (MODE == 2) {
+#pragma unroll 2
+                    for (int g = g_lo; g <= g_hi; ++g) {
+                        const float4 v = xs4[g];
+                        const float xv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                        for (int q = 0; q < K2_NPOS; ++q)
+#pragma unroll
+                            for (int r = 0; r < 4; ++r) eval_welsch(xv[r], kk[q], c0[q], nalpha, S[q], R[q]);
+                    }
+                } else {
 #if UMI_K2_PACKED
 #pragma unroll K2_UNROLL
                 for (int g = g_lo; g <= g_hi; ++g) {
@@ -294,14 +339,17 @@ umi_reweight_kernel(ReweightParams prm)
                         for (int r = 0; r < 4; ++r) eval_weight(xv[r], kk[q], c0[q], nalpha, S[q], R[q]);
                 }
 #endif
+                }
 #pragma unroll
                 for (int q = 0; q < K2_NPOS; ++q) {
 #if UMI_K2_PACKED
-                    float s0, s1, r0, r1;
-                    unpack2(S2[q], s0, s1);
-                    unpack2(R2[q], r0, r1);
-                    S[q] += s0 + s1;
-                    R[q] += r0 + r1;
+                    if constexpr (MODE != 2) {
+                        float s0, s1, r0, r1;
+                        unpack2(S2[q], s0, s1);
+                        unpack2(R2[q], r0, r1);
+                        S[q] += s0 + s1;
+                        R[q] += r0 + r1;
+                    }
 #endif
                     if (act[q] && S[q] > 0.f) mu[q] = fmaf(R[q] / S[q], cs[q], mu[q]);   /* Eq. 4; (R11) */
                 }
@@ -326,9 +374,11 @@ umi_reweight_kernel(ReweightParams prm)
     }
 }
 
-cudaError_t launch_reweight(const ReweightParams& prm, unsigned grid, size_t smem, cudaStream_t stream)
+cudaError_t launch_reweight(const ReweightParams& prm, bool family, unsigned grid, size_t smem, cudaStream_t stream)
 {
-    umi_reweight_kernel<<<grid, K2_THREADS, smem, stream>>>(prm);
+    if (!family) umi_reweight_kernel<0><<<grid, K2_THREADS, smem, stream>>>(prm);
+    else if (prm.weight_kind == WEIGHT_WELSCH) umi_reweight_kernel<2><<<grid, K2_THREADS, smem, stream>>>(prm);
+    else umi_reweight_kernel<1><<<grid, K2_THREADS, smem, stream>>>(prm);
     return cudaGetLastError();
 }
 

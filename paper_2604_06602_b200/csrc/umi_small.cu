@@ -79,7 +79,9 @@ __device__ __forceinline__ void batcher_sort(float (&a)[N])
 
 } // namespace
 
-template <int WT>
+/* FAMILY = false: the paper's path.  true: sibling estimators (F4): MAD scale by a second network
+   on the absolute deviations (R21), Welsch weights (R22), optional scale output. */
+template <int WT, bool FAMILY>
 __global__ void __launch_bounds__(KS_THREADS)
 umi_small_kernel(ReweightParams prm, int min_valid)
 {
@@ -125,7 +127,10 @@ umi_small_kernel(ReweightParams prm, int min_valid)
         }
         float sent = 0.f;                                           /* DESIGN.md, "Sentinel" */
         if (tmin <= tmax) {
-            sent = tmin - 2.f * (prm.c * SCALE_CONST / prm.alpha) * (tmax - tmin);
+            if constexpr (!FAMILY)
+                sent = tmin - 2.f * (prm.c * SCALE_CONST / prm.alpha) * (tmax - tmin);
+            else   /* s <= tmax - tmin for either scale; Welsch needs |u_eff| >= 16 for an exact 0 */
+                sent = tmin - (prm.weight_kind == WEIGHT_WELSCH ? 24.f : 2.f) * (prm.c / prm.alpha) * (tmax - tmin);
             sent = fmaxf(sent, -3.0e38f);
         }
 
@@ -144,6 +149,7 @@ umi_small_kernel(ReweightParams prm, int min_valid)
         float a[WT];
         int n = WT;
         bool own_ok = true;
+        uint64_t okmask = ~0ull;                                    /* FAMILY: which wires are valid */
         if (__all_sync(0xFFFFFFFFu, all_ok)) {
 #pragma unroll
             for (int i = 0; i < WT; ++i) a[i] = x[i];
@@ -160,6 +166,7 @@ umi_small_kernel(ReweightParams prm, int min_valid)
                 if (i == h) own_ok = ok && (i < W);
                 a[i] = ok ? x[i] : ((seen < n_low) ? -INFINITY : INFINITY);
                 seen += ok ? 0 : 1;
+                if (!ok) okmask &= ~(1ull << i);
                 x[i] = ok ? x[i] : sent;
             }
         }
@@ -169,7 +176,24 @@ umi_small_kernel(ReweightParams prm, int min_valid)
         const bool has = in_row && own_ok && n >= min_valid && n > 0;   /* (R4, R5) */
 
         float mu = med;
-        if (prm.n_iter > 0 && __any_sync(0xFFFFFFFFu, has)) {
+        const bool want_scale = FAMILY && prm.scale_out != nullptr;
+        if ((prm.n_iter > 0 || want_scale) && __any_sync(0xFFFFFFFFu, has)) {
+            bool on;
+            float s = 0.f;
+            if (FAMILY && prm.scale_kind == SCALE_MAD) {
+                /* ---- MAD (R21): rank (n-1)/2 of the n absolute deviations, same padding trick ---- */
+                const int n_low = (WT - n + 1) >> 1;
+                int seen = 0;
+#pragma unroll
+                for (int i = 0; i < WT; ++i) {
+                    const bool ok = (okmask >> i) & 1ull;
+                    a[i] = ok ? fabsf(x[i] - med) : ((seen < n_low) ? -INFINITY : INFINITY);
+                    seen += ok ? 0 : 1;
+                }
+                batcher_sort<WT>(a);
+                s = a[(WT - 1) / 2];
+                on = has && s > 0.f;
+            } else {
             /* ---- Phase 2 (Eq. 1) ---- */
             float ss = 0.f, cnt = 0.f;
 #pragma unroll
@@ -179,12 +203,13 @@ umi_small_kernel(ReweightParams prm, int min_valid)
                 ss = fmaf(dp, dp, ss);
                 cnt += (d > 0.f) ? 1.f : 0.f;
             }
-            bool on = has && cnt > 0.f;                             /* (R8) */
-            float s = 0.f;
+            on = has && cnt > 0.f;                                  /* (R8) */
             if (on) {
                 s = SCALE_CONST * sqrtf(ss / cnt);
                 on = s > 0.f;
             }
+            }
+            if (want_scale && in_row) prm.scale_out[star * prm.N + j] = has ? s : qnan;
             const float cs = on ? prm.c * s : 0.f;
             const float k = on ? 1.f / cs : 0.f;
             /* ---- Phase 3 (Eq. 2-4) ---- */
@@ -196,8 +221,13 @@ umi_small_kernel(ReweightParams prm, int min_valid)
                     const float u = fmaf(x[i], k, c0);
                     const float b = u * nalpha;
                     const float e = fmaxf(u, b);
-                    const float t = __saturatef(fmaf(-e, e, 1.f));
-                    const float w = t * t;
+                    float w;
+                    if (FAMILY && prm.weight_kind == WEIGHT_WELSCH) {
+                        w = exp2f(e * e * -1.4426950408889634f);    /* (R22) exp(-u_eff^2) */
+                    } else {
+                        const float t = __saturatef(fmaf(-e, e, 1.f));
+                        w = t * t;
+                    }
                     if (i & 1) { S1 += w; R1 = fmaf(w, u, R1); }
                     else       { S0 += w; R0 = fmaf(w, u, R0); }
                 }
@@ -205,6 +235,7 @@ umi_small_kernel(ReweightParams prm, int min_valid)
                 if (on && S > 0.f) mu = fmaf(R / S, cs, mu);        /* Eq. 4; (R11) */
             }
         }
+        if (want_scale && in_row && !has) prm.scale_out[star * prm.N + j] = qnan;
         if (in_row) {
             orow[j] = has ? mu : qnan;
             if (prm.flat != nullptr)                                /* PAPER.md:155 normalisation */
@@ -214,18 +245,25 @@ umi_small_kernel(ReweightParams prm, int min_valid)
     }
 }
 
-cudaError_t launch_small(const ReweightParams& prm, int min_valid, int wt, unsigned grid, cudaStream_t stream)
+template <bool FAMILY>
+static cudaError_t launch_small_t(const ReweightParams& prm, int min_valid, int wt, unsigned grid, cudaStream_t stream)
 {
     const size_t smem = (size_t)(KS_THREADS + wt - 1) * sizeof(float);
     switch (wt) {
-    case 9: umi_small_kernel<9><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
-    case 17: umi_small_kernel<17><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
-    case 25: umi_small_kernel<25><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
-    case 33: umi_small_kernel<33><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
-    case 49: umi_small_kernel<49><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
+    case 9: umi_small_kernel<9, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
+    case 17: umi_small_kernel<17, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
+    case 25: umi_small_kernel<25, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
+    case 33: umi_small_kernel<33, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
+    case 49: umi_small_kernel<49, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
+}
+
+cudaError_t launch_small(const ReweightParams& prm, bool family, int min_valid, int wt, unsigned grid, cudaStream_t stream)
+{
+    return family ? launch_small_t<true>(prm, min_valid, wt, grid, stream)
+                  : launch_small_t<false>(prm, min_valid, wt, grid, stream);
 }
 
 } // namespace umi

@@ -87,6 +87,12 @@ def test_validation_happens_on_the_host():
     assert gap(ws=None) == umi.UMI_ERR_INVALID_ARG
     assert gap(wsb=95) == umi.UMI_ERR_INVALID_ARG      # 2 * 1 * 12 * 4 = 96 bytes needed
     assert gap(S=0) == umi.UMI_OK
+    fam = lambda **k: L.umi_detrend_family(None, one, k.get("S", 1), 10, 5, k.get("sk", 0), k.get("wk", 0), 2.0, 5.0, 5, -1,
+                                           one, k.get("scale", one), None, None)
+    assert fam(sk=2) == umi.UMI_ERR_INVALID_ARG
+    assert fam(wk=-1) == umi.UMI_ERR_INVALID_ARG
+    assert fam(sk=1, scale=None) == umi.UMI_ERR_INVALID_ARG    # the MAD needs its buffer
+    assert fam(S=0, scale=None) == umi.UMI_OK
     assert umi.umi_gapped_workspace_bytes(3, 100) == 2400
     assert umi.umi_gapped_workspace_bytes(0, 100) == 0
     for s in range(5):

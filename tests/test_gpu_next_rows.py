@@ -114,3 +114,75 @@ def test_gapped_tess_batch_stars_compacted(umi):
     torch.cuda.synchronize()
     parity.compare_trend(trend.cpu().numpy(), ref)
     _check_flat(flat.cpu().numpy(), f, ref)
+
+
+# ------------------------------------------------------------------ F4: sibling estimators
+def _family_case(umi, x, W, sk, wk, alpha=2.0, c=5.0, n_iter=5, time=None):
+    import torch
+    ref = orc.family(x, W, sk, wk, alpha=alpha, c=c, n_iter=n_iter, time=time)
+    t = None if time is None else _cuda(time, np.float64)
+    trend, scale, flat = umi.umi_detrend_family(t, _cuda(x, np.float32), W, sk, wk, alpha=alpha, c=c,
+                                                n_iter=n_iter, flat=True)
+    torch.cuda.synchronize()
+    trend, scale, flat = trend.cpu().numpy(), scale.cpu().numpy(), flat.cpu().numpy()
+    if n_iter == 0:
+        parity.compare_median(trend, ref.median)
+    else:
+        parity.compare_trend(trend, ref)
+    _check_flat(flat, x, ref)
+    # the scale: NaN pattern of the trend; the MAD is a difference of two samples (one fp32
+    # rounding), the upper-RMS an fp32 sum of squares
+    nan = np.isnan(ref.trend64)
+    assert np.array_equal(np.isnan(scale), nan)
+    want = ref.scale[~nan]
+    got = scale[~nan].astype(np.float64)
+    tol = 2e-7 if sk == 1 else 1e-5
+    assert np.all(np.abs(got - want) <= tol * np.abs(want)), np.abs(got / np.maximum(want, 1e-300) - 1).max()
+
+
+@pytest.mark.parametrize("W", [1, 5, 9, 25, 33, 49, 51, 217, 361, 1081])
+@pytest.mark.parametrize("sk,wk", [(0, 0), (1, 0), (0, 1), (1, 1)])
+def test_family_matches_oracle(umi, W, sk, wk):
+    x = lc.random_series(700 + W + 2 * sk + wk, 3, 3001)
+    _family_case(umi, x, W, sk, wk)
+
+
+@pytest.mark.parametrize("W", [25, 361])
+def test_family_median_and_scale_only(umi, W):
+    x = lc.random_series(41 + W, 2, 2500, nan_frac=0.03)
+    _family_case(umi, x, W, 1, 0, n_iter=0)
+    _family_case(umi, x, W, 0, 0, n_iter=0)
+
+
+@pytest.mark.parametrize("W", [25, 361])
+def test_family_heavy_ties_and_presets(umi, W):
+    x = lc.random_series(300 + W, 2, 2500, nan_frac=0.02, inf_frac=0.0, ties=True)
+    _family_case(umi, x, W, 1, 0, alpha=1.0)          # classic symmetric biweight (MAD)
+    _family_case(umi, x, W, 1, 1, alpha=1.0, c=2.5)
+    y = lc.random_series(17, 2, 2000, nan_frac=0.02)
+    _family_case(umi, y, W, 1, 0, alpha=10.0, c=2.5)
+    _family_case(umi, y, W, 0, 1, alpha=3.0, n_iter=2)
+
+
+def test_family_large_window_and_config_stars(umi):
+    x = lc.random_series(8, 2, 9000, nan_frac=0.02)
+    _family_case(umi, x, 2161, 1, 0)
+    _family_case(umi, x, 4097, 1, 1)
+    cfg = lc.CONFIGS[2]
+    _family_case(umi, lc.stars(2, [5]), cfg.W, 1, 0, alpha=1.0)
+    _family_case(umi, lc.stars(3, [2])[:, :20000], 25, 1, 0, alpha=1.0)
+
+
+def test_family_constant_and_degenerate(umi):
+    import torch
+    x = np.full((2, 1200), 1.25, np.float32)
+    for W in (9, 361):
+        for sk in (0, 1):
+            trend, scale = umi.umi_detrend_family(None, _cuda(x, np.float32), W, sk, 1)
+            torch.cuda.synchronize()
+            assert np.array_equal(trend.cpu().numpy(), x)
+            assert np.array_equal(scale.cpu().numpy(), np.zeros_like(x))
+    x = np.full((1, 800), np.nan, np.float32)
+    trend, scale = umi.umi_detrend_family(None, _cuda(x, np.float32), 51, 1, 0)
+    torch.cuda.synchronize()
+    assert np.isnan(trend.cpu().numpy()).all() and np.isnan(scale.cpu().numpy()).all()

@@ -21,10 +21,15 @@ from workloads import lightcurves as lc
 DEPTHS_PPM = (5.0, 50.0, 100.0, 200.0, 500.0, 1000.0)        # PAPER.md:121, 131 (table columns)
 PERIOD_DAYS = 3.0
 DURATION_DAYS = 3.0 / 24.0
-SETTINGS = {                                                 # PAPER.md:202-209 (Table 4)
-    "UMI default (alpha=2, c=5)": dict(alpha=2.0, c=5.0),
-    "UMI aggressive (alpha=10, c=2.5)": dict(alpha=10.0, c=2.5),
-    "symmetric, upper-RMS scale (alpha=1, c=5)": dict(alpha=1.0, c=5.0),
+SETTINGS = {                                                 # PAPER.md:202-209 (Table 4); scale/weight kinds: include/umi.h
+    "UMI default (alpha=2, c=5)": dict(alpha=2.0, c=5.0, scale_kind=0, weight_kind=0),
+    "UMI aggressive (alpha=10, c=2.5)": dict(alpha=10.0, c=2.5, scale_kind=0, weight_kind=0),
+    "symmetric, upper-RMS scale (alpha=1, c=5)": dict(alpha=1.0, c=5.0, scale_kind=0, weight_kind=0),
+    # the rows the paper takes from wotan, here as the sibling estimators of row F4
+    "biweight, MAD scale (alpha=1, c=5)": dict(alpha=1.0, c=5.0, scale_kind=1, weight_kind=0),
+    "Welsch, MAD scale (alpha=1, c=5)": dict(alpha=1.0, c=5.0, scale_kind=1, weight_kind=1),
+    # the ablation of PAPER.md:91: UMI's asymmetric weights on the MAD instead of the upper-RMS
+    "UMI weights on the MAD (alpha=2, c=5)": dict(alpha=2.0, c=5.0, scale_kind=1, weight_kind=0),
 }
 
 
@@ -83,7 +88,8 @@ def main():
     rows = {}
     for name, kw in SETTINGS.items():
         def flatten(x, kw=kw):
-            _, flat = umi.umi_flatten(None, torch.from_numpy(x).cuda(), cfg.W, n_iter=cfg.n_iter, **kw)
+            _, _, flat = umi.umi_detrend_family(None, torch.from_numpy(x).cuda(), cfg.W, n_iter=cfg.n_iter,
+                                                flat=True, **kw)
             return flat.cpu().numpy()
         rows[name] = depth_errors(flux, cfg.dt_days, flatten, differential=not a.raw)
     print(json.dumps({"config": cfg.name, "stars": a.stars, "W": cfg.W, "depths_ppm": DEPTHS_PPM,
