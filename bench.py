@@ -48,6 +48,9 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, choices=sorted(lc.CONFIGS))
     ap.add_argument("--stars", type=int, default=None, help="override the star count (debug)")
+    ap.add_argument("--row", default="base", choices=["base", "f1", "f2", "f4mad", "f4welsch"],
+                    help="SURVEY.md 8(f) next rows on the same workload: f1 = umi_flatten, f2 = umi_detrend_gapped on the "
+                         "compacted rows, f4mad / f4welsch = umi_detrend_family (symmetric biweight on the MAD / Welsch)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     return ap.parse_args()
@@ -320,13 +323,88 @@ def run_ours(args, cfg, rank, world, local_rank):
                    % (args.config, cfg.name, S, N, W, cfg.alpha, cfg.n_iter),
                    "l2": "256 MiB buffer written between timed iterations",
                    "timing": "CUDA events on the launch stream, per step, summed; max over ranks"},
-        "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * args.steps,
+        "clocks": clocks, "e2e": e2e, "gpu_launches": (1 if W <= 49 else 2) * args.steps,
         "roofline": roofline, "cpu_baseline": cpu,
         "paper_context": "PAPER.md:147: 3.4 ms/star on AMD RX 9060 XT (~5.7e6 cadences/s at N=19440); not a target",
     }
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()
+
+
+def run_row(args, cfg, local_rank):
+    """Next rows on the configured workload, one GPU: device-resident step time with
+    CUDA events, L2 flushed between iterations, next to the base path timed the same way."""
+    import torch
+    import paper_2604_06602_b200 as umi
+    umi.lib()
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    S = cfg.n_stars if args.stars is None else args.stars
+    N, W = cfg.n_cadences, cfg.W
+    flux_np = lc.stars(args.config, range(S))
+    d_flux = torch.from_numpy(flux_np).to(dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+    stream = torch.cuda.Stream(dev)
+    kw = dict(alpha=cfg.alpha, n_iter=cfg.n_iter)
+    extra = {}
+    if args.row == "f1":
+        fn = lambda: umi.umi_flatten(None, d_flux, W, stream=stream, **kw)
+        what = "umi_flatten: trend + flux/trend in the kernels' epilogue"
+    elif args.row == "f2":
+        t_np, f_np, _ = lc.compact(flux_np, cfg.dt_days, t0=1000.0, jitter=0.1, seed=args.config)
+        d_t, d_f = torch.from_numpy(t_np).to(dev), torch.from_numpy(f_np).to(dev)
+        ws = torch.empty(umi.umi_gapped_workspace_bytes(S, N), dtype=torch.uint8, device=dev)
+        fn = lambda: umi.umi_detrend_gapped(d_t, d_f, 1000.0, cfg.dt_days, N, W, flat=True, workspace=ws,
+                                            stream=stream, **kw)
+        what = "umi_detrend_gapped: compacted rows [%d x %d] + fp64 time -> grid [%d x %d] -> trend, flat" % (
+            S, f_np.shape[1], S, N)
+        M = f_np.shape[1]
+        # algorithmic bytes of the two regrid kernels + the NaN fill: scatter reads time (8) + flux (4) per
+        # sample and writes 4 per valid sample; the fill writes 4 per slot; gather reads time (8) + flux (4)
+        # + trend (4) and writes trend (4) + flat (4)
+        extra["regrid_bytes"] = int(S * M * (12 + 4) + S * N * 4 + S * M * (16 + 8))
+    else:
+        wk = 1 if args.row == "f4welsch" else 0
+        fn = lambda: umi.umi_detrend_family(None, d_flux, W, 1, wk, alpha=1.0, n_iter=cfg.n_iter, stream=stream)
+        what = "umi_detrend_family: MAD scale, %s weights, alpha=1" % ("Welsch" if wk else "bisquare")
+    base = lambda: umi.umi_detrend(None, d_flux, W, stream=stream, **kw)
+
+    def timed(f):
+        with torch.cuda.stream(stream):
+            for _ in range(max(args.warmup, 3)):
+                flush.zero_()
+                f()
+        torch.cuda.synchronize()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+        with torch.cuda.stream(stream):
+            for a, b in ev:
+                flush.zero_()
+                a.record(stream)
+                f()
+                b.record(stream)
+        torch.cuda.synchronize()
+        return float(np.mean([a.elapsed_time(b) for a, b in ev]))
+
+    sampler = ClockSampler(local_rank, period=0.01)
+    sampler.start()
+    base_ms = timed(base)
+    row_ms = timed(fn)
+    clocks = sampler.stop()
+    n_cad = int(np.isfinite(flux_np).sum()) if args.row == "f2" else S * N
+    line = {"metric": METRIC, "row": args.row, "what": what, "value": n_cad / (row_ms * 1e-3), "unit": UNIT,
+            "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": row_ms,
+            "base_path_ms_per_step": base_ms, "overhead_ms": row_ms - base_ms, "higher_is_better": True,
+            "dtype": "f32", "data": "synthetic", "clocks": clocks,
+            "config": {"workload": "config%d %s: %d stars x %d cadences, W=%d" % (args.config, cfg.name, S, N, W),
+                       "l2": "256 MiB buffer written between timed iterations"}}
+    if "regrid_bytes" in extra and row_ms > base_ms:
+        pk, _ = peaks()
+        gbs = extra["regrid_bytes"] / ((row_ms - base_ms) * 1e-3) / 1e9
+        line["roofline_regrid"] = {"bound": "hbm", "achieved": gbs, "peak": pk.get("hbm_gbs"), "unit": "GB/s",
+                                   "frac": gbs / pk.get("hbm_gbs"), "bytes": extra["regrid_bytes"],
+                                   "note": "fill + scatter + gather, time = row step - base step"}
+    print(json.dumps(line))
 
 
 def main():
@@ -337,6 +415,9 @@ def main():
     cfg = lc.CONFIGS[args.config]
     if args.impl == "reference":
         run_reference(args, cfg, rank)
+    elif args.row != "base":
+        if rank == 0:
+            run_row(args, cfg, local_rank)
     else:
         run_ours(args, cfg, rank, world, local_rank)
 

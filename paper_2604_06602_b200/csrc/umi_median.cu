@@ -126,7 +126,12 @@ umi_median_kernel(MedianParams prm)
     constexpr int NS = K1_THREADS * E;
     constexpr int BW = NS / 32;                                     /* bitset words per walker */
     constexpr int BWP = BW + 1;                                     /* padded row stride: conflict-free both ways */
-    constexpr int NW = k1_walkers(NS);                              /* walkers per tile */
+#ifndef UMI_K1_MAD_WALKERS
+#define UMI_K1_MAD_WALKERS 128
+#endif
+    /* walkers per tile (measured on config 2: 32 / 64 / 128 MAD walkers -> 20.4 / 18.3 / 18.1 ms per step: the per-slide
+       range repair, not the O(W) set-up, is what costs, so the MAD variant keeps the same count) */
+    constexpr int NW = MAD ? (UMI_K1_MAD_WALKERS < k1_walkers(NS) ? UMI_K1_MAD_WALKERS : k1_walkers(NS)) : k1_walkers(NS);
     constexpr int NWB = NW / 32;                                    /* walker blocks of 32 */
     extern __shared__ __align__(16) unsigned char smem_raw[];
     uint64_t* srt = reinterpret_cast<uint64_t*>(smem_raw);          /* [NS] key<<32 | union index, sorted */
