@@ -29,39 +29,55 @@ namespace {
 
 constexpr int RG_THREADS = 256;
 
-/* slot of a time stamp, or -1 */
-__device__ __forceinline__ int64_t slot_of(double t, double t0, double dt, int64_t n_grid)
+/* rint((t - t0)/dt) as a double (NaN-free input assumed finite), no range check */
+__device__ __forceinline__ double raw_slot(double t, double t0, double dt)
 {
-    if (!finite_f64(t)) return -1;
-    const double k = rint(__ddiv_rn(__dsub_rn(t, t0), dt));   /* no contraction: same bits as the definition */
-    if (!(k >= 0.0) || !(k < (double)n_grid)) return -1;
-    return (int64_t)k;
+    return rint(__ddiv_rn(__dsub_rn(t, t0), dt));     /* no contraction: same bits as the definition */
 }
 
-/* slot of sample (row, i) with the collision rule applied (flux not looked at) */
+/*
+ * Slot of sample i of one row with the collision rule applied (flux not looked at).  One fp64
+ * division per sample: the successor's slot comes from the next lane by shuffle; only lane 31
+ * (and the last sample of a row) computes it itself.  All 32 lanes must call this together;
+ * lanes with i >= M pass a NaN time and get -1.
+ */
 __device__ __forceinline__ int64_t sample_slot(const double* __restrict__ trow, int64_t i, int64_t M,
                                                double t0, double dt, int64_t n_grid)
 {
-    const int64_t k = slot_of(__ldg(trow + i), t0, dt, n_grid);
-    if (k < 0) return -1;
-    if (i + 1 < M) {
-        const double tn = __ldg(trow + i + 1);
-        if (finite_f64(tn) && rint(__ddiv_rn(__dsub_rn(tn, t0), dt)) == (double)k) return -1;
+    const bool in_row = i < M;
+    const double t = in_row ? __ldg(trow + i) : __longlong_as_double(0x7FF8000000000000ll);
+    const bool fin = finite_f64(t);
+    const double k = fin ? raw_slot(t, t0, dt) : -1.0;
+    double kn = __shfl_down_sync(0xFFFFFFFFu, k, 1);
+    bool fin_n = __shfl_down_sync(0xFFFFFFFFu, (int)fin, 1) != 0;
+    if ((threadIdx.x & 31) == 31) {
+        fin_n = false;
+        if (i + 1 < M) {
+            const double tn = __ldg(trow + i + 1);
+            fin_n = finite_f64(tn);
+            if (fin_n) kn = raw_slot(tn, t0, dt);
+        }
     }
-    return k;
+    if (!fin || !(k >= 0.0) || !(k < (double)n_grid)) return -1;
+    if (fin_n && kn == k) return -1;                    /* the next sample lands in the same slot */
+    return (int64_t)k;
 }
 
+/* grid = (chunks of a row, stars): no 64-bit division per sample */
 __global__ void __launch_bounds__(RG_THREADS)
 umi_regrid_scatter_kernel(RegridParams prm, float* __restrict__ grid_flux)
 {
-    const int64_t total = prm.n_stars * prm.M;
-    for (int64_t q = (int64_t)blockIdx.x * RG_THREADS + threadIdx.x; q < total;
-         q += (int64_t)gridDim.x * RG_THREADS) {
-        const int64_t b = q / prm.M, i = q - b * prm.M;
-        const int64_t k = sample_slot(prm.time + b * prm.M, i, prm.M, prm.t0, prm.dt, prm.n_grid);
-        if (k < 0) continue;
-        const float x = __ldg(prm.flux + q);
-        if (finite_f32(x)) grid_flux[b * prm.n_grid + k] = x;
+    for (int64_t b = blockIdx.y; b < prm.n_stars; b += gridDim.y) {
+        const double* trow = prm.time + b * prm.M;
+        const float* frow = prm.flux + b * prm.M;
+        float* grow = grid_flux + b * prm.n_grid;
+        const int64_t Mr = (prm.M + 31) & ~(int64_t)31;             /* whole warps stay together */
+        for (int64_t i = (int64_t)blockIdx.x * RG_THREADS + threadIdx.x; i < Mr; i += (int64_t)gridDim.x * RG_THREADS) {
+            const int64_t k = sample_slot(trow, i, prm.M, prm.t0, prm.dt, prm.n_grid);
+            if (k < 0) continue;
+            const float x = __ldg(frow + i);
+            if (finite_f32(x)) grow[k] = x;
+        }
     }
 }
 
@@ -69,41 +85,46 @@ __global__ void __launch_bounds__(RG_THREADS)
 umi_regrid_gather_kernel(RegridParams prm, const float* __restrict__ grid_trend,
                          float* __restrict__ trend_out, float* __restrict__ flat_out)
 {
-    const int64_t total = prm.n_stars * prm.M;
     const float qnan = __int_as_float(0x7FC00000);
-    for (int64_t q = (int64_t)blockIdx.x * RG_THREADS + threadIdx.x; q < total;
-         q += (int64_t)gridDim.x * RG_THREADS) {
-        const int64_t b = q / prm.M, i = q - b * prm.M;
-        const int64_t k = sample_slot(prm.time + b * prm.M, i, prm.M, prm.t0, prm.dt, prm.n_grid);
-        const float x = __ldg(prm.flux + q);
-        float tr = qnan;
-        if (k >= 0 && finite_f32(x)) tr = __ldg(grid_trend + b * prm.n_grid + k);
-        trend_out[q] = tr;
-        if (flat_out != nullptr) flat_out[q] = (tr == tr) ? x / tr : qnan;
+    for (int64_t b = blockIdx.y; b < prm.n_stars; b += gridDim.y) {
+        const double* trow = prm.time + b * prm.M;
+        const float* frow = prm.flux + b * prm.M;
+        const float* grow = grid_trend + b * prm.n_grid;
+        const int64_t Mr = (prm.M + 31) & ~(int64_t)31;
+        for (int64_t i = (int64_t)blockIdx.x * RG_THREADS + threadIdx.x; i < Mr; i += (int64_t)gridDim.x * RG_THREADS) {
+            const int64_t k = sample_slot(trow, i, prm.M, prm.t0, prm.dt, prm.n_grid);
+            if (i >= prm.M) continue;
+            const float x = __ldg(frow + i);
+            float tr = qnan;
+            if (k >= 0 && finite_f32(x)) tr = __ldg(grow + k);
+            trend_out[b * prm.M + i] = tr;
+            if (flat_out != nullptr) flat_out[b * prm.M + i] = (tr == tr) ? x / tr : qnan;
+        }
     }
 }
 
-unsigned regrid_grid(int64_t total)
+dim3 regrid_grid(int64_t n_stars, int64_t M)
 {
-    int64_t blocks = (total + RG_THREADS - 1) / RG_THREADS;
-    const int64_t cap = 148 * 16;                       /* grid-stride: 16 CTAs of 256 per SM */
-    if (blocks > cap) blocks = cap;
-    if (blocks < 1) blocks = 1;
-    return (unsigned)blocks;
+    int64_t bx = (M + RG_THREADS - 1) / RG_THREADS;
+    if (bx < 1) bx = 1;
+    if (bx > 1024) bx = 1024;
+    int64_t by = n_stars < 1 ? 1 : n_stars;
+    if (by > 65535) by = 65535;
+    return dim3((unsigned)bx, (unsigned)by, 1);
 }
 
 } // namespace
 
 cudaError_t launch_regrid_scatter(const RegridParams& prm, float* grid_flux, cudaStream_t stream)
 {
-    umi_regrid_scatter_kernel<<<regrid_grid(prm.n_stars * prm.M), RG_THREADS, 0, stream>>>(prm, grid_flux);
+    umi_regrid_scatter_kernel<<<regrid_grid(prm.n_stars, prm.M), RG_THREADS, 0, stream>>>(prm, grid_flux);
     return cudaGetLastError();
 }
 
 cudaError_t launch_regrid_gather(const RegridParams& prm, const float* grid_trend, float* trend_out,
                                  float* flat_out, cudaStream_t stream)
 {
-    umi_regrid_gather_kernel<<<regrid_grid(prm.n_stars * prm.M), RG_THREADS, 0, stream>>>(prm, grid_trend,
+    umi_regrid_gather_kernel<<<regrid_grid(prm.n_stars, prm.M), RG_THREADS, 0, stream>>>(prm, grid_trend,
                                                                                          trend_out, flat_out);
     return cudaGetLastError();
 }
