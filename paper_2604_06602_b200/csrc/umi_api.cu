@@ -89,7 +89,7 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.out = trend_out;
         rp.flat = flat_out;
         rp.N = n_cadences;
-        rp.tiles_per_star = (n_cadences + umi::KS_THREADS - 1) / umi::KS_THREADS;
+        rp.tiles_per_star = (n_cadences + umi::KS_TILE - 1) / umi::KS_TILE;
         rp.n_blocks = n_stars * rp.tiles_per_star;
         rp.W = W;
         rp.n_iter = n_iter;

@@ -26,7 +26,8 @@ __host__ __device__ constexpr size_t k1_smem_bytes(int ns, bool mad = false)
 constexpr int SCALE_UPPER_RMS = 0, SCALE_MAD = 1;
 constexpr int WEIGHT_BISQUARE = 0, WEIGHT_WELSCH = 1;
 
-constexpr int KS_THREADS = 256;                  /* fused small-window kernel: one position per thread */
+constexpr int KS_THREADS = 128;                  /* fused small-window kernel: 4 consecutive positions per thread */
+constexpr int KS_TILE = 4 * KS_THREADS;          /* positions per CTA */
 constexpr int KS_MAX_WINDOW = 49;                /* windows up to this length take the fused kernel */
 
 constexpr int K2_THREADS = 128;                  /* reweighting kernel */

@@ -40,9 +40,10 @@ constexpr int K2_UNROLL = UMI_K2_UNROLL;
 __device__ __forceinline__ void eval_scale(float x, float med, float& ss, float& cnt)
 {
     const float d = x - med;
-    const float dp = fmaxf(d, 0.f);
-    ss = fmaf(dp, dp, ss);
-    cnt += (d > 0.f) ? 1.f : 0.f;
+    if (d > 0.f) {                                   /* one compare, two predicated updates */
+        ss = fmaf(d, d, ss);
+        cnt += 1.f;
+    }
 }
 
 /* Phase 3, one (sample, position): accumulates sum w and sum w*u. */

@@ -79,31 +79,170 @@ __device__ __forceinline__ void batcher_sort(float (&a)[N])
 
 } // namespace
 
-/* FAMILY = false: the paper's path.  true: sibling estimators (F4): MAD scale by a second network
-   on the absolute deviations (R21), Welsch weights (R22), optional scale output. */
+/*
+ * One position, general case (any number of valid samples, W <= WT): the window is read from
+ * shared memory at win[0 .. W).  FAMILY = false: the paper's path.  true: sibling estimators
+ * (F4): MAD scale by a second network on the absolute deviations (R21), Welsch weights (R22),
+ * optional scale output.  Called by all 32 lanes together (it votes).
+ */
+template <int WT, bool FAMILY>
+__device__ __noinline__ void small_position(const float* win, int W, float sent, const ReweightParams& prm,
+                                            int min_valid, bool in_row, int64_t gidx)
+{
+    const int h = (W - 1) >> 1;
+    const float nalpha = -prm.alpha;
+    const float qnan = __int_as_float(0x7FC00000);
+    float x[WT];
+    bool all_ok = (W == WT);
+#pragma unroll
+    for (int i = 0; i < WT; ++i) {
+        x[i] = (i < W) ? win[i] : qnan;
+        all_ok = all_ok && (x[i] == x[i]);
+    }
+
+    /* ---- Phase 1 ---- */
+    float a[WT];
+    int n = WT;
+    bool own_ok = true;
+    uint64_t okmask = ~0ull;                                    /* FAMILY: which wires are valid */
+    if (__all_sync(0xFFFFFFFFu, all_ok)) {
+#pragma unroll
+        for (int i = 0; i < WT; ++i) a[i] = x[i];
+    } else {
+        n = 0;
+#pragma unroll
+        for (int i = 0; i < WT; ++i) n += (x[i] == x[i]) ? 1 : 0;
+        const int n_low = (WT - n + 1) >> 1;                    /* wires sent to -inf */
+        int seen = 0;
+        own_ok = false;
+#pragma unroll
+        for (int i = 0; i < WT; ++i) {
+            const bool ok = (x[i] == x[i]);
+            if (i == h) own_ok = ok && (i < W);
+            a[i] = ok ? x[i] : ((seen < n_low) ? -INFINITY : INFINITY);
+            seen += ok ? 0 : 1;
+            if (!ok) okmask &= ~(1ull << i);
+            x[i] = ok ? x[i] : sent;
+        }
+    }
+    batcher_sort<WT>(a);
+    float med = a[(WT - 1) / 2];
+    med += 0.f;                                                 /* -0.0 -> +0.0 (R18) */
+    const bool has = in_row && own_ok && n >= min_valid && n > 0;   /* (R4, R5) */
+
+    float mu = med;
+    const bool want_scale = FAMILY && prm.scale_out != nullptr;
+    if ((prm.n_iter > 0 || want_scale) && __any_sync(0xFFFFFFFFu, has)) {
+        bool on;
+        float s = 0.f;
+        if (FAMILY && prm.scale_kind == SCALE_MAD) {
+            /* ---- MAD (R21): rank (n-1)/2 of the n absolute deviations, same padding trick ---- */
+            const int n_low = (WT - n + 1) >> 1;
+            int seen = 0;
+#pragma unroll
+            for (int i = 0; i < WT; ++i) {
+                const bool ok = (okmask >> i) & 1ull;
+                a[i] = ok ? fabsf(x[i] - med) : ((seen < n_low) ? -INFINITY : INFINITY);
+                seen += ok ? 0 : 1;
+            }
+            batcher_sort<WT>(a);
+            s = a[(WT - 1) / 2];
+            on = has && s > 0.f;
+        } else {
+        /* ---- Phase 2 (Eq. 1) ---- */
+        float ss = 0.f, cnt = 0.f;
+#pragma unroll
+        for (int i = 0; i < WT; ++i) {
+            const float d = x[i] - med;
+            const float dp = fmaxf(d, 0.f);
+            ss = fmaf(dp, dp, ss);
+            cnt += (d > 0.f) ? 1.f : 0.f;
+        }
+        on = has && cnt > 0.f;                                  /* (R8) */
+        if (on) {
+            s = SCALE_CONST * sqrtf(ss / cnt);
+            on = s > 0.f;
+        }
+        }
+        if (want_scale && in_row) prm.scale_out[gidx] = has ? s : qnan;
+        const float cs = on ? prm.c * s : 0.f;
+        const float k = on ? 1.f / cs : 0.f;
+        /* ---- Phase 3 (Eq. 2-4) ---- */
+        for (int it = 0; it < prm.n_iter; ++it) {
+            const float c0 = -mu * k;
+            float S0 = 0.f, S1 = 0.f, R0 = 0.f, R1 = 0.f;
+#pragma unroll
+            for (int i = 0; i < WT; ++i) {
+                const float u = fmaf(x[i], k, c0);
+                const float b = u * nalpha;
+                const float e = fmaxf(u, b);
+                float w;
+                if (FAMILY && prm.weight_kind == WEIGHT_WELSCH) {
+                    w = exp2f(e * e * -1.4426950408889634f);    /* (R22) exp(-u_eff^2) */
+                } else {
+                    const float t = __saturatef(fmaf(-e, e, 1.f));
+                    w = t * t;
+                }
+                if (i & 1) { S1 += w; R1 = fmaf(w, u, R1); }
+                else       { S0 += w; R0 = fmaf(w, u, R0); }
+            }
+            const float S = S0 + S1, R = R0 + R1;
+            if (on && S > 0.f) mu = fmaf(R / S, cs, mu);        /* Eq. 4; (R11) */
+        }
+    }
+    if (want_scale && in_row && !has) prm.scale_out[gidx] = qnan;
+    if (in_row) {
+        prm.out[gidx] = has ? mu : qnan;
+        if (prm.flat != nullptr)                                /* PAPER.md:155 normalisation */
+            prm.flat[gidx] = has ? win[h] / mu : qnan;
+    }
+}
+
+/* three values ascending */
+__device__ __forceinline__ void sort3(float& a, float& b, float& c)
+{
+    float t = fminf(a, b); b = fmaxf(a, b); a = t;
+    t = fminf(b, c); c = fmaxf(b, c); b = t;
+    t = fminf(a, b); b = fmaxf(a, b); a = t;
+}
+
+/*
+ * CTA = KS_TILE = 4 * KS_THREADS consecutive positions of one star; a thread owns 4 consecutive
+ * positions and the WT + 3 samples their windows share.
+ *
+ * Fast path (the paper's estimator, W == WT, every one of the thread's WT + 3 samples valid, decided
+ * per warp): the 4 windows have WT - 3 samples in common.  That core is sorted ONCE (only its
+ * ranks m-3 .. m are kept, m = (WT-1)/2, so most of the network is dead code); the median of a
+ * window is the 4th smallest of those four core values and its own 3 remaining samples:
+ *     med = min(C[m], max(C[m-1], e0), max(C[m-2], e1), max(C[m-3], e2)),   e0 <= e1 <= e2
+ * (the m-3 core values below C[m-3] are below everything that can be the answer).  Phases 2-3 then
+ * run on the registers, 4 independent positions interleaved.
+ * Any other case goes through small_position, one position at a time.
+ */
 template <int WT, bool FAMILY>
 __global__ void __launch_bounds__(KS_THREADS)
 umi_small_kernel(ReweightParams prm, int min_valid)
 {
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float* xs = reinterpret_cast<float*>(smem_raw);                 /* [KS_THREADS + WT - 1] */
+    float* xs = reinterpret_cast<float*>(smem_raw);                 /* [KS_TILE + WT - 1] */
     __shared__ float s_red[2 * (KS_THREADS / 32)];
 
+    constexpr int NSAMP = WT + 3;                                   /* multiple of 4 (WT = 1 mod 8) */
+    constexpr int M = (WT - 1) / 2;
     const int tid = threadIdx.x;
     const int W = prm.W;                                            /* odd, <= WT */
     const int h = (W - 1) >> 1;
-    const int nx = KS_THREADS + WT - 1;
+    const int nx = KS_TILE + WT - 1;
     const float nalpha = -prm.alpha;
     const float qnan = __int_as_float(0x7FC00000);
 
     for (int64_t bid = blockIdx.x; bid < prm.n_blocks; bid += gridDim.x) {
         const int64_t star = bid / prm.tiles_per_star;
         const int64_t tile = bid - star * prm.tiles_per_star;
-        const int64_t j0 = tile * KS_THREADS;
+        const int64_t j0 = tile * KS_TILE;
         const int64_t jbase = j0 - h;                               /* cadence of staged index 0 */
         const float* frow = prm.flux + star * prm.N;
         const double* trow = prm.time ? prm.time + star * prm.N : nullptr;
-        float* orow = prm.out + star * prm.N;
 
         /* stage; NaN marks invalid; tile min / max of the valid samples */
         float tmin = INFINITY, tmax = -INFINITY;
@@ -134,112 +273,102 @@ umi_small_kernel(ReweightParams prm, int min_valid)
             sent = fmaxf(sent, -3.0e38f);
         }
 
-        /* window of position j0 + tid: staged indices tid .. tid + W - 1 */
-        float x[WT];
-        bool all_ok = (W == WT);
+        const int64_t jq = j0 + 4 * tid;                            /* first of the thread's 4 positions */
+        bool fast = false;
+        if constexpr (!FAMILY) {
+            if (W == WT) {
+                /* all WT + 3 samples valid <=> all 4 windows complete (and inside the row) */
+                bool ok = true;
 #pragma unroll
-        for (int i = 0; i < WT; ++i) {
-            x[i] = (i < W) ? xs[tid + i] : qnan;
-            all_ok = all_ok && (x[i] == x[i]);
-        }
-        const int64_t j = j0 + tid;
-        const bool in_row = j < prm.N;
-
-        /* ---- Phase 1 ---- */
-        float a[WT];
-        int n = WT;
-        bool own_ok = true;
-        uint64_t okmask = ~0ull;                                    /* FAMILY: which wires are valid */
-        if (__all_sync(0xFFFFFFFFu, all_ok)) {
-#pragma unroll
-            for (int i = 0; i < WT; ++i) a[i] = x[i];
-        } else {
-            n = 0;
-#pragma unroll
-            for (int i = 0; i < WT; ++i) n += (x[i] == x[i]) ? 1 : 0;
-            const int n_low = (WT - n + 1) >> 1;                    /* wires sent to -inf */
-            int seen = 0;
-            own_ok = false;
-#pragma unroll
-            for (int i = 0; i < WT; ++i) {
-                const bool ok = (x[i] == x[i]);
-                if (i == h) own_ok = ok && (i < W);
-                a[i] = ok ? x[i] : ((seen < n_low) ? -INFINITY : INFINITY);
-                seen += ok ? 0 : 1;
-                if (!ok) okmask &= ~(1ull << i);
-                x[i] = ok ? x[i] : sent;
-            }
-        }
-        batcher_sort<WT>(a);
-        float med = a[(WT - 1) / 2];
-        med += 0.f;                                                 /* -0.0 -> +0.0 (R18) */
-        const bool has = in_row && own_ok && n >= min_valid && n > 0;   /* (R4, R5) */
-
-        float mu = med;
-        const bool want_scale = FAMILY && prm.scale_out != nullptr;
-        if ((prm.n_iter > 0 || want_scale) && __any_sync(0xFFFFFFFFu, has)) {
-            bool on;
-            float s = 0.f;
-            if (FAMILY && prm.scale_kind == SCALE_MAD) {
-                /* ---- MAD (R21): rank (n-1)/2 of the n absolute deviations, same padding trick ---- */
-                const int n_low = (WT - n + 1) >> 1;
-                int seen = 0;
-#pragma unroll
-                for (int i = 0; i < WT; ++i) {
-                    const bool ok = (okmask >> i) & 1ull;
-                    a[i] = ok ? fabsf(x[i] - med) : ((seen < n_low) ? -INFINITY : INFINITY);
-                    seen += ok ? 0 : 1;
+                for (int g = 0; g < NSAMP / 4; ++g) {
+                    const float4 v = reinterpret_cast<const float4*>(xs)[tid + g];
+                    ok = ok && (v.x == v.x) && (v.y == v.y) && (v.z == v.z) && (v.w == v.w);
                 }
-                batcher_sort<WT>(a);
-                s = a[(WT - 1) / 2];
-                on = has && s > 0.f;
-            } else {
-            /* ---- Phase 2 (Eq. 1) ---- */
-            float ss = 0.f, cnt = 0.f;
+                fast = __all_sync(0xFFFFFFFFu, ok) && WT >= min_valid;
+            }
+        }
+        if (fast) {
+            float s[NSAMP];
 #pragma unroll
-            for (int i = 0; i < WT; ++i) {
-                const float d = x[i] - med;
-                const float dp = fmaxf(d, 0.f);
-                ss = fmaf(dp, dp, ss);
-                cnt += (d > 0.f) ? 1.f : 0.f;
+            for (int g = 0; g < NSAMP / 4; ++g) {
+                const float4 v = reinterpret_cast<const float4*>(xs)[tid + g];
+                s[4 * g] = v.x; s[4 * g + 1] = v.y; s[4 * g + 2] = v.z; s[4 * g + 3] = v.w;
             }
-            on = has && cnt > 0.f;                                  /* (R8) */
-            if (on) {
-                s = SCALE_CONST * sqrtf(ss / cnt);
-                on = s > 0.f;
-            }
-            }
-            if (want_scale && in_row) prm.scale_out[star * prm.N + j] = has ? s : qnan;
-            const float cs = on ? prm.c * s : 0.f;
-            const float k = on ? 1.f / cs : 0.f;
-            /* ---- Phase 3 (Eq. 2-4) ---- */
-            for (int it = 0; it < prm.n_iter; ++it) {
-                const float c0 = -mu * k;
-                float S0 = 0.f, S1 = 0.f, R0 = 0.f, R1 = 0.f;
+            /* ---- Phase 1: shared core s[3 .. WT), sorted once ---- */
+            float core[WT - 3];
 #pragma unroll
-                for (int i = 0; i < WT; ++i) {
-                    const float u = fmaf(x[i], k, c0);
-                    const float b = u * nalpha;
-                    const float e = fmaxf(u, b);
-                    float w;
-                    if (FAMILY && prm.weight_kind == WEIGHT_WELSCH) {
-                        w = exp2f(e * e * -1.4426950408889634f);    /* (R22) exp(-u_eff^2) */
-                    } else {
-                        const float t = __saturatef(fmaf(-e, e, 1.f));
-                        w = t * t;
+            for (int i = 0; i < WT - 3; ++i) core[i] = s[3 + i];
+            batcher_sort<WT - 3>(core);
+            const float c0 = core[M - 3], c1 = core[M - 2], c2 = core[M - 1], c3 = core[M];
+            float med[4], mu[4];
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                /* the 3 samples of window q outside the core: s[q .. 3) and s[WT .. WT + q) */
+                float e0 = (q < 1) ? s[0] : s[WT + q - 1];
+                float e1 = (q < 2) ? s[1] : s[WT + q - 2];
+                float e2 = (q < 3) ? s[2] : s[WT + q - 3];
+                sort3(e0, e1, e2);
+                float m = fminf(fminf(c3, fmaxf(c2, e0)), fminf(fmaxf(c1, e1), fmaxf(c0, e2)));
+                m += 0.f;                                           /* -0.0 -> +0.0 (R18) */
+                med[q] = m;
+                mu[q] = m;
+            }
+            if (prm.n_iter > 0) {
+                /* ---- Phase 2 (Eq. 1) ---- */
+                float cs[4], k[4];
+                bool on[4];
+#pragma unroll
+                for (int q = 0; q < 4; ++q) {
+                    float ss = 0.f, cnt = 0.f;
+#pragma unroll
+                    for (int i = 0; i < WT; ++i) {
+                        const float d = s[q + i] - med[q];
+                        if (d > 0.f) {                              /* one compare, two predicated updates */
+                            ss = fmaf(d, d, ss);
+                            cnt += 1.f;
+                        }
                     }
-                    if (i & 1) { S1 += w; R1 = fmaf(w, u, R1); }
-                    else       { S0 += w; R0 = fmaf(w, u, R0); }
+                    on[q] = cnt > 0.f;                              /* (R8) */
+                    float sc = 0.f;
+                    if (on[q]) {
+                        sc = SCALE_CONST * sqrtf(ss / cnt);
+                        on[q] = sc > 0.f;
+                    }
+                    cs[q] = on[q] ? prm.c * sc : 0.f;
+                    k[q] = on[q] ? 1.f / cs[q] : 0.f;
                 }
-                const float S = S0 + S1, R = R0 + R1;
-                if (on && S > 0.f) mu = fmaf(R / S, cs, mu);        /* Eq. 4; (R11) */
+                /* ---- Phase 3 (Eq. 2-4) ---- */
+                for (int it = 0; it < prm.n_iter; ++it) {
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) {
+                        const float c0k = -mu[q] * k[q];
+                        float S0 = 0.f, S1 = 0.f, R0 = 0.f, R1 = 0.f;
+#pragma unroll
+                        for (int i = 0; i < WT; ++i) {
+                            const float u = fmaf(s[q + i], k[q], c0k);
+                            const float b = u * nalpha;
+                            const float e = fmaxf(u, b);
+                            const float t = __saturatef(fmaf(-e, e, 1.f));
+                            const float w = t * t;
+                            if (i & 1) { S1 += w; R1 = fmaf(w, u, R1); }
+                            else       { S0 += w; R0 = fmaf(w, u, R0); }
+                        }
+                        const float S = S0 + S1, R = R0 + R1;
+                        if (on[q] && S > 0.f) mu[q] = fmaf(R / S, cs[q], mu[q]);   /* Eq. 4; (R11) */
+                    }
+                }
             }
-        }
-        if (want_scale && in_row && !has) prm.scale_out[star * prm.N + j] = qnan;
-        if (in_row) {
-            orow[j] = has ? mu : qnan;
-            if (prm.flat != nullptr)                                /* PAPER.md:155 normalisation */
-                prm.flat[star * prm.N + j] = has ? xs[tid + h] / mu : qnan;
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+                const int64_t gi = star * prm.N + jq + q;
+                prm.out[gi] = mu[q];
+                if (prm.flat != nullptr) prm.flat[gi] = s[q + M] / mu[q];   /* PAPER.md:155 normalisation */
+            }
+        } else {
+#pragma unroll 1
+            for (int q = 0; q < 4; ++q)
+                small_position<WT, FAMILY>(xs + 4 * tid + q, W, sent, prm, min_valid, jq + q < prm.N,
+                                           star * prm.N + jq + q);
         }
         __syncthreads();
     }
@@ -248,7 +377,7 @@ umi_small_kernel(ReweightParams prm, int min_valid)
 template <bool FAMILY>
 static cudaError_t launch_small_t(const ReweightParams& prm, int min_valid, int wt, unsigned grid, cudaStream_t stream)
 {
-    const size_t smem = (size_t)(KS_THREADS + wt - 1) * sizeof(float);
+    const size_t smem = (size_t)(KS_TILE + wt - 1) * sizeof(float);
     switch (wt) {
     case 9: umi_small_kernel<9, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
     case 17: umi_small_kernel<17, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
