@@ -49,6 +49,59 @@ __device__ __forceinline__ bool load_sample(const double* __restrict__ trow,
     return ok;
 }
 
+/* ---- sm_100a packed fp32x2 arithmetic (FFMA2 / FMUL2 / FADD2): two fp32 in one 64-bit register pair ---- */
+typedef unsigned long long f32x2;                    /* two fp32 in one 64-bit register pair */
+
+__device__ __forceinline__ f32x2 pack2(float lo, float hi)
+{
+    f32x2 r;
+    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+    return r;
+}
+__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi)
+{
+    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
+}
+__device__ __forceinline__ f32x2 ffma2(f32x2 a, f32x2 b, f32x2 c)
+{
+    f32x2 d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+__device__ __forceinline__ f32x2 fmul2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ f32x2 fadd2(f32x2 a, f32x2 b)
+{
+    f32x2 d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+
+
+/* Phase 3 (Eq. 2-4) on two samples of one position at once: S2 += w, R2 += w*u per half.
+   k2 = (k, k), c02 = (c0, c0), nalpha2 = (-alpha, -alpha). */
+__device__ __forceinline__ void eval_weight_pair(f32x2 x2, f32x2 k2, f32x2 c02, f32x2 nalpha2,
+                                                 f32x2& S2, f32x2& R2)
+{
+    const f32x2 a2 = ffma2(x2, k2, c02);                 /* u */
+    const f32x2 b2 = fmul2(a2, nalpha2);                 /* -alpha*u */
+    float a0, a1, b0, b1;
+    unpack2(a2, a0, a1);
+    unpack2(b2, b0, b1);
+    const f32x2 e2 = pack2(fmaxf(a0, b0), fmaxf(a1, b1));   /* |u_eff| */
+    const f32x2 n2 = ffma2(e2, e2, pack2(-1.f, -1.f));
+    float n0, n1;
+    unpack2(n2, n0, n1);
+    const f32x2 t2 = pack2(fmaxf(-n0, 0.f), fmaxf(-n1, 0.f));   /* Eq. 3 clamp (R12) */
+    const f32x2 w2 = fmul2(t2, t2);
+    S2 = fadd2(S2, w2);
+    R2 = ffma2(w2, a2, R2);
+}
+
 } // namespace umi
 
 #endif

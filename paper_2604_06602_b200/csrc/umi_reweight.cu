@@ -71,37 +71,6 @@ __device__ __forceinline__ void eval_welsch(float x, float k, float c0, float na
 }
 
 #if UMI_K2_PACKED
-typedef unsigned long long f32x2;                    /* two fp32 in one 64-bit register pair */
-
-__device__ __forceinline__ f32x2 pack2(float lo, float hi)
-{
-    f32x2 r;
-    asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
-    return r;
-}
-__device__ __forceinline__ void unpack2(f32x2 v, float& lo, float& hi)
-{
-    asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v));
-}
-__device__ __forceinline__ f32x2 ffma2(f32x2 a, f32x2 b, f32x2 c)
-{
-    f32x2 d;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-    return d;
-}
-__device__ __forceinline__ f32x2 fmul2(f32x2 a, f32x2 b)
-{
-    f32x2 d;
-    asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-__device__ __forceinline__ f32x2 fadd2(f32x2 a, f32x2 b)
-{
-    f32x2 d;
-    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
-    return d;
-}
-
 /* Phase 3 on one 128-bit group: 4 samples (two fp32x2 pairs) x 4 positions = 8 pair
    evaluations, written stage by stage so that the 8 dependency chains interleave. */
 __device__ __forceinline__ void eval_weight_group(f32x2 x01, f32x2 x23, const f32x2 (&k2)[K2_NPOS],

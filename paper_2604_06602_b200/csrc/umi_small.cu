@@ -342,16 +342,29 @@ umi_small_kernel(ReweightParams prm, int min_valid)
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
                         const float c0k = -mu[q] * k[q];
-                        float S0 = 0.f, S1 = 0.f, R0 = 0.f, R1 = 0.f;
+                        /* the WT samples of window q as (WT-1)/2 register-aligned pairs + one single:
+                           pairs start at an even index of s[], so q odd peels s[q], q even peels s[q+WT-1] */
+                        constexpr int NPAIR = (WT - 1) / 2;
+                        const int first = q + (q & 1);
+                        const f32x2 k2 = pack2(k[q], k[q]), c02 = pack2(c0k, c0k), na2 = pack2(nalpha, nalpha);
+                        f32x2 Sa = pack2(0.f, 0.f), Sb = Sa, Ra = Sa, Rb = Sa;
 #pragma unroll
-                        for (int i = 0; i < WT; ++i) {
-                            const float u = fmaf(s[q + i], k[q], c0k);
-                            const float b = u * nalpha;
-                            const float e = fmaxf(u, b);
+                        for (int j = 0; j < NPAIR; ++j) {
+                            const f32x2 x2 = pack2(s[first + 2 * j], s[first + 2 * j + 1]);
+                            if (j & 1) eval_weight_pair(x2, k2, c02, na2, Sb, Rb);
+                            else       eval_weight_pair(x2, k2, c02, na2, Sa, Ra);
+                        }
+                        float S0, S1, R0, R1;
+                        unpack2(fadd2(Sa, Sb), S0, S1);
+                        unpack2(fadd2(Ra, Rb), R0, R1);
+                        {
+                            const float xs1 = (q & 1) ? s[q] : s[q + WT - 1];
+                            const float u = fmaf(xs1, k[q], c0k);
+                            const float e = fmaxf(u, u * nalpha);
                             const float t = __saturatef(fmaf(-e, e, 1.f));
                             const float w = t * t;
-                            if (i & 1) { S1 += w; R1 = fmaf(w, u, R1); }
-                            else       { S0 += w; R0 = fmaf(w, u, R0); }
+                            S0 += w;
+                            R0 = fmaf(w, u, R0);
                         }
                         const float S = S0 + S1, R = R0 + R1;
                         if (on[q] && S > 0.f) mu[q] = fmaf(R / S, cs[q], mu[q]);   /* Eq. 4; (R11) */
