@@ -95,6 +95,7 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.n_iter = n_iter;
         rp.alpha = alpha;
         rp.c = c;
+        rp.split = 1;
         rp.scale_in = nullptr;
         rp.scale_out = fam.scale_out;
         rp.weight_kind = fam.weight_kind;
@@ -138,6 +139,15 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.N = n_cadences;
         rp.tiles_per_star = (n_cadences + umi::K2_TILE - 1) / umi::K2_TILE;
         rp.n_blocks = n_stars * rp.tiles_per_star;
+        rp.split = 1;
+        if (!fam.on && rp.n_blocks <= 4 * 148) {
+            /* the grid would leave most of the 148 x 8 CTA slots empty: split every window over
+               K2_SPLIT lanes instead (latency, not throughput, is what is left to win) */
+            rp.split = umi::K2_SPLIT;
+            const int tile = umi::K2_TILE / umi::K2_SPLIT;
+            rp.tiles_per_star = (n_cadences + tile - 1) / tile;
+            rp.n_blocks = n_stars * rp.tiles_per_star;
+        }
         rp.W = W;
         rp.n_iter = n_iter;
         rp.alpha = alpha;
@@ -147,7 +157,8 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.weight_kind = fam.weight_kind;
         rp.scale_kind = fam.scale_kind;
         const unsigned grid2 = (unsigned)std::min<int64_t>(rp.n_blocks, MAX_GRID);
-        if (cuda_failed(umi::launch_reweight(rp, fam.on, grid2, g.smem2, stream))) return UMI_ERR_CUDA;
+        const size_t smem2 = g.smem2 - (size_t)(umi::K2_TILE - umi::K2_TILE / rp.split) * sizeof(float);
+        if (cuda_failed(umi::launch_reweight(rp, fam.on, grid2, smem2, stream))) return UMI_ERR_CUDA;
     }
     if (ev && cuda_failed(cudaEventRecord(ev[2], stream))) return UMI_ERR_CUDA;
     return UMI_OK;

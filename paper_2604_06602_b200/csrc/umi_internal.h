@@ -33,6 +33,7 @@ constexpr int KS_MAX_WINDOW = 49;                /* windows up to this length ta
 constexpr int K2_THREADS = 128;                  /* reweighting kernel */
 constexpr int K2_NPOS = 4;                       /* consecutive positions per thread */
 constexpr int K2_TILE = K2_THREADS * K2_NPOS;    /* positions per CTA */
+constexpr int K2_SPLIT = 8;                      /* small batches: lanes per 4 positions (tile = K2_TILE / K2_SPLIT) */
 
 struct MedianParams {
     const double* time;      /* may be null */
@@ -53,6 +54,7 @@ struct ReweightParams {
     float* flat;             /* null, or flux / trend (PAPER.md:155 normalisation), NaN where trend is NaN */
     const float* scale_in;   /* family kernels: null, or s per position (replaces Phase 2) */
     float* scale_out;        /* family kernels: null, or receives s per position */
+    int split;               /* reweighting kernel: 1, or K2_SPLIT for batches too small to fill the GPU */
     int weight_kind;         /* family kernels: WEIGHT_BISQUARE / WEIGHT_WELSCH */
     int scale_kind;          /* fused short-window kernel only */
     int64_t N;

@@ -117,30 +117,39 @@ __device__ __forceinline__ void eval_weight_group(f32x2 x01, f32x2 x23, const f3
 
 /* MODE 0: the paper's path.  MODE 1: sibling estimators with bisquare weights (scale from a buffer
    and / or written out).  MODE 2: the same with Welsch weights. */
-template <int MODE>
+/* SPLIT > 1 (small batches, where the grid would not fill the GPU): SPLIT adjacent lanes share the 4
+   positions, each taking every SPLIT-th 128-bit group of the windows; the partial sums are combined
+   with xor shuffles after every pass.  A CTA then owns K2_TILE / SPLIT positions and a thread's serial
+   chain is SPLIT times shorter.  SPLIT = 1 is the throughput configuration. */
+template <int MODE, int SPLIT>
 __global__ void __launch_bounds__(K2_THREADS, UMI_K2_MIN_CTAS)
 umi_reweight_kernel(ReweightParams prm)
 {
+    constexpr int TILE = K2_TILE / SPLIT;
     extern __shared__ __align__(16) unsigned char smem_raw[];
     float* xs = reinterpret_cast<float*>(smem_raw);
     __shared__ float s_red[2 * (K2_THREADS / 32)];
 
     const int tid = threadIdx.x;
+    const int pt = tid / SPLIT;                         /* which 4 positions of the tile */
+    const int sl = tid % SPLIT;                         /* which slice of their windows */
     const int W = prm.W;
     const int h = (W - 1) >> 1;
     const int hal = (h + 3) & ~3;
     const int delta = hal - h;
     const int G = (3 + delta + 2 * h) / 4 + 1;          /* float4 groups per thread */
-    const int nx = K2_TILE + 4 * G;                     /* staged floats */
+    const int nx = TILE + 4 * G;                        /* staged floats */
     const int g_lo = (3 + delta + 3) >> 2;              /* first group fully inside all 4 windows */
     const int g_hi = (delta + 2 * h - 3) >= 0 ? ((delta + 2 * h - 3) >> 2) : -1;   /* last such group */
+    /* first interior group of this lane's slice: the smallest g >= g_lo with g = sl (mod SPLIT) */
+    const int g_first = (SPLIT == 1) ? g_lo : g_lo + ((sl - g_lo % SPLIT) + SPLIT) % SPLIT;
     const float nalpha = -prm.alpha;
     const float qnan = __int_as_float(0x7FC00000);
 
     for (int64_t bid = blockIdx.x; bid < prm.n_blocks; bid += gridDim.x) {
         const int64_t star = bid / prm.tiles_per_star;
         const int64_t tile = bid - star * prm.tiles_per_star;
-        const int64_t j0 = tile * K2_TILE;
+        const int64_t j0 = tile * TILE;
         const int64_t jbase = j0 - hal;                 /* cadence of staged index 0 */
         const float* frow = prm.flux + star * prm.N;
         const double* trow = prm.time ? prm.time + star * prm.N : nullptr;
@@ -188,7 +197,7 @@ umi_reweight_kernel(ReweightParams prm)
         bool any_act = false;
 #pragma unroll
         for (int q = 0; q < K2_NPOS; ++q) {
-            const int64_t j = j0 + 4 * tid + q;
+            const int64_t j = j0 + 4 * pt + q;
             med[q] = (j < prm.N) ? orow[j] : qnan;
             act[q] = (med[q] == med[q]);
             any_act = any_act || act[q];
@@ -200,7 +209,7 @@ umi_reweight_kernel(ReweightParams prm)
                     prm.scale_out[star * prm.N + j] = qnan;
             }
         }
-        const float4* xs4 = reinterpret_cast<const float4*>(xs) + tid;
+        const float4* xs4 = reinterpret_cast<const float4*>(xs) + pt;
 
         if (__any_sync(0xFFFFFFFFu, any_act)) {
             /* ---- Phase 2 (Eq. 1) ---- */
@@ -208,7 +217,7 @@ umi_reweight_kernel(ReweightParams prm)
 #pragma unroll
             for (int q = 0; q < K2_NPOS; ++q) { ss[q] = 0.f; cnt[q] = 0.f; }
             const bool given = (MODE != 0) && prm.scale_in != nullptr;
-            for (int g = 0; g < (given ? 0 : G); ++g) {
+            for (int g = sl; g < (given ? 0 : G); g += SPLIT) {
                 const float4 v = xs4[g];
                 const float xv[4] = {v.x, v.y, v.z, v.w};
                 if (g >= g_lo && g <= g_hi) {
@@ -226,6 +235,15 @@ umi_reweight_kernel(ReweightParams prm)
                         }
                 }
             }
+            if constexpr (SPLIT > 1) {
+#pragma unroll
+                for (int q = 0; q < K2_NPOS; ++q)
+#pragma unroll
+                    for (int o = SPLIT / 2; o > 0; o >>= 1) {
+                        ss[q] += __shfl_xor_sync(0xFFFFFFFFu, ss[q], o);
+                        cnt[q] += __shfl_xor_sync(0xFFFFFFFFu, cnt[q], o);
+                    }
+            }
 #pragma unroll
             for (int q = 0; q < K2_NPOS; ++q) {
                 bool on = act[q] && cnt[q] > 0.f;                   /* (R8) */
@@ -235,11 +253,11 @@ umi_reweight_kernel(ReweightParams prm)
                     on = s > 0.f;
                 }
                 if constexpr (MODE != 0) {
-                    const int64_t j = j0 + 4 * tid + q;
+                    const int64_t j = j0 + 4 * pt + q;
                     if (given) {                                    /* the MAD from the selection kernel */
                         s = (act[q] && j < prm.N) ? prm.scale_in[star * prm.N + j] : 0.f;
                         on = act[q] && s > 0.f;
-                    } else if (prm.scale_out != nullptr && j < prm.N && act[q]) {
+                    } else if (prm.scale_out != nullptr && j < prm.N && act[q] && sl == 0) {
                         prm.scale_out[star * prm.N + j] = s;
                     }
                 }
@@ -265,8 +283,11 @@ umi_reweight_kernel(ReweightParams prm)
                 }
 #endif
                 /* edge groups: samples that belong to some but not all of the 4 windows */
-                for (int g = 0; g < G; ++g) {
-                    if (g >= g_lo && g <= g_hi) { g = g_hi; continue; }
+                for (int g = sl; g < G; g += SPLIT) {
+                    if (g >= g_lo && g <= g_hi) {
+                        if constexpr (SPLIT == 1) g = g_hi;
+                        continue;
+                    }
                     const float4 v = xs4[g];
                     const float xv[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
@@ -283,7 +304,7 @@ umi_reweight_kernel(ReweightParams prm)
                 /* interior groups: every sample belongs to all 4 windows */
                 if constexpr (MODE == 2) {
 #pragma unroll 2
-                    for (int g = g_lo; g <= g_hi; ++g) {
+                    for (int g = g_first; g <= g_hi; g += SPLIT) {
                         const float4 v = xs4[g];
                         const float xv[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
@@ -294,13 +315,13 @@ umi_reweight_kernel(ReweightParams prm)
                 } else {
 #if UMI_K2_PACKED
 #pragma unroll K2_UNROLL
-                for (int g = g_lo; g <= g_hi; ++g) {
+                for (int g = g_first; g <= g_hi; g += SPLIT) {
                     const ulonglong2 v2 = reinterpret_cast<const ulonglong2*>(xs4)[g];
                     eval_weight_group(v2.x, v2.y, k2, c02, nalpha2, S2, R2);
                 }
 #else
 #pragma unroll 2
-                for (int g = g_lo; g <= g_hi; ++g) {
+                for (int g = g_first; g <= g_hi; g += SPLIT) {
                     const float4 v = xs4[g];
                     const float xv[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
@@ -321,6 +342,13 @@ umi_reweight_kernel(ReweightParams prm)
                         R[q] += r0 + r1;
                     }
 #endif
+                    if constexpr (SPLIT > 1) {
+#pragma unroll
+                        for (int o = SPLIT / 2; o > 0; o >>= 1) {
+                            S[q] += __shfl_xor_sync(0xFFFFFFFFu, S[q], o);
+                            R[q] += __shfl_xor_sync(0xFFFFFFFFu, R[q], o);
+                        }
+                    }
                     if (act[q] && S[q] > 0.f) mu[q] = fmaf(R[q] / S[q], cs[q], mu[q]);   /* Eq. 4; (R11) */
                 }
             }
@@ -328,16 +356,16 @@ umi_reweight_kernel(ReweightParams prm)
 
 #pragma unroll
         for (int q = 0; q < K2_NPOS; ++q) {
-            const int64_t j = j0 + 4 * tid + q;
-            if (j < prm.N && med[q] == med[q]) orow[j] = mu[q];
+            const int64_t j = j0 + 4 * pt + q;
+            if (j < prm.N && med[q] == med[q] && sl == 0) orow[j] = mu[q];
         }
         if (prm.flat != nullptr) {                                  /* PAPER.md:155 normalisation */
             float* flrow = prm.flat + star * prm.N;
 #pragma unroll
             for (int q = 0; q < K2_NPOS; ++q) {
-                const int64_t j = j0 + 4 * tid + q;
+                const int64_t j = j0 + 4 * pt + q;
                 /* own sample = staged index hal + 4*tid + q (valid whenever the median is not NaN) */
-                if (j < prm.N) flrow[j] = (med[q] == med[q]) ? xs[hal + 4 * tid + q] / mu[q] : qnan;
+                if (j < prm.N && sl == 0) flrow[j] = (med[q] == med[q]) ? xs[hal + 4 * pt + q] / mu[q] : qnan;
             }
         }
         __syncthreads();
@@ -346,9 +374,10 @@ umi_reweight_kernel(ReweightParams prm)
 
 cudaError_t launch_reweight(const ReweightParams& prm, bool family, unsigned grid, size_t smem, cudaStream_t stream)
 {
-    if (!family) umi_reweight_kernel<0><<<grid, K2_THREADS, smem, stream>>>(prm);
-    else if (prm.weight_kind == WEIGHT_WELSCH) umi_reweight_kernel<2><<<grid, K2_THREADS, smem, stream>>>(prm);
-    else umi_reweight_kernel<1><<<grid, K2_THREADS, smem, stream>>>(prm);
+    if (!family && prm.split == K2_SPLIT) umi_reweight_kernel<0, K2_SPLIT><<<grid, K2_THREADS, smem, stream>>>(prm);
+    else if (!family) umi_reweight_kernel<0, 1><<<grid, K2_THREADS, smem, stream>>>(prm);
+    else if (prm.weight_kind == WEIGHT_WELSCH) umi_reweight_kernel<2, 1><<<grid, K2_THREADS, smem, stream>>>(prm);
+    else umi_reweight_kernel<1, 1><<<grid, K2_THREADS, smem, stream>>>(prm);
     return cudaGetLastError();
 }
 

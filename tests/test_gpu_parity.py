@@ -133,3 +133,11 @@ def test_extreme_magnitudes(umi):
     base = lc.random_series(31, 1, 1500, nan_frac=0.01, inf_frac=0.0)
     for scale, offset in ((1.0, 0.0), (1e4, 0.0), (1e-3, 0.0), (1.0, 100.0)):
         _both(umi, (base * scale + offset).astype(np.float32), 51)
+
+
+@pytest.mark.parametrize("W", [51, 361])
+def test_large_batch_takes_the_throughput_kernel(umi, W):
+    # batches of at most 4 x 148 reweighting tiles run the split-window (latency) variant of the
+    # reweighting kernel; 160 stars x 2100 cadences = 800 tiles run the throughput variant
+    x = lc.random_series(900 + W, 160, 2100)
+    _both(umi, x, W)
