@@ -15,10 +15,10 @@
  * falls outside [0, n_grid), or the NEXT sample of its row lands in the same slot (rows are
  * assumed non-decreasing in time; anything else is memory-safe but unspecified).
  *
- * Both kernels are pure data movement, one thread per sample, coalesced reads; the writes
- * of the scatter and the reads of the gather are monotone in the slot, i.e. coalesced
- * except across gaps.  Bytes per sample: scatter 8 (time) + 4 (flux) + 8 (next time, L1/L2
- * hit) read, 4 written; gather 8 + 4 + 4 read, 4 (+4) written.  HBM-bound.
+ * Both kernels are pure data movement, four samples per thread with every load issued before its
+ * first use, coalesced reads; the writes of the scatter and the reads of the gather are monotone
+ * in the slot, i.e. coalesced except across gaps.  Bytes per sample: scatter 8 (time) + 4 (flux)
+ * read, 4 written; gather 8 + 4 + 4 read, 4 (+4) written.  HBM-bound.
  * Nothing here is shared with oracle/.
  */
 #include "umi_device.cuh"
@@ -36,16 +36,13 @@ __device__ __forceinline__ double raw_slot(double t, double t0, double dt)
 }
 
 /*
- * Slot of sample i of one row with the collision rule applied (flux not looked at).  One fp64
- * division per sample: the successor's slot comes from the next lane by shuffle; only lane 31
- * (and the last sample of a row) computes it itself.  All 32 lanes must call this together;
- * lanes with i >= M pass a NaN time and get -1.
+ * Slot of a sample with the collision rule applied (flux not looked at), given its own time t (NaN
+ * when the lane is outside the row).  One fp64 division per sample: the successor's slot comes from
+ * the next lane by shuffle; only lane 31 computes it itself.  All 32 lanes must call this together.
  */
-__device__ __forceinline__ int64_t sample_slot(const double* __restrict__ trow, int64_t i, int64_t M,
+__device__ __forceinline__ int64_t sample_slot(double t, const double* __restrict__ trow, int64_t i, int64_t M,
                                                double t0, double dt, int64_t n_grid)
 {
-    const bool in_row = i < M;
-    const double t = in_row ? __ldg(trow + i) : __longlong_as_double(0x7FF8000000000000ll);
     const bool fin = finite_f64(t);
     const double k = fin ? raw_slot(t, t0, dt) : -1.0;
     double kn = __shfl_down_sync(0xFFFFFFFFu, k, 1);
@@ -63,20 +60,33 @@ __device__ __forceinline__ int64_t sample_slot(const double* __restrict__ trow, 
     return (int64_t)k;
 }
 
+constexpr int RG_ITEMS = 4;                             /* samples per thread: all loads issued before any use */
+
 /* grid = (chunks of a row, stars): no 64-bit division per sample */
 __global__ void __launch_bounds__(RG_THREADS)
 umi_regrid_scatter_kernel(RegridParams prm, float* __restrict__ grid_flux)
 {
+    const double dnan = __longlong_as_double(0x7FF8000000000000ll);
     for (int64_t b = blockIdx.y; b < prm.n_stars; b += gridDim.y) {
         const double* trow = prm.time + b * prm.M;
         const float* frow = prm.flux + b * prm.M;
         float* grow = grid_flux + b * prm.n_grid;
-        const int64_t Mr = (prm.M + 31) & ~(int64_t)31;             /* whole warps stay together */
-        for (int64_t i = (int64_t)blockIdx.x * RG_THREADS + threadIdx.x; i < Mr; i += (int64_t)gridDim.x * RG_THREADS) {
-            const int64_t k = sample_slot(trow, i, prm.M, prm.t0, prm.dt, prm.n_grid);
-            if (k < 0) continue;
-            const float x = __ldg(frow + i);
-            if (finite_f32(x)) grow[k] = x;
+        for (int64_t base = (int64_t)blockIdx.x * (RG_THREADS * RG_ITEMS); base < prm.M;
+             base += (int64_t)gridDim.x * (RG_THREADS * RG_ITEMS)) {
+            double t[RG_ITEMS];
+            float x[RG_ITEMS];
+#pragma unroll
+            for (int r = 0; r < RG_ITEMS; ++r) {
+                const int64_t i = base + r * RG_THREADS + threadIdx.x;
+                t[r] = i < prm.M ? __ldg(trow + i) : dnan;
+                x[r] = i < prm.M ? __ldg(frow + i) : 0.f;
+            }
+#pragma unroll
+            for (int r = 0; r < RG_ITEMS; ++r) {
+                const int64_t i = base + r * RG_THREADS + threadIdx.x;
+                const int64_t k = sample_slot(t[r], trow, i, prm.M, prm.t0, prm.dt, prm.n_grid);
+                if (k >= 0 && finite_f32(x[r])) grow[k] = x[r];
+            }
         }
     }
 }
@@ -86,26 +96,41 @@ umi_regrid_gather_kernel(RegridParams prm, const float* __restrict__ grid_trend,
                          float* __restrict__ trend_out, float* __restrict__ flat_out)
 {
     const float qnan = __int_as_float(0x7FC00000);
+    const double dnan = __longlong_as_double(0x7FF8000000000000ll);
     for (int64_t b = blockIdx.y; b < prm.n_stars; b += gridDim.y) {
         const double* trow = prm.time + b * prm.M;
         const float* frow = prm.flux + b * prm.M;
         const float* grow = grid_trend + b * prm.n_grid;
-        const int64_t Mr = (prm.M + 31) & ~(int64_t)31;
-        for (int64_t i = (int64_t)blockIdx.x * RG_THREADS + threadIdx.x; i < Mr; i += (int64_t)gridDim.x * RG_THREADS) {
-            const int64_t k = sample_slot(trow, i, prm.M, prm.t0, prm.dt, prm.n_grid);
-            if (i >= prm.M) continue;
-            const float x = __ldg(frow + i);
-            float tr = qnan;
-            if (k >= 0 && finite_f32(x)) tr = __ldg(grow + k);
-            trend_out[b * prm.M + i] = tr;
-            if (flat_out != nullptr) flat_out[b * prm.M + i] = (tr == tr) ? x / tr : qnan;
+        for (int64_t base = (int64_t)blockIdx.x * (RG_THREADS * RG_ITEMS); base < prm.M;
+             base += (int64_t)gridDim.x * (RG_THREADS * RG_ITEMS)) {
+            double t[RG_ITEMS];
+            float x[RG_ITEMS], tr[RG_ITEMS];
+#pragma unroll
+            for (int r = 0; r < RG_ITEMS; ++r) {
+                const int64_t i = base + r * RG_THREADS + threadIdx.x;
+                t[r] = i < prm.M ? __ldg(trow + i) : dnan;
+                x[r] = i < prm.M ? __ldg(frow + i) : 0.f;
+            }
+#pragma unroll
+            for (int r = 0; r < RG_ITEMS; ++r) {
+                const int64_t i = base + r * RG_THREADS + threadIdx.x;
+                const int64_t k = sample_slot(t[r], trow, i, prm.M, prm.t0, prm.dt, prm.n_grid);
+                tr[r] = (k >= 0 && finite_f32(x[r])) ? __ldg(grow + k) : qnan;
+            }
+#pragma unroll
+            for (int r = 0; r < RG_ITEMS; ++r) {
+                const int64_t i = base + r * RG_THREADS + threadIdx.x;
+                if (i >= prm.M) continue;
+                trend_out[b * prm.M + i] = tr[r];
+                if (flat_out != nullptr) flat_out[b * prm.M + i] = (tr[r] == tr[r]) ? x[r] / tr[r] : qnan;
+            }
         }
     }
 }
 
 dim3 regrid_grid(int64_t n_stars, int64_t M)
 {
-    int64_t bx = (M + RG_THREADS - 1) / RG_THREADS;
+    int64_t bx = (M + RG_THREADS * RG_ITEMS - 1) / (RG_THREADS * RG_ITEMS);
     if (bx < 1) bx = 1;
     if (bx > 1024) bx = 1024;
     int64_t by = n_stars < 1 ? 1 : n_stars;
