@@ -155,7 +155,8 @@ def ncu_traffic(config_id, n_stars):
     if config_id != 2 or n_stars != 1000 or not os.path.exists(path):
         return None
     with open(path) as f:
-        k = json.load(f)["kernels"].get("umi_reweight_kernel")
+        kernels = json.load(f)["kernels"]
+    k = next((v for n, v in kernels.items() if n.startswith("umi_reweight_kernel<0, 1>") and "config2" in n), None)
     return None if k is None else k["dram_bytes_read"] + k["dram_bytes_write"]
 
 

@@ -30,7 +30,10 @@ constexpr int KS_THREADS = 128;                  /* fused small-window kernel: 4
 constexpr int KS_TILE = 4 * KS_THREADS;          /* positions per CTA */
 constexpr int KS_MAX_WINDOW = 49;                /* windows up to this length take the fused kernel */
 
-constexpr int K2_THREADS = 128;                  /* reweighting kernel */
+#ifndef UMI_K2_THREADS
+#define UMI_K2_THREADS 128
+#endif
+constexpr int K2_THREADS = UMI_K2_THREADS;       /* reweighting kernel */
 constexpr int K2_NPOS = 4;                       /* consecutive positions per thread */
 constexpr int K2_TILE = K2_THREADS * K2_NPOS;    /* positions per CTA */
 constexpr int K2_SPLIT = 8;                      /* small batches: lanes per 4 positions (tile = K2_TILE / K2_SPLIT) */

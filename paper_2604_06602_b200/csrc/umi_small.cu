@@ -275,7 +275,7 @@ umi_small_kernel(ReweightParams prm, int min_valid)
 
         const int64_t jq = j0 + 4 * tid;                            /* first of the thread's 4 positions */
         bool fast = false;
-        if constexpr (!FAMILY) {
+        {
             if (W == WT) {
                 /* all WT + 3 samples valid <=> all 4 windows complete (and inside the row) */
                 bool ok = true;
@@ -313,27 +313,38 @@ umi_small_kernel(ReweightParams prm, int min_valid)
                 med[q] = m;
                 mu[q] = m;
             }
-            if (prm.n_iter > 0) {
-                /* ---- Phase 2 (Eq. 1) ---- */
+            const bool want_scale = FAMILY && prm.scale_out != nullptr;
+            if (prm.n_iter > 0 || want_scale) {
+                /* ---- Phase 2 (Eq. 1), or the MAD (R21) for the sibling estimators ---- */
                 float cs[4], k[4];
                 bool on[4];
 #pragma unroll
                 for (int q = 0; q < 4; ++q) {
-                    float ss = 0.f, cnt = 0.f;
+                    float sc = 0.f;
+                    if (FAMILY && prm.scale_kind == SCALE_MAD) {
+                        float a[WT];
 #pragma unroll
-                    for (int i = 0; i < WT; ++i) {
-                        const float d = s[q + i] - med[q];
-                        if (d > 0.f) {                              /* one compare, two predicated updates */
-                            ss = fmaf(d, d, ss);
-                            cnt += 1.f;
+                        for (int i = 0; i < WT; ++i) a[i] = fabsf(s[q + i] - med[q]);
+                        batcher_sort<WT>(a);
+                        sc = a[M];
+                        on[q] = sc > 0.f;
+                    } else {
+                        float ss = 0.f, cnt = 0.f;
+#pragma unroll
+                        for (int i = 0; i < WT; ++i) {
+                            const float d = s[q + i] - med[q];
+                            if (d > 0.f) {                          /* one compare, two predicated updates */
+                                ss = fmaf(d, d, ss);
+                                cnt += 1.f;
+                            }
+                        }
+                        on[q] = cnt > 0.f;                          /* (R8) */
+                        if (on[q]) {
+                            sc = SCALE_CONST * sqrtf(ss / cnt);
+                            on[q] = sc > 0.f;
                         }
                     }
-                    on[q] = cnt > 0.f;                              /* (R8) */
-                    float sc = 0.f;
-                    if (on[q]) {
-                        sc = SCALE_CONST * sqrtf(ss / cnt);
-                        on[q] = sc > 0.f;
-                    }
+                    if (want_scale) prm.scale_out[star * prm.N + jq + q] = sc;
                     cs[q] = on[q] ? prm.c * sc : 0.f;
                     k[q] = on[q] ? 1.f / cs[q] : 0.f;
                 }
@@ -342,6 +353,19 @@ umi_small_kernel(ReweightParams prm, int min_valid)
 #pragma unroll
                     for (int q = 0; q < 4; ++q) {
                         const float c0k = -mu[q] * k[q];
+                        if (FAMILY && prm.weight_kind == WEIGHT_WELSCH) {
+                            float S = 0.f, R = 0.f;
+#pragma unroll
+                            for (int i = 0; i < WT; ++i) {
+                                const float u = fmaf(s[q + i], k[q], c0k);
+                                const float e = fmaxf(u, u * nalpha);
+                                const float w = exp2f(e * e * -1.4426950408889634f);   /* (R22) exp(-u_eff^2) */
+                                S += w;
+                                R = fmaf(w, u, R);
+                            }
+                            if (on[q] && S > 0.f) mu[q] = fmaf(R / S, cs[q], mu[q]);
+                            continue;
+                        }
                         /* the WT samples of window q as (WT-1)/2 register-aligned pairs + one single:
                            pairs start at an even index of s[], so q odd peels s[q], q even peels s[q+WT-1] */
                         constexpr int NPAIR = (WT - 1) / 2;
