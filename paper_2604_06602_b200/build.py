@@ -10,7 +10,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 SOURCES = [os.path.join(CSRC, "umi_api.cu"), os.path.join(CSRC, "umi_median.cu"), os.path.join(CSRC, "umi_reweight.cu"),
-           os.path.join(CSRC, "umi_small.cu"), os.path.join(CSRC, "umi_regrid.cu")]
+           os.path.join(CSRC, "umi_small.cu"), os.path.join(CSRC, "umi_regrid.cu"),
+           os.path.join(CSRC, "umi_reweight_tc.cu")]
 HEADERS = [os.path.join(CSRC, "umi_internal.h"), os.path.join(CSRC, "umi_device.cuh"), os.path.join(ROOT, "include", "umi.h")]
 LIB = os.path.join(HERE, "libumi_b200.so")
 

@@ -5,6 +5,7 @@
 #include <cuda_runtime.h>
 #include <math.h>
 #include <stdint.h>
+#include <stdlib.h>
 
 #include <algorithm>
 #include <vector>
@@ -15,6 +16,7 @@
 namespace {
 
 constexpr int64_t MAX_GRID = 0x7FFFFFFF;
+constexpr int TC_MAX_WINDOW = 1101;      /* tensor-core reweighting: B tile + samples <= ~45 KB of shared memory per CTA */
 
 /* sibling-estimator selection (F4); the default is the paper's path */
 struct Family {
@@ -44,6 +46,12 @@ Geometry geometry_for(int W)
     const int G = (3 + (hal - h) + 2 * h) / 4 + 1;
     g.smem2 = (size_t)(umi::K2_TILE + 4 * G) * sizeof(float);
     return g;
+}
+
+bool tc_requested()
+{
+    const char* e = getenv("UMI_B200_TC");
+    return e != nullptr && e[0] == '1';
 }
 
 int check_window(int W)
@@ -156,6 +164,21 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.scale_out = mad ? nullptr : fam.scale_out;
         rp.weight_kind = fam.weight_kind;
         rp.scale_kind = fam.scale_kind;
+        /* Experimental, off by default: weights on the CUDA cores, the two sums of Eq. 4 on the tensor cores
+           (umi_reweight_tc.cu: tcgen05.mma with the weights in TMEM).  Correct (same parity tests) but measured
+           slower than the all-CUDA-core kernel on config 2 (13.8 ms vs 8.78 ms), so it only
+           runs when UMI_B200_TC=1 is set in the environment. */
+        if (!fam.on && rp.split == 1 && n_iter > 0 && W <= TC_MAX_WINDOW && tc_requested()) {
+            rp.tiles_per_star = (n_cadences + umi::tc_tile() - 1) / umi::tc_tile();
+            rp.n_blocks = n_stars * rp.tiles_per_star;
+            if (rp.n_blocks <= MAX_GRID) {
+                if (cuda_failed(umi::launch_reweight_tc(rp, (unsigned)rp.n_blocks, stream))) return UMI_ERR_CUDA;
+                if (ev && cuda_failed(cudaEventRecord(ev[2], stream))) return UMI_ERR_CUDA;
+                return UMI_OK;
+            }
+            rp.tiles_per_star = (n_cadences + umi::K2_TILE - 1) / umi::K2_TILE;
+            rp.n_blocks = n_stars * rp.tiles_per_star;
+        }
         const unsigned grid2 = (unsigned)std::min<int64_t>(rp.n_blocks, MAX_GRID);
         const size_t smem2 = g.smem2 - (size_t)(umi::K2_TILE - umi::K2_TILE / rp.split) * sizeof(float);
         if (cuda_failed(umi::launch_reweight(rp, fam.on, grid2, smem2, stream))) return UMI_ERR_CUDA;

@@ -71,6 +71,11 @@ struct ReweightParams {
 cudaError_t launch_median(const MedianParams& prm, unsigned grid, size_t smem, cudaStream_t stream);
 /* family = false: the paper's path (scale_in/scale_out/weight_kind ignored); true: the sibling-estimator variants */
 cudaError_t launch_reweight(const ReweightParams& prm, bool family, unsigned grid, size_t smem, cudaStream_t stream);
+/* umi_reweight_tc.cu: Phases 2-3 with the two sums of Eq. 4 on the tensor cores (tcgen05 / TMEM) */
+int tc_chunks(int W);
+size_t tc_smem_bytes(int W);
+int tc_tile();
+cudaError_t launch_reweight_tc(const ReweightParams& prm, unsigned grid, cudaStream_t stream);
 /* fused kernel for W <= KS_MAX_WINDOW; wt = compiled wire count (9, 17, 25, 33 or 49) >= W */
 cudaError_t launch_small(const ReweightParams& prm, bool family, int min_valid, int wt, unsigned grid, cudaStream_t stream);
 

@@ -141,3 +141,14 @@ def test_large_batch_takes_the_throughput_kernel(umi, W):
     # reweighting kernel; 160 stars x 2100 cadences = 800 tiles run the throughput variant
     x = lc.random_series(900 + W, 160, 2100)
     _both(umi, x, W)
+
+
+@pytest.mark.parametrize("W", [51, 361, 1081])
+def test_tensor_core_variant_of_the_reweighting_kernel(umi, W, monkeypatch):
+    # experimental path (UMI_B200_TC=1): weights on the CUDA cores, the sums of Eq. 4 by tcgen05.mma
+    # with tf32 operands and fp32 accumulation in TMEM -- same bars as the default kernel
+    monkeypatch.setenv("UMI_B200_TC", "1")
+    x = lc.random_series(950 + W, 160, 2100)
+    _both(umi, x, W)
+    y = (lc.random_series(951 + W, 160, 2100, nan_frac=0.01, inf_frac=0.0) * 1e3 + 50.0).astype(np.float32)
+    _both(umi, y, W)
