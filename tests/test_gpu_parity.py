@@ -152,3 +152,26 @@ def test_tensor_core_variant_of_the_reweighting_kernel(umi, W, monkeypatch):
     _both(umi, x, W)
     y = (lc.random_series(951 + W, 160, 2100, nan_frac=0.01, inf_frac=0.0) * 1e3 + 50.0).astype(np.float32)
     _both(umi, y, W)
+
+
+@pytest.mark.parametrize("case", range(24))
+def test_fuzz_random_shapes_and_parameters(umi, case):
+    # seeded fuzz over window length, series length, batch size and estimator parameters: every
+    # kernel variant (fused short-window, split-window, throughput) sees shapes nobody hand-picked
+    rng = np.random.default_rng(7000 + case)
+    W = int(rng.choice([3, 7, 13, 21, 29, 41, 47, 49, 51, 53, 77, 101, 215, 217, 301, 363, 511, 801, 1279, 2047])) | 1
+    S = int(rng.choice([1, 2, 5, 40, 200]))
+    N = int(rng.integers(1, 2400)) if S > 5 else int(rng.integers(1, 6000))
+    alpha = float(rng.choice([0.5, 1.0, 2.0, 3.0, 10.0]))
+    c = float(rng.choice([2.5, 5.0, 8.0]))
+    n_iter = int(rng.choice([1, 3, 5, 9]))
+    min_valid = int(rng.choice([-1, 1, max(1, W // 2)]))
+    # ties only with the paper's default tuning: flux quantised to ~5 levels under alpha = 10, c = 2.5
+    # and 9 passes is an expanding iteration (one fp32 ulp of mu moves the result by 200 ulps, measured:
+    # DESIGN.md 5.2, "fp32 tolerance"), which no fp32-in / fp32-out path can follow to 1e-5
+    ties = bool(rng.integers(0, 2)) and alpha <= 3.0 and c >= 5.0
+    x = lc.random_series(8000 + case, S, N, nan_frac=float(rng.choice([0.0, 0.02, 0.2])),
+                         inf_frac=float(rng.choice([0.0, 0.01])), ties=ties)
+    x = (x * float(rng.choice([1.0, 1e-2, 1e3])) + float(rng.choice([0.0, 0.0, 3.0]))).astype(np.float32)
+    kw = {} if min_valid < 0 else {"min_valid": min_valid}
+    _both(umi, x, W, alpha=alpha, n_iter=n_iter, c=c, **kw)
