@@ -186,3 +186,34 @@ def test_family_constant_and_degenerate(umi):
     trend, scale = umi.umi_detrend_family(None, _cuda(x, np.float32), 51, 1, 0)
     torch.cuda.synchronize()
     assert np.isnan(trend.cpu().numpy()).all() and np.isnan(scale.cpu().numpy()).all()
+
+
+@pytest.mark.parametrize("case", range(16))
+def test_fuzz_family_and_gapped(umi, case):
+    # seeded fuzz over the next rows: random window, shape, kinds, parameters; odd cases through the
+    # time-stamped path (compacted rows, jittered times, grid shorter than the data)
+    import torch
+    rng = np.random.default_rng(9100 + case)
+    W = int(rng.choice([5, 9, 25, 33, 49, 51, 101, 217, 361, 801])) | 1
+    S = int(rng.choice([1, 3, 40, 180]))
+    N = int(rng.integers(2, 2200))
+    alpha = float(rng.choice([1.0, 2.0, 3.0]))
+    n_iter = int(rng.choice([0, 1, 5]))
+    x = lc.random_series(9200 + case, S, N, nan_frac=float(rng.choice([0.0, 0.03, 0.15])), inf_frac=0.0)
+    if case % 2 == 0:
+        sk, wk = int(rng.integers(0, 2)), int(rng.integers(0, 2))
+        _family_case(umi, x, W, sk, wk, alpha=alpha, n_iter=n_iter)
+    else:
+        dt = float(rng.choice([2.0 / 1440, 0.02, 1.0]))
+        t0 = float(rng.choice([0.0, 2457000.5, -3.25]))
+        t, f, slot = lc.compact(x, dt, t0=t0, jitter=float(rng.choice([0.0, 0.25, 0.45])), seed=case)
+        n_grid = max(0, N - int(rng.integers(0, 5)))
+        ref = orc.gapped(t, f, t0, dt, n_grid, W, alpha=alpha, n_iter=n_iter)
+        trend, flat = umi.umi_detrend_gapped(_cuda(t, np.float64), _cuda(f, np.float32), t0, dt, n_grid, W,
+                                             alpha=alpha, n_iter=n_iter, flat=True)
+        torch.cuda.synchronize()
+        if n_iter == 0:
+            parity.compare_median(trend.cpu().numpy(), ref.median)
+        else:
+            parity.compare_trend(trend.cpu().numpy(), ref)
+        _check_flat(flat.cpu().numpy(), f, ref)
