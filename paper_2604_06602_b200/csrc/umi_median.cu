@@ -248,6 +248,7 @@ umi_median_kernel(MedianParams prm)
 
         /* first window of each walker: n = population of its bitset, median = k-th set bit */
         int n = 0, rho = -1;
+        MadRange mr = {0, 0, 0};
         if (tid < nwa) {
             const uint32_t* row = bits + tid * BWP;
             const uint32_t* off = boff + (tid >> 5) * BW;
@@ -264,6 +265,34 @@ umi_median_kernel(MedianParams prm)
                     }
                     need -= pc;
                 }
+                if constexpr (MAD) {
+                    /* A first guess of the MAD range from the bitset, a whole 32-rank word at a time (about
+                       W/U * 32 members each) instead of one member at a time: grow on the side whose word
+                       boundary is nearer to the median in value until at least (n-1)/2 + 1 members are inside;
+                       mad_fix() below then trims and balances it exactly.  ~NS/64 steps instead of ~W/2. */
+                    const int target = ((n - 1) >> 1) + 1;
+                    const float med = key_to_float((uint32_t)(srt[rho] >> 32));
+                    int wl = rho >> 5, wr = wl;
+                    int cnt = __popc(row[wl] ^ off[wl]);
+                    const int wmax = (nvu - 1) >> 5;
+                    while (cnt < target) {
+                        const bool can_l = wl > 0, can_r = wr < wmax;
+                        if (!can_l && !can_r) break;
+                        bool left = can_l;
+                        if (can_l && can_r) {
+                            const float dl = med - key_to_float((uint32_t)(srt[32 * wl - 1] >> 32));
+                            const float dr = key_to_float((uint32_t)(srt[32 * (wr + 1)] >> 32)) - med;
+                            left = dl <= dr;
+                        }
+                        if (left) { --wl; cnt += __popc(row[wl] ^ off[wl]); }
+                        else      { ++wr; cnt += __popc(row[wr] ^ off[wr]); }
+                    }
+                    while ((row[wl] ^ off[wl]) == 0u) ++wl;             /* rho's word is inside: both loops stop */
+                    while ((row[wr] ^ off[wr]) == 0u) --wr;
+                    mr.L = 32 * wl + __ffs((int)(row[wl] ^ off[wl])) - 1;
+                    mr.R = 32 * wr + 31 - __clz((int)(row[wr] ^ off[wr]));
+                    mr.cnt = cnt;
+                }
             }
         }
         __syncthreads();                                            /* bitsets are dead: medbuf reuses them */
@@ -275,7 +304,6 @@ umi_median_kernel(MedianParams prm)
             if (pend > Tact) pend = Tact;
             const uint32_t uW = (uint32_t)W;
             int p = pbeg;
-            MadRange mr = {0, 0, 0};
             float mad = 0.f;
             /* window members next to rank r, under the window of position q */
             auto val = [&](int r) { return key_to_float((uint32_t)(srt[r] >> 32)); };
