@@ -129,8 +129,9 @@ umi_median_kernel(MedianParams prm)
 #ifndef UMI_K1_MAD_WALKERS
 #define UMI_K1_MAD_WALKERS 128
 #endif
-    /* walkers per tile (measured on config 2: 32 / 64 / 128 MAD walkers -> 20.4 / 18.3 / 18.1 ms per step: the per-slide
-       range repair, not the O(W) set-up, is what costs, so the MAD variant keeps the same count) */
+    /* walkers per tile: the MAD variant keeps the same count (with the member-by-member set-up of the range,
+       32 / 64 / 128 walkers measured 20.4 / 18.3 / 18.1 ms per config-2 step: fewer, longer walks lose more in
+       parallelism than they save in set-up; the set-up itself is now word-by-word from the bitset) */
     constexpr int NW = MAD ? (UMI_K1_MAD_WALKERS < k1_walkers(NS) ? UMI_K1_MAD_WALKERS : k1_walkers(NS)) : k1_walkers(NS);
     constexpr int NWB = NW / 32;                                    /* walker blocks of 32 */
     extern __shared__ __align__(16) unsigned char smem_raw[];
