@@ -26,6 +26,10 @@
  *  - Invalid sample: flux not finite (NaN, +Inf, -Inf), or time given and not
  *    finite.  Invalid samples and slots outside [0, n_cadences) are skipped by
  *    every window (R2, R3, R16).
+ *  - Reproducibility: a call is deterministic (no atomics on floating-point data), and the median is
+ *    bit-exact always.  The trend of a star may differ in its last bits (~1e-7 relative) between calls
+ *    with different batch sizes, because small batches run the split-window variant of the
+ *    reweighting kernel, which sums the same terms in another order.
  *  - Supported dynamic range: within one tile of ~512 consecutive cadences,
  *    (max - min) * 8 * max(1, 1/alpha) must be finite in fp32.
  */
@@ -186,6 +190,21 @@ int umi_detrend_host(const double* time, const float* flux,
                      int64_t n_stars, int64_t n_cadences,
                      int W, float alpha, int n_iter,
                      float* trend_out,
+                     int64_t stars_per_batch, int n_streams);
+
+/*
+ * The batch driver with the normalisation fused in (detrending + normalization on a
+ * whole sector from host memory): umi_detrend_host with c / min_valid exposed and
+ * flat_out = flux / trend copied back as well.
+ *   trend_out  HOST, float [n_stars*n_cadences], or NULL when only the flattened curve is wanted
+ *              (the trend then never crosses PCIe).
+ *   flat_out   HOST, float [n_stars*n_cadences]; required.
+ * Everything else as umi_detrend_host.
+ */
+int umi_flatten_host(const double* time, const float* flux,
+                     int64_t n_stars, int64_t n_cadences,
+                     int W, float alpha, float c, int n_iter, int min_valid,
+                     float* trend_out, float* flat_out,
                      int64_t stars_per_batch, int n_streams);
 
 /*

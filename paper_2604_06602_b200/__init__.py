@@ -22,7 +22,7 @@ UMI_SCALE_UPPER_RMS, UMI_SCALE_MAD = 0, 1
 UMI_WEIGHT_BISQUARE, UMI_WEIGHT_WELSCH = 0, 1
 
 EXPORTS = ("umi_window_len", "umi_detrend", "umi_detrend_ex", "umi_detrend_host", "umi_detrend_profile",
-           "umi_flatten", "umi_detrend_family", "umi_detrend_gapped", "umi_gapped_workspace_bytes",
+           "umi_flatten", "umi_flatten_host", "umi_detrend_family", "umi_detrend_gapped", "umi_gapped_workspace_bytes",
            "umi_launch_geometry", "umi_status_string", "umi_version")
 
 _lib = None
@@ -57,6 +57,8 @@ def lib():
     L.umi_detrend_host.argtypes = [vp, vp, i64, i64, ci, cf, ci, vp, i64, ci]
     L.umi_flatten.restype = ci
     L.umi_flatten.argtypes = [vp, vp, i64, i64, ci, cf, cf, ci, ci, vp, vp, vp]
+    L.umi_flatten_host.restype = ci
+    L.umi_flatten_host.argtypes = [vp, vp, i64, i64, ci, cf, cf, ci, ci, vp, vp, i64, ci]
     L.umi_detrend_family.restype = ci
     L.umi_detrend_family.argtypes = [vp, vp, i64, i64, ci, ci, ci, cf, cf, ci, ci, vp, vp, vp, vp]
     L.umi_gapped_workspace_bytes.restype = ctypes.c_size_t
@@ -299,3 +301,32 @@ def umi_detrend_host(time, flux, W, alpha=2.0, n_iter=5, out=None, stars_per_bat
         _check(lib().umi_detrend_host(tptr, f.ctypes.data, S, N, int(W), float(alpha), int(n_iter),
                                       o.ctypes.data, int(stars_per_batch), int(n_streams)))
     return out
+
+
+def umi_flatten_host(time, flux, W, alpha=2.0, n_iter=5, c=5.0, min_valid=-1, want_trend=True,
+                     stars_per_batch=0, n_streams=0):
+    """Host path with the normalisation fused in: returns (trend or None, flat) as numpy arrays of
+    flux's shape.  `flux`: C-contiguous fp32 numpy array or CPU tensor; pinned memory overlaps copies."""
+    import numpy as np
+    try:
+        import torch
+    except ImportError:  # pragma: no cover
+        torch = None
+    f = flux.numpy() if (torch is not None and isinstance(flux, torch.Tensor)) else flux
+    if not isinstance(f, np.ndarray) or f.dtype != np.float32 or not f.flags.c_contiguous:
+        raise TypeError("flux must be a C-contiguous float32 host array")
+    f2 = f.reshape(1, -1) if f.ndim == 1 else f
+    tptr = None
+    if time is not None:
+        t = time.numpy() if (torch is not None and isinstance(time, torch.Tensor)) else time
+        if not isinstance(t, np.ndarray) or t.dtype != np.float64 or not t.flags.c_contiguous or t.size != f.size:
+            raise TypeError("time must be a C-contiguous float64 host array of flux's shape")
+        tptr = t.ctypes.data
+    trend = np.empty_like(f) if want_trend else None
+    flat = np.empty_like(f)
+    S, N = f2.shape
+    if S and N:
+        _check(lib().umi_flatten_host(tptr, f.ctypes.data, S, N, int(W), float(alpha), float(c), int(n_iter),
+                                      int(min_valid), trend.ctypes.data if want_trend else None, flat.ctypes.data,
+                                      int(stars_per_batch), int(n_streams)))
+    return trend, flat

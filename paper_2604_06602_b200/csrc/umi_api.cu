@@ -312,11 +312,18 @@ int umi_detrend(const double* time, const float* flux, int64_t n_stars, int64_t 
                           trend_out, stream);
 }
 
-int umi_detrend_host(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
-                     int W, float alpha, int n_iter, float* trend_out,
-                     int64_t stars_per_batch, int n_streams)
+} /* extern "C" */
+
+namespace {
+
+/* the batch driver behind umi_detrend_host / umi_flatten_host: trend_out and flat_out are HOST pointers,
+   either may be null (not both) */
+int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
+                int W, float alpha, float c, int n_iter, int min_valid, float* trend_out, float* flat_out,
+                int64_t stars_per_batch, int n_streams)
 {
-    const int st = validate(flux, n_stars, n_cadences, W, alpha, 5.0f, n_iter, trend_out);
+    if (trend_out == nullptr && flat_out == nullptr) return UMI_ERR_INVALID_ARG;
+    const int st = validate(flux, n_stars, n_cadences, W, alpha, c, n_iter, trend_out ? trend_out : flat_out);
     if (st != UMI_OK) return st;
     if (n_stars == 0 || n_cadences == 0) return UMI_OK;
     if (n_streams <= 0) n_streams = 3;
@@ -337,6 +344,7 @@ int umi_detrend_host(const double* time, const float* flux, int64_t n_stars, int
         cudaStream_t stream = nullptr;
         float* d_flux = nullptr;
         float* d_trend = nullptr;
+        float* d_flat = nullptr;
         double* d_time = nullptr;
     };
     std::vector<Slot> slots((size_t)n_streams);
@@ -362,6 +370,7 @@ int umi_detrend_host(const double* time, const float* flux, int64_t n_stars, int
             /* stream-ordered allocations: served from the driver's pool after the first call */
             cuda_failed(cudaMallocAsync((void**)&s.d_flux, elems * sizeof(float), s.stream)) ||
             cuda_failed(cudaMallocAsync((void**)&s.d_trend, elems * sizeof(float), s.stream)) ||
+            (flat_out != nullptr && cuda_failed(cudaMallocAsync((void**)&s.d_flat, elems * sizeof(float), s.stream))) ||
             (time != nullptr && cuda_failed(cudaMallocAsync((void**)&s.d_time, elems * sizeof(double), s.stream)))) {
             status = UMI_ERR_CUDA;
             break;
@@ -381,9 +390,13 @@ int umi_detrend_host(const double* time, const float* flux, int64_t n_stars, int
             status = UMI_ERR_CUDA;
             break;
         }
-        status = launch_device(s.d_time, s.d_flux, ns, n_cadences, W, alpha, 5.0f, n_iter, -1, s.d_trend, s.stream);
+        status = launch_device(s.d_time, s.d_flux, ns, n_cadences, W, alpha, c, n_iter, min_valid, s.d_trend, s.stream,
+                               nullptr, s.d_flat);
         if (status != UMI_OK) break;
-        if (cuda_failed(cudaMemcpyAsync(trend_out + off, s.d_trend, cnt * sizeof(float), cudaMemcpyDeviceToHost, s.stream)))
+        if ((trend_out != nullptr &&
+             cuda_failed(cudaMemcpyAsync(trend_out + off, s.d_trend, cnt * sizeof(float), cudaMemcpyDeviceToHost, s.stream))) ||
+            (flat_out != nullptr &&
+             cuda_failed(cudaMemcpyAsync(flat_out + off, s.d_flat, cnt * sizeof(float), cudaMemcpyDeviceToHost, s.stream))))
             status = UMI_ERR_CUDA;
     }
 
@@ -391,6 +404,7 @@ int umi_detrend_host(const double* time, const float* flux, int64_t n_stars, int
         if (s.stream == nullptr) continue;
         if (s.d_flux) (void)cudaFreeAsync(s.d_flux, s.stream);
         if (s.d_trend) (void)cudaFreeAsync(s.d_trend, s.stream);
+        if (s.d_flat) (void)cudaFreeAsync(s.d_flat, s.stream);
         if (s.d_time) (void)cudaFreeAsync(s.d_time, s.stream);
         if (cuda_failed(cudaStreamSynchronize(s.stream))) status = UMI_ERR_CUDA;
     }
@@ -399,6 +413,28 @@ int umi_detrend_host(const double* time, const float* flux, int64_t n_stars, int
     }
     (void)cudaGetLastError();
     return status;
+}
+
+} // namespace
+
+extern "C" {
+
+int umi_detrend_host(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
+                     int W, float alpha, int n_iter, float* trend_out,
+                     int64_t stars_per_batch, int n_streams)
+{
+    if (trend_out == nullptr) return UMI_ERR_INVALID_ARG;
+    return host_driver(time, flux, n_stars, n_cadences, W, alpha, 5.0f /* PAPER.md:63 */, n_iter, -1, trend_out, nullptr,
+                       stars_per_batch, n_streams);
+}
+
+int umi_flatten_host(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
+                     int W, float alpha, float c, int n_iter, int min_valid,
+                     float* trend_out, float* flat_out, int64_t stars_per_batch, int n_streams)
+{
+    if (flat_out == nullptr) return UMI_ERR_INVALID_ARG;
+    return host_driver(time, flux, n_stars, n_cadences, W, alpha, c, n_iter, min_valid, trend_out, flat_out,
+                       stars_per_batch, n_streams);
 }
 
 int umi_launch_geometry(int W, int* median_tile, int* median_sort_n, int* weight_tile)

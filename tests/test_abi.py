@@ -87,6 +87,8 @@ def test_validation_happens_on_the_host():
     assert gap(ws=None) == umi.UMI_ERR_INVALID_ARG
     assert gap(wsb=95) == umi.UMI_ERR_INVALID_ARG      # 2 * 1 * 12 * 4 = 96 bytes needed
     assert gap(S=0) == umi.UMI_OK
+    assert L.umi_flatten_host(None, one, 1, 10, 5, 2.0, 5.0, 5, -1, one, None, 0, 0) == umi.UMI_ERR_INVALID_ARG
+    assert L.umi_flatten_host(None, one, 0, 10, 5, 2.0, 5.0, 5, -1, None, one, 0, 0) == umi.UMI_OK
     fam = lambda **k: L.umi_detrend_family(None, one, k.get("S", 1), 10, 5, k.get("sk", 0), k.get("wk", 0), 2.0, 5.0, 5, -1,
                                            one, k.get("scale", one), None, None)
     assert fam(sk=2) == umi.UMI_ERR_INVALID_ARG

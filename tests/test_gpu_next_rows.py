@@ -217,3 +217,17 @@ def test_fuzz_family_and_gapped(umi, case):
         else:
             parity.compare_trend(trend.cpu().numpy(), ref)
         _check_flat(flat.cpu().numpy(), f, ref)
+
+
+def test_flatten_host_driver(umi):
+    # host buffers in, (trend, flat) back through the streamed batch driver; and flat only
+    cfg = lc.CONFIGS[5]
+    flux = lc.stars(5, range(40))
+    ref = orc.detrend(flux, cfg.W, alpha=3.0, c=2.5)
+    trend, flat = umi.umi_flatten_host(None, flux, cfg.W, alpha=3.0, c=2.5, stars_per_batch=7, n_streams=3)
+    parity.compare_trend(trend, ref)
+    _check_flat(flat, flux, ref)
+    none, flat2 = umi.umi_flatten_host(None, flux, cfg.W, alpha=3.0, c=2.5, want_trend=False)
+    # other batch size -> the other variant of the reweighting kernel (split-window vs throughput): same
+    # arithmetic, another summation order, so equal to rounding, not bit for bit
+    assert none is None and np.allclose(flat2, flat, rtol=2e-6, atol=0.0, equal_nan=True)
