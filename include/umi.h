@@ -31,7 +31,7 @@
  *    with different batch sizes, because small batches run the split-window variant of the
  *    reweighting kernel, which sums the same terms in another order.
  *  - Supported dynamic range: within one tile of ~512 consecutive cadences,
- *    (max - min) * 8 * max(1, 1/alpha) must be finite in fp32.
+ *    (max - min) * 16 * max(1, 1/alpha) must be finite in fp32.
  */
 #ifndef UMI_B200_H
 #define UMI_B200_H

@@ -24,10 +24,10 @@
 #define UMI_K2_PACKED 1
 #endif
 #ifndef UMI_K2_MIN_CTAS
-#define UMI_K2_MIN_CTAS 8
+#define UMI_K2_MIN_CTAS 5
 #endif
 #ifndef UMI_K2_UNROLL
-#define UMI_K2_UNROLL 2
+#define UMI_K2_UNROLL 8
 #endif
 
 namespace umi {
@@ -56,7 +56,7 @@ __device__ __forceinline__ void eval_weight(float x, float k, float c0, float na
     const float t = __saturatef(fmaf(-e, e, 1.f));   /* FFMA.SAT */
     const float w = t * t;
     S += w;
-    R = fmaf(w, a, R);
+    R = fmaf(w, x, R);                               /* sum w x (centred samples): Eq. 4's numerator */
 }
 
 /* Sibling weight (F4; R22): Welsch, w = exp(-u_eff^2), no cut-off. */
@@ -67,7 +67,7 @@ __device__ __forceinline__ void eval_welsch(float x, float k, float c0, float na
     const float e = fmaxf(a, a * nalpha);            /* |u_eff| */
     const float w = exp2f(e * e * -1.4426950408889634f);   /* exp(-e^2); 0 for the sentinel (e >= 16) */
     S += w;
-    R = fmaf(w, a, R);
+    R = fmaf(w, x, R);
 }
 
 #if UMI_K2_PACKED
@@ -107,8 +107,9 @@ __device__ __forceinline__ void eval_weight_group(f32x2 x01, f32x2 x23, const f3
 #pragma unroll
     for (int q = 0; q < K2_NPOS; ++q) {
         S2[q] = fadd2(S2[q], fadd2(w2[2 * q], w2[2 * q + 1]));
-        R2[q] = ffma2(w2[2 * q], a2[2 * q], R2[q]);
-        R2[q] = ffma2(w2[2 * q + 1], a2[2 * q + 1], R2[q]);
+        /* sum w x on the sample pairs themselves (shared by the 4 positions), so that u need not stay live */
+        R2[q] = ffma2(w2[2 * q], x01, R2[q]);
+        R2[q] = ffma2(w2[2 * q + 1], x23, R2[q]);
     }
 }
 #endif
@@ -185,9 +186,12 @@ umi_reweight_kernel(ReweightParams prm)
                 sent = tmin - (MODE == 2 ? 24.f : 2.f) * (prm.c / prm.alpha) * (tmax - tmin);
             sent = fmaxf(sent, -3.0e38f);
         }
+        /* everything below works on samples centred on the middle of the tile's range: Eq. 4 is then
+           mu' = sum(w x') / sum(w) with |x'| small, i.e. exact to fp32 without a separate sum of w*u */
+        const float xref = (tmin <= tmax) ? 0.5f * tmin + 0.5f * tmax : 0.f;
         for (int u = tid; u < nx; u += K2_THREADS) {
             const float x = xs[u];
-            if (x != x) xs[u] = sent;
+            xs[u] = ((x != x) ? sent : x) - xref;
         }
         __syncthreads();
 
@@ -198,7 +202,7 @@ umi_reweight_kernel(ReweightParams prm)
 #pragma unroll
         for (int q = 0; q < K2_NPOS; ++q) {
             const int64_t j = j0 + 4 * pt + q;
-            med[q] = (j < prm.N) ? orow[j] : qnan;
+            med[q] = (j < prm.N) ? orow[j] - xref : qnan;
             act[q] = (med[q] == med[q]);
             any_act = any_act || act[q];
             mu[q] = act[q] ? med[q] : 0.f;
@@ -349,7 +353,7 @@ umi_reweight_kernel(ReweightParams prm)
                             R[q] += __shfl_xor_sync(0xFFFFFFFFu, R[q], o);
                         }
                     }
-                    if (act[q] && S[q] > 0.f) mu[q] = fmaf(R[q] / S[q], cs[q], mu[q]);   /* Eq. 4; (R11) */
+                    if (act[q] && S[q] > 0.f) mu[q] = R[q] / S[q];                       /* Eq. 4; (R11) */
                 }
             }
         }
@@ -357,7 +361,7 @@ umi_reweight_kernel(ReweightParams prm)
 #pragma unroll
         for (int q = 0; q < K2_NPOS; ++q) {
             const int64_t j = j0 + 4 * pt + q;
-            if (j < prm.N && med[q] == med[q] && sl == 0) orow[j] = mu[q];
+            if (j < prm.N && med[q] == med[q] && sl == 0) orow[j] = mu[q] + xref;
         }
         if (prm.flat != nullptr) {                                  /* PAPER.md:155 normalisation */
             float* flrow = prm.flat + star * prm.N;
@@ -365,7 +369,7 @@ umi_reweight_kernel(ReweightParams prm)
             for (int q = 0; q < K2_NPOS; ++q) {
                 const int64_t j = j0 + 4 * pt + q;
                 /* own sample = staged index hal + 4*tid + q (valid whenever the median is not NaN) */
-                if (j < prm.N && sl == 0) flrow[j] = (med[q] == med[q]) ? xs[hal + 4 * pt + q] / mu[q] : qnan;
+                if (j < prm.N && sl == 0) flrow[j] = (med[q] == med[q]) ? __ldg(frow + j) / (mu[q] + xref) : qnan;
             }
         }
         __syncthreads();
