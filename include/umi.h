@@ -226,7 +226,8 @@ int umi_detrend_profile(const double* time, const float* flux,
  * arithmetic; host only).  Any pointer may be NULL.
  *   median_tile    positions per CTA of the Phase-1 (median) kernel
  *   median_sort_n  power-of-two length of the per-tile sort
- *   weight_tile    positions per CTA of the Phase-2/3 (reweighting) kernel
+ *   weight_tile    positions per CTA of the Phase-2/3 (reweighting) kernel in its throughput variant
+ *                  (batches of at most 4 x 148 such tiles run the split-window variant: 1/8 of it)
  * Returns UMI_OK, or INVALID_ARG / UNSUPPORTED for a bad W.
  */
 int umi_launch_geometry(int W, int* median_tile, int* median_sort_n, int* weight_tile);
