@@ -1,0 +1,46 @@
+"""CPU checks of the input generators and of the injection-recovery bookkeeping (no method
+arithmetic lives in `workloads/`; these tests only pin shapes, seeds and the depth metric)."""
+import numpy as np
+
+from workloads import injection_recovery as ir
+from workloads import lightcurves as lc
+
+
+def test_stars_regenerate_identically_and_have_the_config_shape():
+    a = lc.stars(2, [7, 3])
+    b = lc.stars(2, [3, 7])
+    assert a.shape == (2, lc.CONFIGS[2].n_cadences) and a.dtype == np.float32
+    assert np.array_equal(a[0], b[1], equal_nan=True) and np.array_equal(a[1], b[0], equal_nan=True)
+    assert np.isnan(a[:, 9360:10080]).all() and np.isfinite(a[:, :9360]).all()
+    k = lc.stars(3, [0])
+    assert 0.01 <= np.isnan(k).mean() <= 0.03            # runs of 10-100 NaNs until >= 1 %
+
+
+def test_compact_removes_invalid_slots_and_pads_with_nan_time():
+    grid = lc.random_series(5, 3, 300, nan_frac=0.1, inf_frac=0.0)
+    t, f, slot = lc.compact(grid, 0.5, t0=10.0, jitter=0.2, seed=1)
+    assert t.shape == f.shape == slot.shape and t.shape[0] == 3
+    for b in range(3):
+        m = slot[b] >= 0
+        assert m.sum() == np.isfinite(grid[b]).sum()
+        assert np.array_equal(f[b, m], grid[b, slot[b, m]])
+        assert np.all(np.diff(slot[b, m]) > 0)
+        assert np.all(np.abs((t[b, m] - 10.0) / 0.5 - slot[b, m]) <= 0.2 + 1e-9)
+        assert np.isnan(t[b, ~m]).all() and np.isnan(f[b, ~m]).all()
+
+
+def test_injection_metric_with_a_perfect_and_a_transit_eating_detrender():
+    cfg = lc.CONFIGS[2]
+    rng = np.random.default_rng(0)
+    flux = (1.0 + 1e-4 * rng.standard_normal((6, cfg.n_cadences))).astype(np.float32)
+    mask = ir.transit_mask(6, cfg.n_cadences, cfg.dt_days, seed=0)
+    # 3 h every 3 d at 2-min cadence: ~90 cadences per transit, ~9 transits
+    assert 700 <= mask[0].sum() <= 1000
+    inj = ir.inject(flux, mask, 1000.0)
+    assert np.allclose(flux[mask] - inj[mask], 1e-3, atol=2e-7) and np.array_equal(inj[~mask], flux[~mask])
+    perfect = lambda x: x / 1.0                           # trend == 1: nothing absorbed
+    err = ir.depth_errors(flux, cfg.dt_days, perfect, depths_ppm=(1000.0,))
+    assert err[0] < 0.1
+    eater = lambda x: np.ones_like(x)                     # trend == flux: everything absorbed
+    err = ir.depth_errors(flux, cfg.dt_days, eater, depths_ppm=(1000.0,))
+    assert abs(err[0] - 100.0) < 1e-6
