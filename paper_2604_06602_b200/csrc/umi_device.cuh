@@ -82,22 +82,29 @@ __device__ __forceinline__ f32x2 fadd2(f32x2 a, f32x2 b)
 }
 
 
-/* Phase 3 (Eq. 2-4) on two samples of one position at once: S2 += w, R2 += w*u per half.
-   k2 = (k, k), c02 = (c0, c0), nalpha2 = (-alpha, -alpha). */
-__device__ __forceinline__ void eval_weight_pair(f32x2 x2, f32x2 k2, f32x2 c02, f32x2 nalpha2,
+/* -min(|u_eff|, 1) from nu = -u and au = alpha*u (Eq. 2-3).  Exactly one of the two is
+   <= 0 and that one is -|u_eff|; compared as signed integers a non-positive float is below every
+   positive one and, among non-positive floats, a larger magnitude is a larger integer, so the
+   three-input integer minimum with bits(-1.0f) selects -|u_eff| and clamps it at -1 in one DPX
+   instruction (VIMNMX3).  NaN inputs come out as -1 (weight 0), like the float form did. */
+__device__ __forceinline__ float neg_ueff_clamped(float nu, float au)
+{
+    return __int_as_float(__vimin3_s32(__float_as_int(nu), __float_as_int(au), (int)0xBF800000));
+}
+
+/* Phase 3 (Eq. 2-4) on two samples of one position at once, on u' = -u: S2 += w, R2 += w*u' per half
+   (the caller negates the sum).  kn2 = (-k, -k), cn2 = (-c0, -c0), nalpha2 = (-alpha, -alpha). */
+__device__ __forceinline__ void eval_weight_pair(f32x2 x2, f32x2 kn2, f32x2 cn2, f32x2 nalpha2,
                                                  f32x2& S2, f32x2& R2)
 {
-    const f32x2 a2 = ffma2(x2, k2, c02);                 /* u */
-    const f32x2 b2 = fmul2(a2, nalpha2);                 /* -alpha*u */
+    const f32x2 a2 = ffma2(x2, kn2, cn2);                /* -u */
+    const f32x2 b2 = fmul2(a2, nalpha2);                 /* alpha*u */
     float a0, a1, b0, b1;
     unpack2(a2, a0, a1);
     unpack2(b2, b0, b1);
-    const f32x2 e2 = pack2(fmaxf(a0, b0), fmaxf(a1, b1));   /* |u_eff| */
-    const f32x2 n2 = ffma2(e2, e2, pack2(-1.f, -1.f));
-    float n0, n1;
-    unpack2(n2, n0, n1);
-    const f32x2 t2 = pack2(fmaxf(-n0, 0.f), fmaxf(-n1, 0.f));   /* Eq. 3 clamp (R12) */
-    const f32x2 w2 = fmul2(t2, t2);
+    const f32x2 ne2 = pack2(neg_ueff_clamped(a0, b0), neg_ueff_clamped(a1, b1));
+    const f32x2 n2 = ffma2(ne2, ne2, pack2(-1.f, -1.f)); /* -(1 - e^2) <= 0: Eq. 3 cut-off already applied (R12) */
+    const f32x2 w2 = fmul2(n2, n2);
     S2 = fadd2(S2, w2);
     R2 = ffma2(w2, a2, R2);
 }

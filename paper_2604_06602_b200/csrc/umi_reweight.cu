@@ -72,37 +72,34 @@ __device__ __forceinline__ void eval_welsch(float x, float k, float c0, float na
 
 #if UMI_K2_PACKED
 /* Phase 3 on one 128-bit group: 4 samples (two fp32x2 pairs) x 4 positions = 8 pair
-   evaluations, written stage by stage so that the 8 dependency chains interleave. */
-__device__ __forceinline__ void eval_weight_group(f32x2 x01, f32x2 x23, const f32x2 (&k2)[K2_NPOS],
-                                                  const f32x2 (&c02)[K2_NPOS], f32x2 nalpha2,
+   evaluations, written stage by stage so that the 8 dependency chains interleave.
+   kn2 = (-k, -k), cn2 = (mu k, mu k): the group works on u' = -u.  Exactly one of u' and
+   alpha*u = -alpha*u' is <= 0, and it is -|u_eff| of Eq. 2; as signed integers a non-positive float
+   sorts below every positive one, and among non-positive floats the larger magnitude is the larger
+   integer, so ONE three-input integer minimum (DPX VIMNMX3) with the bit pattern of -1.0f gives
+   -min(|u_eff|, 1): Eq. 2's case split and Eq. 3's cut-off in a single ALU-pipe instruction
+   (was: FMNMX for |u_eff| and a second FMNMX for the clamp).  1 - min(|u_eff|,1)^2 is then >= 0
+   by construction, and bitwise the value max(1 - u_eff^2, 0) had. */
+__device__ __forceinline__ void eval_weight_group(f32x2 x01, f32x2 x23, const f32x2 (&kn2)[K2_NPOS],
+                                                  const f32x2 (&cn2)[K2_NPOS], f32x2 nalpha2,
                                                   f32x2 (&S2)[K2_NPOS], f32x2 (&R2)[K2_NPOS])
 {
     f32x2 a2[2 * K2_NPOS], w2[2 * K2_NPOS];
-    float e[4 * K2_NPOS];
 #pragma unroll
     for (int q = 0; q < K2_NPOS; ++q) {
-        a2[2 * q] = ffma2(x01, k2[q], c02[q]);
-        a2[2 * q + 1] = ffma2(x23, k2[q], c02[q]);
-    }
-#pragma unroll
-    for (int i = 0; i < 2 * K2_NPOS; ++i) {
-        const f32x2 b2 = fmul2(a2[i], nalpha2);
-        float a0, a1, b0, b1;
-        unpack2(a2[i], a0, a1);
-        unpack2(b2, b0, b1);
-        e[2 * i] = fmaxf(a0, b0);
-        e[2 * i + 1] = fmaxf(a1, b1);
+        a2[2 * q] = ffma2(x01, kn2[q], cn2[q]);                    /* -u */
+        a2[2 * q + 1] = ffma2(x23, kn2[q], cn2[q]);
     }
     const f32x2 mone2 = pack2(-1.f, -1.f);
 #pragma unroll
     for (int i = 0; i < 2 * K2_NPOS; ++i) {
-        /* e*e - 1 packed; the clamp max(1 - e*e, 0) runs on the ALU pipe (FMNMX, negated source),
-           so the FMA pipe only ever sees packed instructions */
-        const f32x2 n2 = ffma2(pack2(e[2 * i], e[2 * i + 1]), pack2(e[2 * i], e[2 * i + 1]), mone2);
-        float n0, n1;
-        unpack2(n2, n0, n1);
-        const f32x2 t2 = pack2(fmaxf(-n0, 0.f), fmaxf(-n1, 0.f));
-        w2[i] = fmul2(t2, t2);
+        const f32x2 b2 = fmul2(a2[i], nalpha2);                    /* alpha*u */
+        float a0, a1, b0, b1;
+        unpack2(a2[i], a0, a1);
+        unpack2(b2, b0, b1);
+        const f32x2 ne2 = pack2(neg_ueff_clamped(a0, b0), neg_ueff_clamped(a1, b1));
+        const f32x2 n2 = ffma2(ne2, ne2, mone2);                   /* -(1 - e^2) <= 0 */
+        w2[i] = fmul2(n2, n2);                                     /* Eq. 3 */
     }
 #pragma unroll
     for (int q = 0; q < K2_NPOS; ++q) {
@@ -276,14 +273,14 @@ umi_reweight_kernel(ReweightParams prm)
 #pragma unroll
                 for (int q = 0; q < K2_NPOS; ++q) { S[q] = 0.f; R[q] = 0.f; c0[q] = -mu[q] * kk[q]; }
 #if UMI_K2_PACKED
-                f32x2 S2[K2_NPOS], R2[K2_NPOS], k2[K2_NPOS], c02[K2_NPOS];
+                f32x2 S2[K2_NPOS], R2[K2_NPOS], kn2[K2_NPOS], cn2[K2_NPOS];
                 const f32x2 nalpha2 = pack2(nalpha, nalpha);
 #pragma unroll
                 for (int q = 0; q < K2_NPOS; ++q) {
                     S2[q] = pack2(0.f, 0.f);
                     R2[q] = pack2(0.f, 0.f);
-                    k2[q] = pack2(kk[q], kk[q]);
-                    c02[q] = pack2(c0[q], c0[q]);
+                    kn2[q] = pack2(-kk[q], -kk[q]);                 /* exact negations: u' = -u bit for bit */
+                    cn2[q] = pack2(-c0[q], -c0[q]);
                 }
 #endif
                 /* edge groups: samples that belong to some but not all of the 4 windows */
@@ -321,7 +318,7 @@ umi_reweight_kernel(ReweightParams prm)
 #pragma unroll K2_UNROLL
                 for (int g = g_first; g <= g_hi; g += SPLIT) {
                     const ulonglong2 v2 = reinterpret_cast<const ulonglong2*>(xs4)[g];
-                    eval_weight_group(v2.x, v2.y, k2, c02, nalpha2, S2, R2);
+                    eval_weight_group(v2.x, v2.y, kn2, cn2, nalpha2, S2, R2);
                 }
 #else
 #pragma unroll 2

@@ -370,7 +370,7 @@ umi_small_kernel(ReweightParams prm, int min_valid)
                            pairs start at an even index of s[], so q odd peels s[q], q even peels s[q+WT-1] */
                         constexpr int NPAIR = (WT - 1) / 2;
                         const int first = q + (q & 1);
-                        const f32x2 k2 = pack2(k[q], k[q]), c02 = pack2(c0k, c0k), na2 = pack2(nalpha, nalpha);
+                        const f32x2 k2 = pack2(-k[q], -k[q]), c02 = pack2(-c0k, -c0k), na2 = pack2(nalpha, nalpha);   /* pairs work on -u */
                         f32x2 Sa = pack2(0.f, 0.f), Sb = Sa, Ra = Sa, Rb = Sa;
 #pragma unroll
                         for (int j = 0; j < NPAIR; ++j) {
@@ -381,6 +381,8 @@ umi_small_kernel(ReweightParams prm, int min_valid)
                         float S0, S1, R0, R1;
                         unpack2(fadd2(Sa, Sb), S0, S1);
                         unpack2(fadd2(Ra, Rb), R0, R1);
+                        R0 = -R0;                                   /* the pairs summed w*(-u) */
+                        R1 = -R1;
                         {
                             const float xs1 = (q & 1) ? s[q] : s[q + WT - 1];
                             const float u = fmaf(xs1, k[q], c0k);
