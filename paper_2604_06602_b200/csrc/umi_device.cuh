@@ -92,21 +92,50 @@ __device__ __forceinline__ float neg_ueff_clamped(float nu, float au)
     return __int_as_float(__vimin3_s32(__float_as_int(nu), __float_as_int(au), (int)0xBF800000));
 }
 
+/* The same when alpha = 2^APOW exactly (alpha = 2 is the paper's default): alpha*u = -alpha*nu
+   is then ONE integer add on the bit pattern of nu -- 0x80000000 flips the sign, APOW << 23 raises the
+   exponent -- so the multiply leaves the FMA pipe, which is the pipe that limits the kernel, for the ALU
+   pipe (VIADDMNMX = min(nu + const, nu), then VIMNMX with -1.0f).  Bit-identical to the multiply for
+   every normal nu with |nu| < 2^(127-APOW); zero / denormal nu give a |u_eff| below 2^-125 either way
+   (weight exactly 1); the callers route windows in which nu could overflow (k * tile range >= 2^100) to
+   the multiply form, because a nu of -Inf or NaN would wrap to a small value here instead of to weight 0. */
+template <int APOW>
+__device__ __forceinline__ float neg_ueff_clamped_pow2(float nu)
+{
+    constexpr int ADDC = (int)(0x80000000u + ((unsigned)APOW << 23));
+    const int i = __float_as_int(nu);
+    return __int_as_float(__vimin3_s32(i, i + ADDC, (int)0xBF800000));
+}
+
 /* Phase 3 (Eq. 2-4) on two samples of one position at once, on u' = -u: S2 += w, R2 += w*u' per half
-   (the caller negates the sum).  kn2 = (-k, -k), cn2 = (-c0, -c0), nalpha2 = (-alpha, -alpha). */
+   (the caller negates the sum).  kn2 = (-k, -k), cn2 = (-c0, -c0), nalpha2 = (-alpha, -alpha).
+   APOW < 0: any alpha; APOW >= 0: alpha = 2^APOW (nalpha2 unused). */
+template <int APOW>
 __device__ __forceinline__ void eval_weight_pair(f32x2 x2, f32x2 kn2, f32x2 cn2, f32x2 nalpha2,
                                                  f32x2& S2, f32x2& R2)
 {
     const f32x2 a2 = ffma2(x2, kn2, cn2);                /* -u */
-    const f32x2 b2 = fmul2(a2, nalpha2);                 /* alpha*u */
-    float a0, a1, b0, b1;
+    float a0, a1;
     unpack2(a2, a0, a1);
-    unpack2(b2, b0, b1);
-    const f32x2 ne2 = pack2(neg_ueff_clamped(a0, b0), neg_ueff_clamped(a1, b1));
+    f32x2 ne2;
+    if constexpr (APOW >= 0) {
+        ne2 = pack2(neg_ueff_clamped_pow2<APOW>(a0), neg_ueff_clamped_pow2<APOW>(a1));
+    } else {
+        const f32x2 b2 = fmul2(a2, nalpha2);             /* alpha*u */
+        float b0, b1;
+        unpack2(b2, b0, b1);
+        ne2 = pack2(neg_ueff_clamped(a0, b0), neg_ueff_clamped(a1, b1));
+    }
     const f32x2 n2 = ffma2(ne2, ne2, pack2(-1.f, -1.f)); /* -(1 - e^2) <= 0: Eq. 3 cut-off already applied (R12) */
     const f32x2 w2 = fmul2(n2, n2);
     S2 = fadd2(S2, w2);
     R2 = ffma2(w2, a2, R2);
+}
+
+/* alpha = 2^m for m in {0, 1, 2} -> m, else -1 (which compiled variant of the passes a launch takes) */
+__host__ __device__ inline int alpha_pow2(float alpha)
+{
+    return alpha == 1.f ? 0 : alpha == 2.f ? 1 : alpha == 4.f ? 2 : -1;
 }
 
 } // namespace umi

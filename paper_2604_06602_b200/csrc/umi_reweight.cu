@@ -26,8 +26,14 @@
 #ifndef UMI_K2_MIN_CTAS
 #define UMI_K2_MIN_CTAS 5
 #endif
+#ifndef UMI_K2_MIN_CTAS_POW2
+#define UMI_K2_MIN_CTAS_POW2 8     /* alpha = 2^m builds: one FMA-pipe value fewer is live; 64 registers, 8 CTAs/SM measured best */
+#endif
 #ifndef UMI_K2_UNROLL
 #define UMI_K2_UNROLL 8
+#endif
+#ifndef UMI_K2_UNROLL_POW2
+#define UMI_K2_UNROLL_POW2 4     /* measured with 8 CTAs/SM: 4 is best across W = 217 / 361 / 2161 (8 wins 0.4 % at 361, loses 5 % at 217) */
 #endif
 
 namespace umi {
@@ -35,6 +41,7 @@ namespace umi {
 namespace {
 
 constexpr int K2_UNROLL = UMI_K2_UNROLL;
+constexpr int K2_UNROLL_POW2 = UMI_K2_UNROLL_POW2;
 
 /* Phase 2, Eq. 1: strictly-above-median residuals (R7). */
 __device__ __forceinline__ void eval_scale(float x, float med, float& ss, float& cnt)
@@ -80,6 +87,7 @@ __device__ __forceinline__ void eval_welsch(float x, float k, float c0, float na
    -min(|u_eff|, 1): Eq. 2's case split and Eq. 3's cut-off in a single ALU-pipe instruction
    (was: FMNMX for |u_eff| and a second FMNMX for the clamp).  1 - min(|u_eff|,1)^2 is then >= 0
    by construction, and bitwise the value max(1 - u_eff^2, 0) had. */
+template <int APOW>
 __device__ __forceinline__ void eval_weight_group(f32x2 x01, f32x2 x23, const f32x2 (&kn2)[K2_NPOS],
                                                   const f32x2 (&cn2)[K2_NPOS], f32x2 nalpha2,
                                                   f32x2 (&S2)[K2_NPOS], f32x2 (&R2)[K2_NPOS])
@@ -93,11 +101,17 @@ __device__ __forceinline__ void eval_weight_group(f32x2 x01, f32x2 x23, const f3
     const f32x2 mone2 = pack2(-1.f, -1.f);
 #pragma unroll
     for (int i = 0; i < 2 * K2_NPOS; ++i) {
-        const f32x2 b2 = fmul2(a2[i], nalpha2);                    /* alpha*u */
-        float a0, a1, b0, b1;
+        float a0, a1;
         unpack2(a2[i], a0, a1);
-        unpack2(b2, b0, b1);
-        const f32x2 ne2 = pack2(neg_ueff_clamped(a0, b0), neg_ueff_clamped(a1, b1));
+        f32x2 ne2;
+        if constexpr (APOW >= 0) {                                  /* alpha = 2^APOW: no multiply (umi_device.cuh) */
+            ne2 = pack2(neg_ueff_clamped_pow2<APOW>(a0), neg_ueff_clamped_pow2<APOW>(a1));
+        } else {
+            const f32x2 b2 = fmul2(a2[i], nalpha2);                /* alpha*u */
+            float b0, b1;
+            unpack2(b2, b0, b1);
+            ne2 = pack2(neg_ueff_clamped(a0, b0), neg_ueff_clamped(a1, b1));
+        }
         const f32x2 n2 = ffma2(ne2, ne2, mone2);                   /* -(1 - e^2) <= 0 */
         w2[i] = fmul2(n2, n2);                                     /* Eq. 3 */
     }
@@ -118,9 +132,11 @@ __device__ __forceinline__ void eval_weight_group(f32x2 x01, f32x2 x23, const f3
 /* SPLIT > 1 (small batches, where the grid would not fill the GPU): SPLIT adjacent lanes share the 4
    positions, each taking every SPLIT-th 128-bit group of the windows; the partial sums are combined
    with xor shuffles after every pass.  A CTA then owns K2_TILE / SPLIT positions and a thread's serial
-   chain is SPLIT times shorter.  SPLIT = 1 is the throughput configuration. */
-template <int MODE, int SPLIT>
-__global__ void __launch_bounds__(K2_THREADS, UMI_K2_MIN_CTAS)
+   chain is SPLIT times shorter.  SPLIT = 1 is the throughput configuration.
+   APOW >= 0: the launch has alpha = 2^APOW and the interior loop forms alpha*u without a multiply;
+   warps in which -u could overflow take the general loop, which is compiled in beside it. */
+template <int MODE, int SPLIT, int APOW>
+__global__ void __launch_bounds__(K2_THREADS, (APOW >= 0 && SPLIT == 1) ? UMI_K2_MIN_CTAS_POW2 : UMI_K2_MIN_CTAS)
 umi_reweight_kernel(ReweightParams prm)
 {
     constexpr int TILE = K2_TILE / SPLIT;
@@ -151,7 +167,8 @@ umi_reweight_kernel(ReweightParams prm)
         const int64_t jbase = j0 - hal;                 /* cadence of staged index 0 */
         const float* frow = prm.flux + star * prm.N;
         const double* trow = prm.time ? prm.time + star * prm.N : nullptr;
-        float* orow = prm.out + star * prm.N;
+        float* otile = prm.out + star * prm.N + j0;          /* the tile's TILE positions of the output row */
+        const int nrow = (int)((prm.N - j0 < TILE) ? prm.N - j0 : TILE);   /* positions of the tile inside the row */
 
         /* stage the union, NaN marks invalid; tile min / max of the valid samples */
         float tmin = INFINITY, tmax = -INFINITY;
@@ -186,6 +203,7 @@ umi_reweight_kernel(ReweightParams prm)
         /* everything below works on samples centred on the middle of the tile's range: Eq. 4 is then
            mu' = sum(w x') / sum(w) with |x'| small, i.e. exact to fp32 without a separate sum of w*u */
         const float xref = (tmin <= tmax) ? 0.5f * tmin + 0.5f * tmax : 0.f;
+        const float xabs = (tmin <= tmax) ? fmaxf(fabsf(sent - xref), fabsf(tmax - xref)) : 0.f;   /* max |x'| staged */
         for (int u = tid; u < nx; u += K2_THREADS) {
             const float x = xs[u];
             xs[u] = ((x != x) ? sent : x) - xref;
@@ -193,21 +211,23 @@ umi_reweight_kernel(ReweightParams prm)
         __syncthreads();
 
         /* per-position state: 4 consecutive positions, local index 4*tid + q */
-        float med[K2_NPOS], mu[K2_NPOS], kk[K2_NPOS], cs[K2_NPOS];
+        float mu[K2_NPOS], kk[K2_NPOS], cs[K2_NPOS];
         bool act[K2_NPOS];
         bool any_act = false;
+        unsigned has_med = 0u;                              /* bit q: position q has a median, i.e. a trend */
 #pragma unroll
         for (int q = 0; q < K2_NPOS; ++q) {
-            const int64_t j = j0 + 4 * pt + q;
-            med[q] = (j < prm.N) ? orow[j] - xref : qnan;
-            act[q] = (med[q] == med[q]);
+            const int jl = 4 * pt + q;                      /* position inside the tile (32-bit from here on) */
+            const float med = (jl < nrow) ? otile[jl] - xref : qnan;
+            act[q] = (med == med);
+            has_med |= act[q] ? (1u << q) : 0u;
             any_act = any_act || act[q];
-            mu[q] = act[q] ? med[q] : 0.f;
+            mu[q] = act[q] ? med : 0.f;
             kk[q] = 0.f;
             cs[q] = 0.f;
             if constexpr (MODE != 0) {                              /* no trend, no scale */
-                if (prm.scale_in == nullptr && prm.scale_out != nullptr && j < prm.N && !act[q])
-                    prm.scale_out[star * prm.N + j] = qnan;
+                if (prm.scale_in == nullptr && prm.scale_out != nullptr && jl < nrow && !act[q])
+                    prm.scale_out[star * prm.N + j0 + jl] = qnan;
             }
         }
         const float4* xs4 = reinterpret_cast<const float4*>(xs) + pt;
@@ -254,12 +274,12 @@ umi_reweight_kernel(ReweightParams prm)
                     on = s > 0.f;
                 }
                 if constexpr (MODE != 0) {
-                    const int64_t j = j0 + 4 * pt + q;
+                    const int jl = 4 * pt + q;
                     if (given) {                                    /* the MAD from the selection kernel */
-                        s = (act[q] && j < prm.N) ? prm.scale_in[star * prm.N + j] : 0.f;
+                        s = (act[q] && jl < nrow) ? prm.scale_in[star * prm.N + j0 + jl] : 0.f;
                         on = act[q] && s > 0.f;
-                    } else if (prm.scale_out != nullptr && j < prm.N && act[q] && sl == 0) {
-                        prm.scale_out[star * prm.N + j] = s;
+                    } else if (prm.scale_out != nullptr && jl < nrow && act[q] && sl == 0) {
+                        prm.scale_out[star * prm.N + j0 + jl] = s;
                     }
                 }
                 act[q] = on;
@@ -267,6 +287,13 @@ umi_reweight_kernel(ReweightParams prm)
                 kk[q] = on ? 1.f / cs[q] : 0.f;
             }
 
+            /* alpha = 2^APOW loop only where -u = k (mu' - x') cannot overflow: |x'|, |mu'| <= xabs */
+            bool risky = false;
+            if constexpr (APOW >= 0) {
+#pragma unroll
+                for (int q = 0; q < K2_NPOS; ++q) risky = risky || !(kk[q] * xabs < 1.2676506e30f);   /* 2^100 */
+                risky = __any_sync(0xFFFFFFFFu, risky);
+            }
             /* ---- Phase 3 (Eq. 2-4), s held fixed (R9), exactly n_iter passes (R10) ---- */
             for (int it = 0; it < prm.n_iter; ++it) {
                 float S[K2_NPOS], R[K2_NPOS], c0[K2_NPOS];
@@ -315,10 +342,18 @@ umi_reweight_kernel(ReweightParams prm)
                     }
                 } else {
 #if UMI_K2_PACKED
+                if (APOW >= 0 && !risky) {
+#pragma unroll K2_UNROLL_POW2
+                    for (int g = g_first; g <= g_hi; g += SPLIT) {
+                        const ulonglong2 v2 = reinterpret_cast<const ulonglong2*>(xs4)[g];
+                        eval_weight_group<APOW>(v2.x, v2.y, kn2, cn2, nalpha2, S2, R2);
+                    }
+                } else {
 #pragma unroll K2_UNROLL
-                for (int g = g_first; g <= g_hi; g += SPLIT) {
-                    const ulonglong2 v2 = reinterpret_cast<const ulonglong2*>(xs4)[g];
-                    eval_weight_group(v2.x, v2.y, kn2, cn2, nalpha2, S2, R2);
+                    for (int g = g_first; g <= g_hi; g += SPLIT) {
+                        const ulonglong2 v2 = reinterpret_cast<const ulonglong2*>(xs4)[g];
+                        eval_weight_group<-1>(v2.x, v2.y, kn2, cn2, nalpha2, S2, R2);
+                    }
                 }
 #else
 #pragma unroll 2
@@ -357,16 +392,16 @@ umi_reweight_kernel(ReweightParams prm)
 
 #pragma unroll
         for (int q = 0; q < K2_NPOS; ++q) {
-            const int64_t j = j0 + 4 * pt + q;
-            if (j < prm.N && med[q] == med[q] && sl == 0) orow[j] = mu[q] + xref;
+            const int jl = 4 * pt + q;
+            if (jl < nrow && ((has_med >> q) & 1u) && sl == 0) otile[jl] = mu[q] + xref;
         }
         if (prm.flat != nullptr) {                                  /* PAPER.md:155 normalisation */
-            float* flrow = prm.flat + star * prm.N;
+            float* flrow = prm.flat + star * prm.N + j0;
 #pragma unroll
             for (int q = 0; q < K2_NPOS; ++q) {
-                const int64_t j = j0 + 4 * pt + q;
+                const int jl = 4 * pt + q;
                 /* own sample = staged index hal + 4*tid + q (valid whenever the median is not NaN) */
-                if (j < prm.N && sl == 0) flrow[j] = (med[q] == med[q]) ? __ldg(frow + j) / (mu[q] + xref) : qnan;
+                if (jl < nrow && sl == 0) flrow[jl] = ((has_med >> q) & 1u) ? __ldg(frow + j0 + jl) / (mu[q] + xref) : qnan;
             }
         }
         __syncthreads();
@@ -375,10 +410,17 @@ umi_reweight_kernel(ReweightParams prm)
 
 cudaError_t launch_reweight(const ReweightParams& prm, bool family, unsigned grid, size_t smem, cudaStream_t stream)
 {
-    if (!family && prm.split == K2_SPLIT) umi_reweight_kernel<0, K2_SPLIT><<<grid, K2_THREADS, smem, stream>>>(prm);
-    else if (!family) umi_reweight_kernel<0, 1><<<grid, K2_THREADS, smem, stream>>>(prm);
-    else if (prm.weight_kind == WEIGHT_WELSCH) umi_reweight_kernel<2, 1><<<grid, K2_THREADS, smem, stream>>>(prm);
-    else umi_reweight_kernel<1, 1><<<grid, K2_THREADS, smem, stream>>>(prm);
+    const int ap = alpha_pow2(prm.alpha);
+    if (!family && prm.split == K2_SPLIT) {
+        if (ap == 1) umi_reweight_kernel<0, K2_SPLIT, 1><<<grid, K2_THREADS, smem, stream>>>(prm);
+        else umi_reweight_kernel<0, K2_SPLIT, -1><<<grid, K2_THREADS, smem, stream>>>(prm);
+    } else if (!family) {
+        if (ap == 0) umi_reweight_kernel<0, 1, 0><<<grid, K2_THREADS, smem, stream>>>(prm);
+        else if (ap == 1) umi_reweight_kernel<0, 1, 1><<<grid, K2_THREADS, smem, stream>>>(prm);
+        else if (ap == 2) umi_reweight_kernel<0, 1, 2><<<grid, K2_THREADS, smem, stream>>>(prm);
+        else umi_reweight_kernel<0, 1, -1><<<grid, K2_THREADS, smem, stream>>>(prm);
+    } else if (prm.weight_kind == WEIGHT_WELSCH) umi_reweight_kernel<2, 1, -1><<<grid, K2_THREADS, smem, stream>>>(prm);
+    else umi_reweight_kernel<1, 1, -1><<<grid, K2_THREADS, smem, stream>>>(prm);
     return cudaGetLastError();
 }
 

@@ -219,7 +219,7 @@ __device__ __forceinline__ void sort3(float& a, float& b, float& c)
  * run on the registers, 4 independent positions interleaved.
  * Any other case goes through small_position, one position at a time.
  */
-template <int WT, bool FAMILY>
+template <int WT, bool FAMILY, int APOW>
 __global__ void __launch_bounds__(KS_THREADS)
 umi_small_kernel(ReweightParams prm, int min_valid)
 {
@@ -348,6 +348,15 @@ umi_small_kernel(ReweightParams prm, int min_valid)
                     cs[q] = on[q] ? prm.c * sc : 0.f;
                     k[q] = on[q] ? 1.f / cs[q] : 0.f;
                 }
+                /* APOW >= 0 (alpha = 2^APOW): the pairs form alpha*u by an integer add (umi_device.cuh) unless
+                   -u = k (mu - x) could overflow somewhere in the warp; |x|, |mu| <= max(|tmin|, |tmax|) */
+                bool risky = false;
+                if constexpr (APOW >= 0) {
+                    const float amax = fmaxf(fabsf(tmin), fabsf(tmax));
+#pragma unroll
+                    for (int q = 0; q < 4; ++q) risky = risky || !(k[q] * amax < 1.2676506e30f);   /* 2^100 */
+                    risky = __any_sync(0xFFFFFFFFu, risky);
+                }
                 /* ---- Phase 3 (Eq. 2-4) ---- */
                 for (int it = 0; it < prm.n_iter; ++it) {
 #pragma unroll
@@ -372,11 +381,20 @@ umi_small_kernel(ReweightParams prm, int min_valid)
                         const int first = q + (q & 1);
                         const f32x2 k2 = pack2(-k[q], -k[q]), c02 = pack2(-c0k, -c0k), na2 = pack2(nalpha, nalpha);   /* pairs work on -u */
                         f32x2 Sa = pack2(0.f, 0.f), Sb = Sa, Ra = Sa, Rb = Sa;
+                        if (APOW >= 0 && !risky) {
 #pragma unroll
-                        for (int j = 0; j < NPAIR; ++j) {
-                            const f32x2 x2 = pack2(s[first + 2 * j], s[first + 2 * j + 1]);
-                            if (j & 1) eval_weight_pair(x2, k2, c02, na2, Sb, Rb);
-                            else       eval_weight_pair(x2, k2, c02, na2, Sa, Ra);
+                            for (int j = 0; j < NPAIR; ++j) {
+                                const f32x2 x2 = pack2(s[first + 2 * j], s[first + 2 * j + 1]);
+                                if (j & 1) eval_weight_pair<APOW>(x2, k2, c02, na2, Sb, Rb);
+                                else       eval_weight_pair<APOW>(x2, k2, c02, na2, Sa, Ra);
+                            }
+                        } else {
+#pragma unroll
+                            for (int j = 0; j < NPAIR; ++j) {
+                                const f32x2 x2 = pack2(s[first + 2 * j], s[first + 2 * j + 1]);
+                                if (j & 1) eval_weight_pair<-1>(x2, k2, c02, na2, Sb, Rb);
+                                else       eval_weight_pair<-1>(x2, k2, c02, na2, Sa, Ra);
+                            }
                         }
                         float S0, S1, R0, R1;
                         unpack2(fadd2(Sa, Sb), S0, S1);
@@ -413,16 +431,16 @@ umi_small_kernel(ReweightParams prm, int min_valid)
     }
 }
 
-template <bool FAMILY>
+template <bool FAMILY, int APOW>
 static cudaError_t launch_small_t(const ReweightParams& prm, int min_valid, int wt, unsigned grid, cudaStream_t stream)
 {
     const size_t smem = (size_t)(KS_TILE + wt - 1) * sizeof(float);
     switch (wt) {
-    case 9: umi_small_kernel<9, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
-    case 17: umi_small_kernel<17, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
-    case 25: umi_small_kernel<25, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
-    case 33: umi_small_kernel<33, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
-    case 49: umi_small_kernel<49, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
+    case 9: umi_small_kernel<9, FAMILY, APOW><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
+    case 17: umi_small_kernel<17, FAMILY, APOW><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
+    case 25: umi_small_kernel<25, FAMILY, APOW><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
+    case 33: umi_small_kernel<33, FAMILY, APOW><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
+    case 49: umi_small_kernel<49, FAMILY, APOW><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
@@ -430,8 +448,11 @@ static cudaError_t launch_small_t(const ReweightParams& prm, int min_valid, int 
 
 cudaError_t launch_small(const ReweightParams& prm, bool family, int min_valid, int wt, unsigned grid, cudaStream_t stream)
 {
-    return family ? launch_small_t<true>(prm, min_valid, wt, grid, stream)
-                  : launch_small_t<false>(prm, min_valid, wt, grid, stream);
+    /* APOW stays -1 here: the integer-add form of alpha*u (umi_device.cuh) was measured on this kernel and is
+       slower (config 3: 30.7 ms against 27.2 ms) -- its ALU pipe already carries the median network, and the
+       second copy of the unrolled passes costs registers; the reweighting kernel is where it pays */
+    return family ? launch_small_t<true, -1>(prm, min_valid, wt, grid, stream)
+                  : launch_small_t<false, -1>(prm, min_valid, wt, grid, stream);
 }
 
 } // namespace umi

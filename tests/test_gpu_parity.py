@@ -143,6 +143,30 @@ def test_large_batch_takes_the_throughput_kernel(umi, W):
     _both(umi, x, W)
 
 
+@pytest.mark.parametrize("alpha", [1.0, 2.0, 4.0, 0.5, 3.0])
+@pytest.mark.parametrize("W", [51, 361])
+def test_power_of_two_alpha_variants(umi, alpha, W):
+    # alpha = 1, 2, 4 take the compiled variants that form alpha*u by an integer add on the bit
+    # pattern (umi_device.cuh); 0.5 and 3 take the multiply form.  Small batch = split-window
+    # kernel, 160 stars = throughput kernel.
+    _both(umi, lc.random_series(1200 + W, 2, 2100, nan_frac=0.02), W, alpha=alpha)
+    _both(umi, lc.random_series(1300 + W, 160, 2100), W, alpha=alpha)
+
+
+@pytest.mark.parametrize("n_stars", [2, 160])
+@pytest.mark.parametrize("alpha", [1.0, 2.0, 4.0])
+def test_overflowing_u_takes_the_multiply_form(umi, n_stars, alpha):
+    # c = 1e-37 makes 1/(c s) overflow: u is Inf or NaN for every sample but the median itself.  Eq. 3 then
+    # gives weight 0 (the trend stays at the median, R11); the integer-add form of alpha*u would wrap a NaN
+    # to a small |u_eff| (weight 1), so such warps must take the multiply form (the kernel's `risky` vote).
+    x = lc.random_series(1400, n_stars, 2100, nan_frac=0.0, inf_frac=0.0)
+    for W in (51, 361):
+        ref = orc.detrend(x, W, alpha=alpha, n_iter=5, c=1e-37)
+        got = _gpu(umi, x, W, alpha=alpha, c=1e-37)
+        parity.compare_trend(got, ref)
+        assert np.array_equal(got, ref.median)
+
+
 @pytest.mark.parametrize("W", [51, 361, 1081])
 def test_tensor_core_variant_of_the_reweighting_kernel(umi, W, monkeypatch):
     # experimental path (UMI_B200_TC=1): weights on the CUDA cores, the sums of Eq. 4 by tcgen05.mma
