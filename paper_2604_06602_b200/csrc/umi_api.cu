@@ -103,6 +103,7 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.n_iter = n_iter;
         rp.alpha = alpha;
         rp.c = c;
+        rp.c_over_alpha = c / alpha;
         rp.split = 1;
         rp.scale_in = nullptr;
         rp.scale_out = fam.scale_out;
@@ -160,6 +161,7 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.n_iter = n_iter;
         rp.alpha = alpha;
         rp.c = c;
+        rp.c_over_alpha = c / alpha;
         rp.scale_in = mad ? fam.scale_out : nullptr;
         rp.scale_out = mad ? nullptr : fam.scale_out;
         rp.weight_kind = fam.weight_kind;
@@ -316,6 +318,33 @@ int umi_detrend(const double* time, const float* flux, int64_t n_stars, int64_t 
 
 namespace {
 
+/* Streams of the batch driver, kept per host thread and per device between calls: creating and destroying
+   three streams per call cost ~0.3 ms of a 8.7 ms config-2 job.  They are never destroyed (a destructor at
+   thread or process exit would call into a CUDA runtime that may already be gone); at most 16 per thread and
+   device.  This is the only state the library keeps; it holds no memory and no data. */
+struct StreamCache {
+    int dev = -1;
+    std::vector<cudaStream_t> streams;
+};
+
+bool cached_streams(int n, std::vector<cudaStream_t>& out)
+{
+    thread_local StreamCache* cache = new StreamCache();          /* leaked on purpose, see above */
+    int dev = 0;
+    if (cuda_failed(cudaGetDevice(&dev))) return false;
+    if (cache->dev != dev) {                                        /* another device: start over (old ones leak) */
+        cache->dev = dev;
+        cache->streams.clear();
+    }
+    while ((int)cache->streams.size() < n) {
+        cudaStream_t st = nullptr;
+        if (cuda_failed(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking))) return false;
+        cache->streams.push_back(st);
+    }
+    out.assign(cache->streams.begin(), cache->streams.begin() + n);
+    return true;
+}
+
 /* the batch driver behind umi_detrend_host / umi_flatten_host: trend_out and flat_out are HOST pointers,
    either may be null (not both) */
 int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
@@ -328,16 +357,40 @@ int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t 
     if (n_stars == 0 || n_cadences == 0) return UMI_OK;
     if (n_streams <= 0) n_streams = 3;
     if (n_streams > 16) n_streams = 16;
-    if (stars_per_batch <= 0) {
-        const int64_t row_bytes = n_cadences * (int64_t)sizeof(float);
-        /* ~16 MiB of flux per batch, but at least 4 batches per stream when the job allows it */
-        stars_per_batch = std::max<int64_t>(1, (16ll << 20) / std::max<int64_t>(row_bytes, 1));
-        const int64_t by_count = (n_stars + 4 * n_streams - 1) / (4 * n_streams);
-        const int64_t floor_b = std::max<int64_t>(1, (2ll << 20) / std::max<int64_t>(row_bytes, 1));
-        stars_per_batch = std::max(floor_b, std::min(stars_per_batch, by_count));
+    /* batch sizes.  Given by the caller: uniform.  Default: a body of ~32 MiB batches between a ramp up and
+       a ramp down by factors of 4 (body/64, body/16, body/4, body ..., body/4, body/16, body/64): only the
+       first host->device copy and the last device->host copy are not hidden behind a kernel, so those two
+       batches are made small, and a factor of 4 keeps every copy shorter than the kernels it runs beside
+       (the kernels take ~6x longer per star than one copy at W = 361 and PCIe 5 x16). */
+    std::vector<int64_t> sizes;
+    if (stars_per_batch > 0) {
+        stars_per_batch = std::min(stars_per_batch, n_stars);
+        for (int64_t left = n_stars; left > 0; left -= std::min(stars_per_batch, left))
+            sizes.push_back(std::min(stars_per_batch, left));
+    } else {
+        const int64_t row_bytes = std::max<int64_t>(n_cadences * (int64_t)sizeof(float), 1);
+        int64_t body = std::max<int64_t>(1, (32ll << 20) / row_bytes);
+        body = std::min(body, std::max<int64_t>(1, (n_stars * 3) / 5));     /* ramps take ~2/3 of a body */
+        const int64_t ramp[3] = {std::max<int64_t>(1, body / 64), std::max<int64_t>(1, body / 16),
+                                 std::max<int64_t>(1, body / 4)};
+        int64_t left = n_stars;
+        for (int i = 0; i < 3 && left > 0 && ramp[i] < body; ++i) {
+            sizes.push_back(std::min(ramp[i], left));
+            left -= sizes.back();
+        }
+        const int64_t tail = ramp[0] + ramp[1] + ramp[2];
+        while (left > tail) {
+            sizes.push_back(std::min(body, left - tail));
+            left -= sizes.back();
+        }
+        for (int i = 2; i >= 0 && left > 0; --i) {
+            sizes.push_back(std::min(ramp[i], left));
+            left -= sizes.back();
+        }
+        if (left > 0) sizes.push_back(left);
+        stars_per_batch = *std::max_element(sizes.begin(), sizes.end());
     }
-    stars_per_batch = std::min(stars_per_batch, n_stars);
-    const int64_t n_batches = (n_stars + stars_per_batch - 1) / stars_per_batch;
+    const int64_t n_batches = (int64_t)sizes.size();
     if ((int64_t)n_streams > n_batches) n_streams = (int)n_batches;
 
     struct Slot {
@@ -365,9 +418,11 @@ int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t 
     const size_t elems = (size_t)stars_per_batch * (size_t)n_cadences;
     int status = UMI_OK;
 
+    std::vector<cudaStream_t> streams;
+    if (!cached_streams(n_streams, streams)) return UMI_ERR_CUDA;
+    for (size_t i = 0; i < slots.size(); ++i) slots[i].stream = streams[i];
     for (auto& s : slots) {
-        if (cuda_failed(cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking)) ||
-            /* stream-ordered allocations: served from the driver's pool after the first call */
+        if (/* stream-ordered allocations: served from the driver's pool after the first call */
             cuda_failed(cudaMallocAsync((void**)&s.d_flux, elems * sizeof(float), s.stream)) ||
             cuda_failed(cudaMallocAsync((void**)&s.d_trend, elems * sizeof(float), s.stream)) ||
             (flat_out != nullptr && cuda_failed(cudaMallocAsync((void**)&s.d_flat, elems * sizeof(float), s.stream))) ||
@@ -377,10 +432,10 @@ int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t 
         }
     }
 
-    for (int64_t b = 0; status == UMI_OK && b < n_batches; ++b) {
+    int64_t s0 = 0;
+    for (int64_t b = 0; status == UMI_OK && b < n_batches; s0 += sizes[(size_t)b], ++b) {
         Slot& s = slots[(size_t)(b % n_streams)];
-        const int64_t s0 = b * stars_per_batch;
-        const int64_t ns = std::min(stars_per_batch, n_stars - s0);
+        const int64_t ns = sizes[(size_t)b];
         const size_t off = (size_t)s0 * (size_t)n_cadences;
         const size_t cnt = (size_t)ns * (size_t)n_cadences;
         /* the slot's stream serialises reuse of its buffers */
@@ -407,9 +462,6 @@ int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t 
         if (s.d_flat) (void)cudaFreeAsync(s.d_flat, s.stream);
         if (s.d_time) (void)cudaFreeAsync(s.d_time, s.stream);
         if (cuda_failed(cudaStreamSynchronize(s.stream))) status = UMI_ERR_CUDA;
-    }
-    for (auto& s : slots) {
-        if (s.stream) (void)cudaStreamDestroy(s.stream);
     }
     (void)cudaGetLastError();
     return status;

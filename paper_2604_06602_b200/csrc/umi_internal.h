@@ -65,6 +65,7 @@ struct ReweightParams {
     int64_t n_blocks;
     int W, n_iter;
     float alpha, c;
+    float c_over_alpha;      /* c / alpha, formed on the host: the sentinel's distance factor ("Sentinel") */
 };
 
 /* Enqueue one kernel; return the launch status (cudaGetLastError). */

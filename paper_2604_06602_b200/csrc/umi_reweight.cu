@@ -195,9 +195,9 @@ umi_reweight_kernel(ReweightParams prm)
         float sent = 0.f;
         if (tmin <= tmax) {
             if constexpr (MODE == 0)
-                sent = tmin - 2.f * (prm.c * SCALE_CONST / prm.alpha) * (tmax - tmin);
+                sent = tmin - (2.f * SCALE_CONST) * prm.c_over_alpha * (tmax - tmin);
             else   /* s <= tmax - tmin for either scale; Welsch needs |u_eff| >= 16 for an exact 0 */
-                sent = tmin - (MODE == 2 ? 24.f : 2.f) * (prm.c / prm.alpha) * (tmax - tmin);
+                sent = tmin - (MODE == 2 ? 24.f : 2.f) * prm.c_over_alpha * (tmax - tmin);
             sent = fmaxf(sent, -3.0e38f);
         }
         /* everything below works on samples centred on the middle of the tile's range: Eq. 4 is then

@@ -244,7 +244,7 @@ umi_reweight_tc_kernel(ReweightParams prm, int nch)
     /* sentinel: alpha (mu - x)/(c s) >= 2 for every window of the tile ("Sentinel") */
     float sent = 0.f;
     if (tmin <= tmax) {
-        sent = tmin - 2.f * (prm.c * SCALE_CONST / prm.alpha) * (tmax - tmin);
+        sent = tmin - (2.f * SCALE_CONST) * prm.c_over_alpha * (tmax - tmin);
         sent = fmaxf(sent, -3.0e38f);
     }
     __syncthreads();                                                /* bm[0..1] scratch has been read */

@@ -267,9 +267,9 @@ umi_small_kernel(ReweightParams prm, int min_valid)
         float sent = 0.f;                                           /* DESIGN.md, "Sentinel" */
         if (tmin <= tmax) {
             if constexpr (!FAMILY)
-                sent = tmin - 2.f * (prm.c * SCALE_CONST / prm.alpha) * (tmax - tmin);
+                sent = tmin - (2.f * SCALE_CONST) * prm.c_over_alpha * (tmax - tmin);
             else   /* s <= tmax - tmin for either scale; Welsch needs |u_eff| >= 16 for an exact 0 */
-                sent = tmin - (prm.weight_kind == WEIGHT_WELSCH ? 24.f : 2.f) * (prm.c / prm.alpha) * (tmax - tmin);
+                sent = tmin - (prm.weight_kind == WEIGHT_WELSCH ? 24.f : 2.f) * prm.c_over_alpha * (tmax - tmin);
             sent = fmaxf(sent, -3.0e38f);
         }
 

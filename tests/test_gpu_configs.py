@@ -133,3 +133,22 @@ def test_host_path_with_time_and_pinned_memory(umi):
     out = umi.umi_detrend_host(torch.from_numpy(t), flux, cfg.W, stars_per_batch=3, n_streams=2)
     ref = orc.detrend(flux.numpy(), cfg.W, time=t)
     parity.compare_trend(out.numpy(), ref)
+
+
+@pytest.mark.parametrize("n_stars", [1, 2, 5, 23, 131])
+def test_host_path_default_batches_ramp_up_and_down(umi, n_stars):
+    # default batching (stars_per_batch <= 0): ramp / body / ramp sizes must cover every star exactly once,
+    # also when the job is smaller than one ramp; called twice (the second call reuses the cached streams)
+    import threading
+    cfg = lc.CONFIGS[5]
+    flux = lc.stars(5, range(n_stars))
+    ref = orc.detrend(flux, cfg.W)
+    for _ in range(2):
+        out = umi.umi_detrend_host(None, flux, cfg.W)
+        parity.compare_trend(out, ref)
+    # another host thread gets streams of its own
+    res = {}
+    th = threading.Thread(target=lambda: res.setdefault("out", umi.umi_detrend_host(None, flux, cfg.W, n_streams=5)))
+    th.start()
+    th.join()
+    parity.compare_trend(res["out"], ref)
