@@ -14,12 +14,13 @@ constexpr int K1_MIN_SORT = 1024;                /* smallest per-tile sort lengt
 __host__ __device__ constexpr int k1_walkers(int ns) { return (131072 / ns) > 32 ? (131072 / ns) : 32; }
 __host__ __device__ constexpr size_t k1_smem_bytes(int ns, bool mad = false)
 {
-    /* u64 sort entries + u16 ranks + max(rank bitsets [NW][NS/32+1] + scan offsets [NW/32][NS/32], f32 medians) */
+    /* u64 sorted entries + u16 ranks + max(rank bitsets [NW][NS/32+1] + scan offsets [NW/32][NS/32], f32 medians)
+       + u32 sorted keys */
     const size_t bw = (size_t)ns / 32, nw = (size_t)k1_walkers(ns);
     const size_t bits = 4 * (nw * (bw + 1) + (nw / 32) * bw);
     const size_t med = 4 * (size_t)ns;
     /* the MAD variant stages one more fp32 per position (the scale) behind everything else */
-    return (size_t)ns * 10 + (bits > med ? bits : med) + (mad ? 4 * (size_t)ns : 0);
+    return (size_t)ns * 10 + (bits > med ? bits : med) + 4 * (size_t)ns + (mad ? 4 * (size_t)ns : 0);
 }
 
 /* sibling estimators; values match include/umi.h */

@@ -3,9 +3,13 @@
  *
  * CTA = one star x one tile of T consecutive positions.  The T windows of a tile
  * live inside one union of U = T + W - 1 = NS samples (NS a power of two).
- *   1. sort the union ONCE per tile: bitonic network on 64-bit (key << 32 | index)
- *      entries, E = NS/256 per thread -- strides < E in registers, strides < 32 E
- *      with warp shuffles, only the top three strides through shared memory;
+ *   1. sort the 32-bit keys of the union ONCE per tile: bitonic network, E = NS/256 keys per
+ *      thread -- strides < E in registers, strides < 32 E with warp shuffles, only the top three
+ *      strides through shared memory; a compare-exchange is two VIMNMX.  The rank of an entry is
+ *      then the lower bound of its key in the sorted keys (binary search in shared memory) plus
+ *      its turn among the entries with the same key (a shared-memory counter per key value);
+ *      srt[rank] = key << 32 | index and rank[index] are scattered from that.  (Sorting 64-bit
+ *      key|index entries directly cost 4-6 instructions per exchange and two shuffles.)
  *   2. NW "walkers" (one thread each) own T/NW consecutive positions.  A walker's
  *      first window is selected from a bitset of the union ranks it holds; the NW
  *      bitsets are built together as an exclusive-or prefix scan over the entries
@@ -25,24 +29,19 @@ namespace umi {
 namespace {
 
 
-__device__ __forceinline__ uint64_t shfl_xor_u64(uint64_t v, int mask)
+/* 32-bit keys: one compare-exchange is two VIMNMX (the direction is a predicate operand), one exchange
+   with another lane is one shuffle and one VIMNMX.  Equal keys are harmless here: min / max keep the
+   multiset, and the ranks of tied entries are assigned after the sort (see the kernel). */
+__device__ __forceinline__ void cmp_swap(uint32_t& a, uint32_t& b, bool up)
 {
-    const uint32_t lo = __shfl_xor_sync(0xFFFFFFFFu, (uint32_t)v, mask);
-    const uint32_t hi = __shfl_xor_sync(0xFFFFFFFFu, (uint32_t)(v >> 32), mask);
-    return ((uint64_t)hi << 32) | lo;
+    const uint32_t mn = min(a, b), mx = max(a, b);
+    a = up ? mn : mx;
+    b = up ? mx : mn;
 }
 
-__device__ __forceinline__ void cmp_swap(uint64_t& a, uint64_t& b, bool up)
-{
-    const bool sw = (a > b) == up;
-    const uint64_t lo = sw ? b : a, hi = sw ? a : b;
-    a = lo;
-    b = hi;
-}
-
-/* One bitonic stage (merge size K, stride J) on entries i = tid*E + e held in v[e] (blocked). */
+/* One bitonic stage (merge size K, stride J) on keys i = tid*E + e held in v[e] (blocked). */
 template <int E, int K, int J>
-__device__ __forceinline__ void bitonic_stage(uint64_t (&v)[E], uint64_t* srt, int tid)
+__device__ __forceinline__ void bitonic_stage(uint32_t (&v)[E], uint32_t* buf, int tid)
 {
     if constexpr (J < E) {
         /* partner inside the thread */
@@ -61,48 +60,47 @@ __device__ __forceinline__ void bitonic_stage(uint64_t (&v)[E], uint64_t* srt, i
         const bool keep_min = (low == up);
 #pragma unroll
         for (int e = 0; e < E; ++e) {
-            const uint64_t o = shfl_xor_u64(v[e], LM);
-            const bool take = (o < v[e]) == keep_min;               /* entries are unique: o != v[e] */
-            v[e] = take ? o : v[e];
+            const uint32_t o = __shfl_xor_sync(0xFFFFFFFFu, v[e], LM);
+            v[e] = keep_min ? min(v[e], o) : max(v[e], o);
         }
     } else {
         /* partner in another warp: exchange through shared memory */
         __syncthreads();
 #pragma unroll
-        for (int e = 0; e < E; e += 2)
-            *reinterpret_cast<ulonglong2*>(srt + tid * E + e) = make_ulonglong2(v[e], v[e + 1]);
+        for (int e = 0; e < E; e += 4)
+            *reinterpret_cast<uint4*>(buf + tid * E + e) = make_uint4(v[e], v[e + 1], v[e + 2], v[e + 3]);
         __syncthreads();
         const bool up = ((tid * E) & K) == 0;
         const bool low = ((tid * E) & J) == 0;
         const bool keep_min = (low == up);
-        const uint64_t* other = srt + ((tid * E) ^ J);
+        const uint32_t* other = buf + ((tid * E) ^ J);
 #pragma unroll
-        for (int e = 0; e < E; e += 2) {
-            const ulonglong2 o2 = *reinterpret_cast<const ulonglong2*>(other + e);
-            const bool t0 = (o2.x < v[e]) == keep_min;
-            const bool t1 = (o2.y < v[e + 1]) == keep_min;
-            v[e] = t0 ? o2.x : v[e];
-            v[e + 1] = t1 ? o2.y : v[e + 1];
+        for (int e = 0; e < E; e += 4) {
+            const uint4 o4 = *reinterpret_cast<const uint4*>(other + e);
+            v[e] = keep_min ? min(v[e], o4.x) : max(v[e], o4.x);
+            v[e + 1] = keep_min ? min(v[e + 1], o4.y) : max(v[e + 1], o4.y);
+            v[e + 2] = keep_min ? min(v[e + 2], o4.z) : max(v[e + 2], o4.z);
+            v[e + 3] = keep_min ? min(v[e + 3], o4.w) : max(v[e + 3], o4.w);
         }
     }
 }
 
 template <int E, int K, int J>
-__device__ __forceinline__ void bitonic_merge(uint64_t (&v)[E], uint64_t* srt, int tid)
+__device__ __forceinline__ void bitonic_merge(uint32_t (&v)[E], uint32_t* buf, int tid)
 {
     if constexpr (J > 0) {
-        bitonic_stage<E, K, J>(v, srt, tid);
-        bitonic_merge<E, K, J / 2>(v, srt, tid);
+        bitonic_stage<E, K, J>(v, buf, tid);
+        bitonic_merge<E, K, J / 2>(v, buf, tid);
     }
 }
 
-/* Bitonic sort of NS = 256*E entries, ascending. */
+/* Bitonic sort of NS = 256*E keys, ascending. */
 template <int E, int K = 2>
-__device__ __forceinline__ void bitonic_sort_blocked(uint64_t (&v)[E], uint64_t* srt, int tid)
+__device__ __forceinline__ void bitonic_sort_blocked(uint32_t (&v)[E], uint32_t* buf, int tid)
 {
     if constexpr (K <= K1_THREADS * E) {
-        bitonic_merge<E, K, K / 2>(v, srt, tid);
-        bitonic_sort_blocked<E, K * 2>(v, srt, tid);
+        bitonic_merge<E, K, K / 2>(v, buf, tid);
+        bitonic_sort_blocked<E, K * 2>(v, buf, tid);
     }
 }
 
@@ -140,6 +138,7 @@ umi_median_kernel(MedianParams prm)
     uint32_t* bits = reinterpret_cast<uint32_t*>(rank + NS);        /* [NW][BWP] rank bitsets, then ...   */
     uint32_t* boff = bits + NW * BWP;                               /* [NWB][BW] block offsets of the scan */
     float* medbuf = reinterpret_cast<float*>(bits);                 /* ... aliased: [T] medians of the tile */
+    uint32_t* skey = reinterpret_cast<uint32_t*>(smem_raw + k1_smem_bytes(NS, false)) - NS;   /* [NS] sorted keys */
     float* sclbuf = reinterpret_cast<float*>(smem_raw + k1_smem_bytes(NS, false));   /* MAD only: [T] scales */
     __shared__ int s_nvu;
 
@@ -163,8 +162,8 @@ umi_median_kernel(MedianParams prm)
         for (int i = tid; i < NW * BWP + NWB * BW; i += K1_THREADS) bits[i] = 0u;
         __syncthreads();
 
-        /* 1. load E consecutive union entries, sort */
-        uint64_t v[E];
+        /* 1. load E consecutive union entries and sort their 32-bit keys */
+        uint32_t v[E];
         int nvalid = 0;
 #pragma unroll
         for (int e = 0; e < E; ++e) {
@@ -172,20 +171,47 @@ umi_median_kernel(MedianParams prm)
             float x = 0.f;
             const bool ok = load_sample(trow, frow, prm.N, jbase + u, x);
             nvalid += ok ? 1 : 0;
-            v[e] = ((uint64_t)(ok ? float_to_key(x) : KEY_INVALID) << 32) | (uint32_t)u;
+            v[e] = ok ? float_to_key(x) : KEY_INVALID;
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) nvalid += __shfl_xor_sync(0xFFFFFFFFu, nvalid, o);
         if (lane == 0 && nvalid) atomicAdd(&s_nvu, nvalid);
 
-        bitonic_sort_blocked<E>(v, srt, tid);
+        bitonic_sort_blocked<E>(v, reinterpret_cast<uint32_t*>(srt), tid);
 
+#pragma unroll
+        for (int e = 0; e < E; e += 4)
+            *reinterpret_cast<uint4*>(skey + tid * E + e) = make_uint4(v[e], v[e + 1], v[e + 2], v[e + 3]);
+        __syncthreads();                                            /* also: every read of the exchange buffer is done */
+
+        /* rank of every entry = lower bound of its key among the sorted keys + its turn among the entries
+           with that key (a counter per key value, borrowed from the still all-zero bitset area and zeroed
+           again below).  Tied entries carry the same value, so which of them gets which rank changes
+           nothing that is computed from ranks.  Invalid entries get a rank above every valid one. */
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            const int u = tid * E + e;
+            float x = 0.f;
+            const bool ok = load_sample(trow, frow, prm.N, jbase + u, x);   /* the same words again (L1 / L2) */
+            if (ok) {
+                const uint32_t key = float_to_key(x);
+                int pos = 0;
+#pragma unroll
+                for (int step = NS / 2; step > 0; step >>= 1)
+                    pos += (skey[pos + step - 1] < key) ? step : 0;
+                const int r = pos + (int)atomicAdd(&bits[pos], 1u);
+                v[e] = (uint32_t)pos;
+                rank[u] = (uint16_t)r;
+                srt[r] = ((uint64_t)key << 32) | (uint32_t)u;
+            } else {
+                v[e] = 0xFFFFFFFFu;
+                rank[u] = (uint16_t)0xFFFFu;
+            }
+        }
         __syncthreads();
 #pragma unroll
-        for (int e = 0; e < E; e += 2)
-            *reinterpret_cast<ulonglong2*>(srt + tid * E + e) = make_ulonglong2(v[e], v[e + 1]);
-#pragma unroll
-        for (int e = 0; e < E; ++e) rank[(uint32_t)v[e]] = (uint16_t)(tid * E + e);
+        for (int e = 0; e < E; ++e)
+            if (v[e] != 0xFFFFFFFFu) bits[v[e]] = 0u;                  /* the bitset area is all zero again */
         __syncthreads();
         const int nvu = s_nvu;                                      /* valid entries = ranks [0, nvu) */
 
