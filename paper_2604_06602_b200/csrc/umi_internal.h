@@ -8,7 +8,10 @@
 
 namespace umi {
 
-constexpr int K1_THREADS = 256;                  /* median kernel */
+#ifndef UMI_K1_THREADS
+#define UMI_K1_THREADS 256
+#endif
+constexpr int K1_THREADS = UMI_K1_THREADS;       /* median kernel */
 constexpr int K1_MIN_SORT = 1024;                /* smallest per-tile sort length */
 /* walkers per tile of the median kernel and its dynamic shared memory (bytes) */
 __host__ __device__ constexpr int k1_walkers(int ns) { return (131072 / ns) > 32 ? (131072 / ns) : 32; }

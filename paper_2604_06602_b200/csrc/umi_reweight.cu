@@ -27,13 +27,13 @@
 #define UMI_K2_MIN_CTAS 5
 #endif
 #ifndef UMI_K2_MIN_CTAS_POW2
-#define UMI_K2_MIN_CTAS_POW2 8     /* alpha = 2^m builds: one FMA-pipe value fewer is live; 64 registers, 8 CTAs/SM measured best */
+#define UMI_K2_MIN_CTAS_POW2 6     /* alpha = 2^m builds: 78 registers, no spills.  Measured (W = 361 / 2161 / 217, ms): 5 CTAs 7.20 / 48.7 / 8.16, 6 CTAs 7.21 / 49.2 / 8.07, 8 CTAs (64 registers, 8 bytes spilled per thread) 7.18 / 49.0 / 8.02 */
 #endif
 #ifndef UMI_K2_UNROLL
 #define UMI_K2_UNROLL 8
 #endif
 #ifndef UMI_K2_UNROLL_POW2
-#define UMI_K2_UNROLL_POW2 4     /* measured with 8 CTAs/SM: 4 is best across W = 217 / 361 / 2161 (8 wins 0.4 % at 361, loses 5 % at 217) */
+#define UMI_K2_UNROLL_POW2 8
 #endif
 
 namespace umi {
@@ -134,7 +134,7 @@ __device__ __forceinline__ void eval_weight_group(f32x2 x01, f32x2 x23, const f3
    with xor shuffles after every pass.  A CTA then owns K2_TILE / SPLIT positions and a thread's serial
    chain is SPLIT times shorter.  SPLIT = 1 is the throughput configuration.
    APOW >= 0: the launch has alpha = 2^APOW and the interior loop forms alpha*u without a multiply;
-   warps in which -u could overflow take the general loop, which is compiled in beside it. */
+   warps in which -u could overflow run all their groups through the scalar edge loop instead. */
 template <int MODE, int SPLIT, int APOW>
 __global__ void __launch_bounds__(K2_THREADS, (APOW >= 0 && SPLIT == 1) ? UMI_K2_MIN_CTAS_POW2 : UMI_K2_MIN_CTAS)
 umi_reweight_kernel(ReweightParams prm)
@@ -310,9 +310,11 @@ umi_reweight_kernel(ReweightParams prm)
                     cn2[q] = pack2(-c0[q], -c0[q]);
                 }
 #endif
-                /* edge groups: samples that belong to some but not all of the 4 windows */
+                /* edge groups: samples that belong to some but not all of the 4 windows -- and, in the
+                   alpha = 2^m builds, every group of a warp whose -u could overflow (`risky`, never seen on
+                   real data): this scalar loop forms alpha*u by a multiply */
                 for (int g = sl; g < G; g += SPLIT) {
-                    if (g >= g_lo && g <= g_hi) {
+                    if (!(APOW >= 0 && risky) && g >= g_lo && g <= g_hi) {
                         if constexpr (SPLIT == 1) g = g_hi;
                         continue;
                     }
@@ -342,11 +344,13 @@ umi_reweight_kernel(ReweightParams prm)
                     }
                 } else {
 #if UMI_K2_PACKED
-                if (APOW >= 0 && !risky) {
+                if constexpr (APOW >= 0) {
+                    if (!risky) {
 #pragma unroll K2_UNROLL_POW2
-                    for (int g = g_first; g <= g_hi; g += SPLIT) {
-                        const ulonglong2 v2 = reinterpret_cast<const ulonglong2*>(xs4)[g];
-                        eval_weight_group<APOW>(v2.x, v2.y, kn2, cn2, nalpha2, S2, R2);
+                        for (int g = g_first; g <= g_hi; g += SPLIT) {
+                            const ulonglong2 v2 = reinterpret_cast<const ulonglong2*>(xs4)[g];
+                            eval_weight_group<APOW>(v2.x, v2.y, kn2, cn2, nalpha2, S2, R2);
+                        }
                     }
                 } else {
 #pragma unroll K2_UNROLL
