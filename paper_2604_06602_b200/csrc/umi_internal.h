@@ -14,7 +14,10 @@ namespace umi {
 constexpr int K1_THREADS = UMI_K1_THREADS;       /* median kernel */
 constexpr int K1_MIN_SORT = 1024;                /* smallest per-tile sort length */
 /* walkers per tile of the median kernel and its dynamic shared memory (bytes) */
-__host__ __device__ constexpr int k1_walkers(int ns) { return (131072 / ns) > 32 ? (131072 / ns) : 32; }
+#ifndef UMI_K1_WALKER_BUDGET
+#define UMI_K1_WALKER_BUDGET 131072
+#endif
+__host__ __device__ constexpr int k1_walkers(int ns) { return (UMI_K1_WALKER_BUDGET / ns) > 32 ? ((UMI_K1_WALKER_BUDGET / ns) < K1_THREADS ? (UMI_K1_WALKER_BUDGET / ns) : K1_THREADS) : 32; }
 __host__ __device__ constexpr size_t k1_smem_bytes(int ns, bool mad = false)
 {
     /* u64 sorted entries + u16 ranks + max(rank bitsets [NW][NS/32+1] + scan offsets [NW/32][NS/32], f32 medians)
