@@ -40,7 +40,7 @@ Geometry geometry_for(int W)
     while (ns < (W - 1) + (W - 1) / 2) ns <<= 1;
     g.NS = ns;
     g.T1 = ns - (W - 1);
-    g.smem1 = umi::k1_smem_bytes(ns);
+    g.smem1 = umi::k1_smem_bytes(ns, false, g.T1);
     const int h = (W - 1) / 2;
     const int hal = (h + 3) & ~3;
     const int G = (3 + (hal - h) + 2 * h) / 4 + 1;
@@ -77,6 +77,29 @@ int validate(const float* flux, int64_t n_stars, int64_t n_cadences, int W, floa
     return check_window(W);
 }
 
+/* Stream-ordered allocations (the n+ scratch of launch_device, the buffers of the host driver) come from the
+   device's default memory pool.  Its release threshold is 0 by default, i.e. every synchronisation hands the
+   freed memory back to the driver and the next call maps it again (0.1-0.2 ms for 40 MB); raised once per
+   host thread and device to 1 GiB so that repeated calls reuse it. */
+void keep_pool_memory()
+{
+    thread_local int done_for = -1;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return; }
+    if (done_for == dev) return;
+    cudaMemPool_t pool = nullptr;
+    if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+        uint64_t thr = 0;
+        if (cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr) == cudaSuccess &&
+            thr < (1ull << 30)) {
+            thr = 1ull << 30;
+            (void)cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+        }
+    }
+    (void)cudaGetLastError();
+    done_for = dev;
+}
+
 /* Enqueue both kernels for device-resident buffers. */
 int launch_device(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
                   int W, float alpha, float c, int n_iter, int min_valid, float* trend_out,
@@ -86,7 +109,7 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
     if (n_stars == 0 || n_cadences == 0) return UMI_OK;
     Geometry g = geometry_for(W);
     const bool mad = fam.on && fam.scale_kind == umi::SCALE_MAD;
-    if (mad) g.smem1 = umi::k1_smem_bytes(g.NS, true);
+    if (mad) g.smem1 = umi::k1_smem_bytes(g.NS, true, g.T1);
     if (min_valid < 0) min_valid = std::max(1, W / 3);      /* PAPER.md:192 (R4) */
 
     if (W <= umi::KS_MAX_WINDOW) {
@@ -106,6 +129,7 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.c_over_alpha = c / alpha;
         rp.split = 1;
         rp.scale_in = nullptr;
+        rp.nplus = nullptr;
         rp.scale_out = fam.scale_out;
         rp.weight_kind = fam.weight_kind;
         rp.scale_kind = fam.scale_kind;
@@ -118,12 +142,33 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         return UMI_OK;
     }
 
+    /* The paper's path with passes to run: the median kernel also writes n+ (Eq. 1's count, exact on the sorted
+       keys) into a stream-ordered scratch buffer of 2 bytes per cadence, which the reweighting kernel reads
+       instead of counting again.  Allocated and freed in stream order inside this call (default memory pool). */
+    struct StreamScratch {
+        void* p = nullptr;
+        cudaStream_t s = nullptr;
+        ~StreamScratch() { if (p != nullptr) (void)cudaFreeAsync(p, s); }
+    } scratch;
+    scratch.s = stream;
+    uint16_t* nplus = nullptr;
+    /* (not for batches small enough to take the split-window variant: there the call is latency-bound and the
+       allocation would cost as much as the kernels, 45 -> 88 us on config 1) */
+    const int64_t rw_tiles = n_stars * ((n_cadences + umi::K2_TILE - 1) / umi::K2_TILE);
+    if (!fam.on && n_iter > 0 && rw_tiles > 4 * 148) {
+        keep_pool_memory();
+        if (cuda_failed(cudaMallocAsync(&scratch.p, (size_t)n_stars * (size_t)n_cadences * sizeof(uint16_t), stream)))
+            return UMI_ERR_CUDA;
+        nplus = static_cast<uint16_t*>(scratch.p);
+    }
+
     umi::MedianParams mp;
     mp.time = time;
     mp.flux = flux;
     mp.out = trend_out;
     mp.flat = (n_iter == 0) ? flat_out : nullptr;
     mp.scale = mad ? fam.scale_out : nullptr;
+    mp.nplus = nplus;
     mp.N = n_cadences;
     mp.tiles_per_star = (n_cadences + g.T1 - 1) / g.T1;
     mp.n_blocks = n_stars * mp.tiles_per_star;
@@ -163,6 +208,7 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.c = c;
         rp.c_over_alpha = c / alpha;
         rp.scale_in = mad ? fam.scale_out : nullptr;
+        rp.nplus = nplus;
         rp.scale_out = mad ? nullptr : fam.scale_out;
         rp.weight_kind = fam.weight_kind;
         rp.scale_kind = fam.scale_kind;
@@ -401,20 +447,7 @@ int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t 
         double* d_time = nullptr;
     };
     std::vector<Slot> slots((size_t)n_streams);
-    {
-        /* keep the per-call buffers in the driver's stream-ordered pool between calls (up to 1 GiB) */
-        int dev = 0;
-        cudaMemPool_t pool = nullptr;
-        if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-            uint64_t thr = 0;
-            if (cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr) == cudaSuccess &&
-                thr < (1ull << 30)) {
-                thr = 1ull << 30;
-                (void)cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
-            }
-        }
-        (void)cudaGetLastError();
-    }
+    keep_pool_memory();     /* the per-call buffers stay in the driver's stream-ordered pool between calls */
     const size_t elems = (size_t)stars_per_batch * (size_t)n_cadences;
     int status = UMI_OK;
 

@@ -18,13 +18,15 @@ constexpr int K1_MIN_SORT = 1024;                /* smallest per-tile sort lengt
 #define UMI_K1_WALKER_BUDGET 131072
 #endif
 __host__ __device__ constexpr int k1_walkers(int ns) { return (UMI_K1_WALKER_BUDGET / ns) > 32 ? ((UMI_K1_WALKER_BUDGET / ns) < K1_THREADS ? (UMI_K1_WALKER_BUDGET / ns) : K1_THREADS) : 32; }
-__host__ __device__ constexpr size_t k1_smem_bytes(int ns, bool mad = false)
+/* t = positions per tile (T = ns - W + 1; 0: the worst case ns) */
+__host__ __device__ constexpr size_t k1_smem_bytes(int ns, bool mad = false, int t = 0)
 {
     /* u64 sorted entries + u16 ranks + max(rank bitsets [NW][NS/32+1] + scan offsets [NW/32][NS/32], f32 medians)
        + u32 sorted keys */
     const size_t bw = (size_t)ns / 32, nw = (size_t)k1_walkers(ns);
     const size_t bits = 4 * (nw * (bw + 1) + (nw / 32) * bw);
-    const size_t med = 4 * (size_t)ns;
+    /* f32 medians [T], then u16 median ranks [T] and u16 window counts [T] (for n+), rounded to 16 bytes */
+    const size_t med = ((8 * (size_t)(t > 0 ? t : ns)) + 15) / 16 * 16;
     /* the MAD variant stages one more fp32 per position (the scale) behind everything else */
     return (size_t)ns * 10 + (bits > med ? bits : med) + 4 * (size_t)ns + (mad ? 4 * (size_t)ns : 0);
 }
@@ -51,6 +53,7 @@ struct MedianParams {
     float* out;              /* median, NaN where the position has no trend */
     float* flat;             /* null, or flux / median (only set when the call stops after Phase 1) */
     float* scale;            /* null, or MAD of the window (selects the MAD variant of the kernel) */
+    uint16_t* nplus;         /* null, or n+ = number of window samples strictly above the median (Eq. 1, R7) */
     int64_t N;               /* cadences per star */
     int64_t tiles_per_star;
     int64_t n_blocks;        /* n_stars * tiles_per_star */
@@ -64,6 +67,7 @@ struct ReweightParams {
     float* flat;             /* null, or flux / trend (PAPER.md:155 normalisation), NaN where trend is NaN */
     const float* scale_in;   /* family kernels: null, or s per position (replaces Phase 2) */
     float* scale_out;        /* family kernels: null, or receives s per position */
+    const uint16_t* nplus;   /* null, or n+ per position from the median kernel: Phase 2 then only sums squares */
     int split;               /* reweighting kernel: 1, or K2_SPLIT for batches too small to fill the GPU */
     int weight_kind;         /* family kernels: WEIGHT_BISQUARE / WEIGHT_WELSCH */
     int scale_kind;          /* fused short-window kernel only */

@@ -138,8 +138,10 @@ umi_median_kernel(MedianParams prm)
     uint32_t* bits = reinterpret_cast<uint32_t*>(rank + NS);        /* [NW][BWP] rank bitsets, then ...   */
     uint32_t* boff = bits + NW * BWP;                               /* [NWB][BW] block offsets of the scan */
     float* medbuf = reinterpret_cast<float*>(bits);                 /* ... aliased: [T] medians of the tile */
-    uint32_t* skey = reinterpret_cast<uint32_t*>(smem_raw + k1_smem_bytes(NS, false)) - NS;   /* [NS] sorted keys */
-    float* sclbuf = reinterpret_cast<float*>(smem_raw + k1_smem_bytes(NS, false));   /* MAD only: [T] scales */
+    uint16_t* rhobuf = reinterpret_cast<uint16_t*>(medbuf + prm.T); /* ... [T] median ranks and [T] window counts behind them */
+    uint16_t* cntbuf = rhobuf + prm.T;
+    uint32_t* skey = reinterpret_cast<uint32_t*>(smem_raw + k1_smem_bytes(NS, false, prm.T)) - NS;   /* [NS] sorted keys */
+    float* sclbuf = reinterpret_cast<float*>(smem_raw + k1_smem_bytes(NS, false, prm.T));   /* MAD only: [T] scales */
     __shared__ int s_nvu;
 
     const int W = prm.W;
@@ -383,6 +385,10 @@ umi_median_kernel(MedianParams prm)
                 float m = __int_as_float(0x7FC00000);
                 if (has) m = key_to_float((uint32_t)(srt[rho] >> 32));
                 medbuf[p] = m;
+                if (prm.nplus != nullptr) {                         /* for n+, counted after the walk */
+                    rhobuf[p] = has ? (uint16_t)rho : (uint16_t)0xFFFFu;
+                    cntbuf[p] = (uint16_t)n;
+                }
                 if constexpr (MAD) sclbuf[p] = has ? mad : __int_as_float(0x7FC00000);
                 if (++p >= pend) break;
                 /* slide to window p: union index p-1 leaves, p+W-1 enters */
@@ -441,6 +447,23 @@ umi_median_kernel(MedianParams prm)
 
         float* orow = prm.out + star * prm.N + j0;
         for (int p = tid; p < Tact; p += K1_THREADS) orow[p] = medbuf[p];
+        if (prm.nplus != nullptr) {
+            /* n+ of Eq. 1 (R7), all threads, off the walkers' serial chain: the n - 1 - (n-1)/2 members above
+               the median in rank, less those that tie with it in value (they follow it directly in sorted order) */
+            uint16_t* nrow = prm.nplus + star * prm.N + j0;
+            for (int p = tid; p < Tact; p += K1_THREADS) {
+                const int rho = rhobuf[p];
+                int np = 0;
+                if (rho != 0xFFFF) {
+                    const int n = cntbuf[p];
+                    const uint32_t kmed = (uint32_t)(srt[rho] >> 32);
+                    np = n - 1 - ((n - 1) >> 1);
+                    for (int r = rho + 1; r < nvu && (uint32_t)(srt[r] >> 32) == kmed; ++r)
+                        np -= (((uint32_t)srt[r] - (uint32_t)p) < (uint32_t)W) ? 1 : 0;
+                }
+                nrow[p] = (uint16_t)np;
+            }
+        }
         if constexpr (MAD) {
             float* srow = prm.scale + star * prm.N + j0;
             for (int p = tid; p < Tact; p += K1_THREADS) srow[p] = sclbuf[p];

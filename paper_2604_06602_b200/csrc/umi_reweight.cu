@@ -212,6 +212,7 @@ umi_reweight_kernel(ReweightParams prm)
 
         /* per-position state: 4 consecutive positions, local index 4*tid + q */
         float mu[K2_NPOS], kk[K2_NPOS], cs[K2_NPOS];
+        float nplus[K2_NPOS] = {0.f, 0.f, 0.f, 0.f};      /* n+ from the median kernel, when it was asked for one */
         bool act[K2_NPOS];
         bool any_act = false;
         unsigned has_med = 0u;                              /* bit q: position q has a median, i.e. a trend */
@@ -223,6 +224,9 @@ umi_reweight_kernel(ReweightParams prm)
             has_med |= act[q] ? (1u << q) : 0u;
             any_act = any_act || act[q];
             mu[q] = act[q] ? med : 0.f;
+            if constexpr (MODE == 0) {
+                if (prm.nplus != nullptr) nplus[q] = (act[q] && jl < nrow) ? (float)prm.nplus[star * prm.N + j0 + jl] : 0.f;
+            }
             kk[q] = 0.f;
             cs[q] = 0.f;
             if constexpr (MODE != 0) {                              /* no trend, no scale */
@@ -238,7 +242,12 @@ umi_reweight_kernel(ReweightParams prm)
 #pragma unroll
             for (int q = 0; q < K2_NPOS; ++q) { ss[q] = 0.f; cnt[q] = 0.f; }
             const bool given = (MODE != 0) && prm.scale_in != nullptr;
+            const bool counted = (MODE == 0) && UMI_K2_PACKED && prm.nplus != nullptr;   /* n+ already known */
             for (int g = sl; g < (given ? 0 : G); g += SPLIT) {
+                if (counted && g >= g_lo && g <= g_hi) {            /* interior groups: packed loop below */
+                    if constexpr (SPLIT == 1) g = g_hi;
+                    continue;
+                }
                 const float4 v = xs4[g];
                 const float xv[4] = {v.x, v.y, v.z, v.w};
                 if (g >= g_lo && g <= g_hi) {
@@ -256,6 +265,39 @@ umi_reweight_kernel(ReweightParams prm)
                         }
                 }
             }
+#if UMI_K2_PACKED
+            if (counted) {
+                /* With n+ known (the median kernel counts it exactly, on the sorted keys), Eq. 1 is a sum of
+                   squares only: d = x - med on sample pairs (FADD2), max(d, 0) as a signed-integer maximum on
+                   the ALU pipe, ss += d*d (FFMA2).  Two FMA-pipe lane-operations and one ALU instruction per
+                   sample instead of three and one. */
+                f32x2 nmed2[K2_NPOS], ss2[K2_NPOS];
+#pragma unroll
+                for (int q = 0; q < K2_NPOS; ++q) { nmed2[q] = pack2(-mu[q], -mu[q]); ss2[q] = pack2(0.f, 0.f); }
+#pragma unroll 8
+                for (int g = g_first; g <= g_hi; g += SPLIT) {
+                    const ulonglong2 v2 = reinterpret_cast<const ulonglong2*>(xs4)[g];
+#pragma unroll
+                    for (int q = 0; q < K2_NPOS; ++q) {
+#pragma unroll
+                        for (int hh = 0; hh < 2; ++hh) {
+                            const f32x2 d2 = fadd2(hh ? v2.y : v2.x, nmed2[q]);
+                            float d0, d1;
+                            unpack2(d2, d0, d1);
+                            const f32x2 p2 = pack2(__int_as_float(max(__float_as_int(d0), 0)),
+                                                   __int_as_float(max(__float_as_int(d1), 0)));
+                            ss2[q] = ffma2(p2, p2, ss2[q]);
+                        }
+                    }
+                }
+#pragma unroll
+                for (int q = 0; q < K2_NPOS; ++q) {
+                    float s0, s1;
+                    unpack2(ss2[q], s0, s1);
+                    ss[q] += s0 + s1;
+                }
+            }
+#endif
             if constexpr (SPLIT > 1) {
 #pragma unroll
                 for (int q = 0; q < K2_NPOS; ++q)
@@ -264,6 +306,10 @@ umi_reweight_kernel(ReweightParams prm)
                         ss[q] += __shfl_xor_sync(0xFFFFFFFFu, ss[q], o);
                         cnt[q] += __shfl_xor_sync(0xFFFFFFFFu, cnt[q], o);
                     }
+            }
+            if (counted) {
+#pragma unroll
+                for (int q = 0; q < K2_NPOS; ++q) cnt[q] = nplus[q];
             }
 #pragma unroll
             for (int q = 0; q < K2_NPOS; ++q) {
