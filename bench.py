@@ -308,10 +308,10 @@ def run_ours(args, cfg, rank, world, local_rank):
         "traffic": ncu_traffic(args.config, S),
     }
     # What the kernel executes, as opposed to the 49 operations the method is charged with above: FMA-pipe
-    # lane-operations per window-sample as built (Phase 2: 3; a pass: 5 when alpha is 1, 2 or 4 -- alpha*u is an
+    # lane-operations per window-sample as built (Phase 2: 2 with n+ from the median kernel; a pass: 5 when alpha is 1, 2 or 4 -- alpha*u is an
     # integer add on the ALU pipe -- else 6) against the FMA pipe's 128 lanes/clk/SM.  ncu's
     # sm__pipe_fma_cycles_active for the same launch is in profiles/ncu_full_r01.csv.
-    fma_ops = 3 + (5 if cfg.alpha in (1.0, 2.0, 4.0) and W > 49 else 6) * cfg.n_iter
+    fma_ops = (2 if W > 49 else 3) + (5 if cfg.alpha in (1.0, 2.0, 4.0) and W > 49 else 6) * cfg.n_iter
     roofline["executed"] = {"fma_pipe_lane_ops_per_window_sample": fma_ops,
                             "fma_pipe_frac": fma_ops * ws_exact / (rw_ms * 1e-3) / 1e12 / peak,
                             "peak_def": "148 SMs x 128 FP32 lanes x sm_max_mhz"}

@@ -15,10 +15,13 @@
  *  - Every entry point returns a umi_status (int); nothing throws or aborts
  *    across this boundary.  Arguments are validated on the host before any
  *    work is enqueued.
- *  - No torch types, no hidden allocation that outlives a call, no mutable
- *    global state: the library is re-entrant.  (One exception, which holds no
+ *  - No torch types, no hidden allocation that outlives a call (device
+ *    scratch, where a call needs any, is stream-ordered: cudaMallocAsync /
+ *    cudaFreeAsync on the caller's stream, see umi_detrend), no mutable
+ *    global state: the library is re-entrant.  (Two exceptions, which hold no
  *    memory and no data: the host batch driver keeps its CUDA streams per host
- *    thread between calls, see umi_detrend_host.)
+ *    thread between calls, see umi_detrend_host; and the release threshold of
+ *    the device's default memory pool is raised to 1 GiB.)
  *  - "DEVICE pointer": memory of the current CUDA device, readable/writable by
  *    kernels launched on `stream`.  "HOST pointer": ordinary host memory
  *    (pinned memory makes the copies asynchronous and faster, but is not
@@ -83,6 +86,15 @@ int umi_window_len(double dt_days);
  *   stream    cudaStream_t (as void*), or NULL for the legacy default stream.
  *             Work is enqueued; the call does not synchronise.  The caller
  *             keeps all three buffers alive until the stream has drained.
+ *
+ * Scratch: when W > 49, n_iter > 0 and the batch holds more than 592 tiles of
+ * 512 positions, the call takes 2 bytes per cadence from the device's default
+ * memory pool with cudaMallocAsync on `stream` (the count n+ of Eq. 1, which
+ * the first kernel hands to the second) and returns them with cudaFreeAsync
+ * on `stream` before it returns; the pool's release threshold is raised to
+ * 1 GiB (once per host thread) so that repeated calls reuse the memory.
+ * Nothing allocated by the library outlives the work enqueued by the call.
+ * A failed allocation -> UMI_ERR_CUDA, nothing enqueued.
  *
  * c is fixed at 5.0.  Errors: see umi_status.
  */
