@@ -490,7 +490,7 @@ cudaError_t launch_median(const MedianParams& prm, unsigned grid, size_t smem, c
     case 32: k1 = mad ? umi_median_kernel<32, true> : umi_median_kernel<32, false>; break;
     default: return cudaErrorInvalidValue;
     }
-    if (smem > 48 * 1024) {
+    if (smem + 1024 > 48 * 1024) {        /* static shared memory counts towards the 48 KiB default limit too */
         const cudaError_t e = cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
