@@ -104,7 +104,8 @@ void keep_pool_memory()
 int launch_device(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
                   int W, float alpha, float c, int n_iter, int min_valid, float* trend_out,
                   cudaStream_t stream, cudaEvent_t* ev = nullptr /* [3] or null */,
-                  float* flat_out = nullptr, const Family& fam = Family())
+                  float* flat_out = nullptr, const Family& fam = Family(),
+                  uint16_t* nplus_scratch = nullptr /* [n_stars*n_cadences], or null: allocated here when needed */)
 {
     if (n_stars == 0 || n_cadences == 0) return UMI_OK;
     Geometry g = geometry_for(W);
@@ -155,7 +156,9 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
     /* (not for batches small enough to take the split-window variant: there the call is latency-bound and the
        allocation would cost as much as the kernels, 45 -> 88 us on config 1) */
     const int64_t rw_tiles = n_stars * ((n_cadences + umi::K2_TILE - 1) / umi::K2_TILE);
-    if (!fam.on && n_iter > 0 && rw_tiles > 4 * 148) {
+    if (!fam.on && n_iter > 0 && rw_tiles > 4 * 148 && nplus_scratch != nullptr) {
+        nplus = nplus_scratch;
+    } else if (!fam.on && n_iter > 0 && rw_tiles > 4 * 148) {
         keep_pool_memory();
         if (cuda_failed(cudaMallocAsync(&scratch.p, (size_t)n_stars * (size_t)n_cadences * sizeof(uint16_t), stream)))
             return UMI_ERR_CUDA;
@@ -445,6 +448,8 @@ int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t 
         float* d_trend = nullptr;
         float* d_flat = nullptr;
         double* d_time = nullptr;
+        uint16_t* d_nplus = nullptr;   /* the n+ scratch of launch_device, per slot: an allocation inside every batch would
+                                          make the pool hand memory from one stream to another and serialise them */
     };
     std::vector<Slot> slots((size_t)n_streams);
     keep_pool_memory();     /* the per-call buffers stay in the driver's stream-ordered pool between calls */
@@ -459,7 +464,9 @@ int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t 
             cuda_failed(cudaMallocAsync((void**)&s.d_flux, elems * sizeof(float), s.stream)) ||
             cuda_failed(cudaMallocAsync((void**)&s.d_trend, elems * sizeof(float), s.stream)) ||
             (flat_out != nullptr && cuda_failed(cudaMallocAsync((void**)&s.d_flat, elems * sizeof(float), s.stream))) ||
-            (time != nullptr && cuda_failed(cudaMallocAsync((void**)&s.d_time, elems * sizeof(double), s.stream)))) {
+            (time != nullptr && cuda_failed(cudaMallocAsync((void**)&s.d_time, elems * sizeof(double), s.stream))) ||
+            (W > umi::KS_MAX_WINDOW && n_iter > 0 &&
+             cuda_failed(cudaMallocAsync((void**)&s.d_nplus, elems * sizeof(uint16_t), s.stream)))) {
             status = UMI_ERR_CUDA;
             break;
         }
@@ -479,7 +486,7 @@ int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t 
             break;
         }
         status = launch_device(s.d_time, s.d_flux, ns, n_cadences, W, alpha, c, n_iter, min_valid, s.d_trend, s.stream,
-                               nullptr, s.d_flat);
+                               nullptr, s.d_flat, Family(), s.d_nplus);
         if (status != UMI_OK) break;
         if ((trend_out != nullptr &&
              cuda_failed(cudaMemcpyAsync(trend_out + off, s.d_trend, cnt * sizeof(float), cudaMemcpyDeviceToHost, s.stream))) ||
@@ -494,6 +501,7 @@ int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t 
         if (s.d_trend) (void)cudaFreeAsync(s.d_trend, s.stream);
         if (s.d_flat) (void)cudaFreeAsync(s.d_flat, s.stream);
         if (s.d_time) (void)cudaFreeAsync(s.d_time, s.stream);
+        if (s.d_nplus) (void)cudaFreeAsync(s.d_nplus, s.stream);
         if (cuda_failed(cudaStreamSynchronize(s.stream))) status = UMI_ERR_CUDA;
     }
     (void)cudaGetLastError();

@@ -118,7 +118,7 @@ struct MadRange {
 };
 
 template <int E, bool MAD>
-__global__ void __launch_bounds__(K1_THREADS)
+__global__ void __launch_bounds__(K1_THREADS, E == 4 ? 6 : 1)   /* NS = 1024: 6 CTAs/SM fit in shared memory, keep the registers at 40 */
 umi_median_kernel(MedianParams prm)
 {
     constexpr int NS = K1_THREADS * E;
@@ -385,7 +385,7 @@ umi_median_kernel(MedianParams prm)
                 float m = __int_as_float(0x7FC00000);
                 if (has) m = key_to_float((uint32_t)(srt[rho] >> 32));
                 medbuf[p] = m;
-                if (prm.nplus != nullptr) {                         /* for n+, counted after the walk */
+                if (!MAD && prm.nplus != nullptr) {                 /* for n+, counted after the walk (never asked of the MAD build) */
                     rhobuf[p] = has ? (uint16_t)rho : (uint16_t)0xFFFFu;
                     cntbuf[p] = (uint16_t)n;
                 }
@@ -447,7 +447,7 @@ umi_median_kernel(MedianParams prm)
 
         float* orow = prm.out + star * prm.N + j0;
         for (int p = tid; p < Tact; p += K1_THREADS) orow[p] = medbuf[p];
-        if (prm.nplus != nullptr) {
+        if (!MAD && prm.nplus != nullptr) {
             /* n+ of Eq. 1 (R7), all threads, off the walkers' serial chain: the n - 1 - (n-1)/2 members above
                the median in rank, less those that tie with it in value (they follow it directly in sorted order) */
             uint16_t* nrow = prm.nplus + star * prm.N + j0;
