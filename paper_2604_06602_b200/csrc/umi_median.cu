@@ -118,7 +118,7 @@ struct MadRange {
 };
 
 template <int E, bool MAD>
-__global__ void __launch_bounds__(K1_THREADS, E == 4 ? 6 : 1)   /* NS = 1024: 6 CTAs/SM fit in shared memory, keep the registers at 40 */
+__global__ void __launch_bounds__(K1_THREADS, E == 4 ? 6 : 0)   /* NS = 1024: 6 CTAs/SM fit in shared memory, keep the registers at 40 */
 umi_median_kernel(MedianParams prm)
 {
     constexpr int NS = K1_THREADS * E;
