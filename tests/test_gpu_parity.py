@@ -61,6 +61,18 @@ def test_heavy_ties(umi, W):
     _both(umi, x, W)
 
 
+@pytest.mark.parametrize("W", [51, 361])
+def test_heavy_ties_in_a_large_batch(umi, W):
+    # more than 592 reweighting tiles: the median kernel hands n+ (Eq. 1's count of samples STRICTLY above
+    # the median, R7) to the reweighting kernel; with flux quantised to a handful of levels most windows
+    # have members that tie with the median, above and below it in rank, and a miscounted tie changes s
+    x = lc.random_series(1500 + W, 160, 2100, nan_frac=0.02, inf_frac=0.0, ties=True)
+    _both(umi, x, W)
+    x = lc.random_series(1600 + W, 160, 2100, nan_frac=0.0, inf_frac=0.0, ties=True)
+    x[:, ::2] = 1.0                                     # half of every window sits exactly on one value
+    _both(umi, x, W)
+
+
 @pytest.mark.parametrize("N", [1, 2, 3, 4, 5, 31, 32, 33, 511, 512, 513, 663, 664, 665, 1327, 1329])
 def test_ragged_lengths(umi, N):
     x = lc.random_series(N, 2, N, nan_frac=0.03 if N > 8 else 0.0, inf_frac=0.0)
