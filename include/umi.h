@@ -175,7 +175,8 @@ int umi_detrend_family(const double* time, const float* flux,
  *   flat_out   DEVICE, float [n_stars*n_samples] or NULL: flux / trend.
  *   workspace  DEVICE, at least umi_gapped_workspace_bytes(n_stars, n_grid) bytes, owned by
  *              the caller, free to reuse once the stream has passed the call; too small or
- *              NULL -> UMI_ERR_INVALID_ARG.  The library allocates nothing.
+ *              NULL -> UMI_ERR_INVALID_ARG.  It holds the two fp32 slot grids and the hot path's
+ *              n+ scratch (10 bytes per slot): this entry point allocates nothing.
  * Enqueues on `stream`; does not synchronise.
  */
 size_t umi_gapped_workspace_bytes(int64_t n_stars, int64_t n_grid);

@@ -292,7 +292,8 @@ int umi_detrend_family(const double* time, const float* flux, int64_t n_stars, i
 size_t umi_gapped_workspace_bytes(int64_t n_stars, int64_t n_grid)
 {
     if (n_stars <= 0 || n_grid <= 0) return 0;
-    return (size_t)2 * (size_t)n_stars * (size_t)n_grid * sizeof(float);
+    /* two fp32 grids (flux, trend) and the uint16 n+ scratch of the hot path */
+    return (size_t)n_stars * (size_t)n_grid * (2 * sizeof(float) + sizeof(uint16_t));
 }
 
 int umi_detrend_gapped(const double* time, const float* flux, int64_t n_stars, int64_t n_samples,
@@ -323,8 +324,9 @@ int umi_detrend_gapped(const double* time, const float* flux, int64_t n_stars, i
         if (cuda_failed(cudaMemsetAsync(grid_flux, 0xFF, (size_t)n_stars * (size_t)n_grid * sizeof(float), s)))
             return UMI_ERR_CUDA;
         if (cuda_failed(umi::launch_regrid_scatter(gp, grid_flux, s))) return UMI_ERR_CUDA;
+        uint16_t* grid_nplus = reinterpret_cast<uint16_t*>(grid_trend + (size_t)n_stars * (size_t)n_grid);
         const int st2 = launch_device(nullptr, grid_flux, n_stars, n_grid, W, alpha, c, n_iter, min_valid,
-                                      grid_trend, s);
+                                      grid_trend, s, nullptr, nullptr, Family(), grid_nplus);
         if (st2 != UMI_OK) return st2;
     }
     if (cuda_failed(umi::launch_regrid_gather(gp, grid_trend, trend_out, flat_out, s))) return UMI_ERR_CUDA;
