@@ -9,13 +9,15 @@
  * sentinel far below the tile minimum, which Eq. 1 never counts and Eq. 3 always
  * gives weight 0, so the inner loop carries no validity predicate.
  *
- * Inner loop ("Reweighting kernel"): per (sample, position)
- *     u  = x*k + c0                 k = 1/(c s), c0 = -mu*k
- *     e  = max(u, -alpha*u)         = |u_eff| of Eq. 2 for any alpha > 0
- *     t  = sat(1 - e*e)             Eq. 3 (R12): 0 outside the cut-off
- *     w  = t*t;  S += w;  R += w*u  Eq. 4 in centred form: mu <- mu + c s R/S
- * With UMI_K2_PACKED the fma/mul/add steps run as sm_100a packed fp32x2
- * instructions (FFMA2/FMUL2/FADD2) on two consecutive samples at a time.
+ * Inner loop: per (sample, position), on u' = -u
+ *     u' = x*(-k) + mu*k            k = 1/(c s)
+ *     -e = min(u', alpha*u, -1.0f)  as signed integers: -min(|u_eff|, 1), Eq. 2's case split and
+ *                                   Eq. 3's cut-off (R12) in one DPX instruction; for alpha = 2^m
+ *                                   alpha*u is an integer add on the bits of u' (no multiply)
+ *     n  = e*e - 1  (<= 0);  w = n*n;  S += w;  R += w*x'            Eq. 4: mu' <- R/S
+ * The fma/mul/add steps run as sm_100a packed fp32x2 instructions (FFMA2/FMUL2/FADD2) on two
+ * consecutive samples at a time; the edge groups use the scalar float form of the same arithmetic.
+ * Phase 2 takes n+ from the median kernel when the launch provides it and then only sums squares.
  * Nothing here is shared with oracle/.
  */
 #include "umi_device.cuh"
