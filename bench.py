@@ -31,13 +31,31 @@ from workloads import lightcurves as lc  # noqa: E402
 METRIC = "detrended cadences/sec on 1 B200 (TESS W=361 batch) + fraction of roofline"
 UNIT = "cadences/s"
 
-# DESIGN.md, "Roofline": algorithmic lane-operations per window-sample
-#   Phase 2: 4 (sub, compare, predicated fma, count); Phase 3: 9 per pass
-#   (sub, setp, sel, mul, fma, max, mul, add, fma)  -> 4 + 9 * n_iter = 49 at n_iter = 5.
-OPS_PHASE2 = 4
-OPS_PER_PASS = 9
+# DESIGN.md section 6, "Roofline".  The path is bound by the FMA pipe (148 SMs x 128 FP32 lanes, one lane-operation
+# per lane per clock; a packed FFMA2/FMUL2/FADD2 is two lane-operations).  FMA-pipe lane-operations per
+# window-sample the kernels EXECUTE (counted in the SASS of the inner loops, cross-checked against ncu's
+# sm__pipe_fma_cycles_active in profiles/):
+#   reweighting kernel (W > 49): Phase 2 = 2 (x - med, ss += d*d; n+ comes with the median); a pass = 5 when alpha
+#     is 1, 2 or 4 (u' = x(-k) + mu k; n = e*e - 1; w = n*n; S += w; R += w x -- alpha*u is an integer add on the
+#     ALU pipe), 6 for any other alpha (one more multiply)
+#   fused short-window kernel (W <= 49): see FMA_OPS_SMALL below
+# Beside it, as labelled side figures only: the survey's algorithmic FMA-pipe count (2 + 6 per pass) and its
+# nominal 49 issue slots per window-sample (4 + 9 per pass), which packed fp32x2 and DPX instructions beat, so
+# that figure is not a fraction of any hardware ceiling.
 SM_COUNT = 148
-LANES_PER_SM = 128          # 4 schedulers x 32 lanes, one warp instruction per clock each
+LANES_PER_SM = 128          # FP32 lanes of the FMA pipe per SM (4 SMSPs x 32)
+FMA_OPS_SMALL = (3, 6)      # fused short-window kernel: Phase 2 (sub, fma, count), a pass (general-alpha form)
+NOMINAL_PHASE2, NOMINAL_PER_PASS = 4, 9
+SURVEY_FMA_PHASE2, SURVEY_FMA_PER_PASS = 2, 6
+
+
+def fma_ops_per_window_sample(W, alpha, n_iter):
+    """(executed FMA-pipe lane-operations per window-sample, description) for the kernel that runs this W."""
+    if W <= 49:
+        p2, pp = FMA_OPS_SMALL
+        return p2 + pp * n_iter, "%d (Phase 2) + %d x %d passes, fused short-window kernel" % (p2, pp, n_iter)
+    pp = 5 if alpha in (1.0, 2.0, 4.0) else 6
+    return 2 + pp * n_iter, "2 (Phase 2) + %d x %d passes, alpha %s" % (pp, n_iter, "= 2^m: integer-add form" if pp == 5 else "general")
 
 
 def parse_args():
@@ -148,16 +166,23 @@ def peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback"
 
 
-def ncu_traffic(config_id, n_stars):
-    """dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the
-    committed ncu --set full capture (profiles/traffic_r01.json); None for any other workload."""
-    path = os.path.join(ROOT, "profiles", "traffic_r01.json")
-    if config_id != 2 or n_stars != 1000 or not os.path.exists(path):
+def ncu_record(config_id, n_stars, kernel_prefix):
+    """Counters of the dominant kernel for THIS workload from the committed ncu --set full capture
+    (profiles/ncu_r02.json, written from the .ncu-rep by hand; the commands are in profiles/README.md):
+    dram bytes per launch, FMA-pipe utilisation, executed warp instructions.  None if no capture of this
+    configuration at this size is committed."""
+    path = os.path.join(ROOT, "profiles", "ncu_r02.json")
+    if not os.path.exists(path):
         return None
     with open(path) as f:
-        kernels = json.load(f)["kernels"]
-    k = next((v for n, v in kernels.items() if n.startswith("umi_reweight_kernel<0, 1") and "config2" in n), None)
-    return None if k is None else k["dram_bytes_read"] + k["dram_bytes_write"]
+        rec = json.load(f)
+    cfgrec = rec.get("config%d" % config_id)
+    if not cfgrec or cfgrec.get("n_stars") != n_stars:
+        return None
+    for name, v in cfgrec.get("kernels", {}).items():
+        if name.startswith(kernel_prefix):
+            return dict(v, kernel=name)
+    return None
 
 
 def oracle_sample(cfg, flux, n_stars):
@@ -290,33 +315,36 @@ def run_ours(args, cfg, rank, world, local_rank):
     value = world * S * N / (ms_per_step * 1e-3)
     med_ms = float(np.mean([a for a, _ in k_ms]))
     rw_ms = float(np.mean([b for _, b in k_ms]))
-    ops_per_ws = OPS_PHASE2 + OPS_PER_PASS * cfg.n_iter
     sm_max = float(clocks["sm_max_mhz"] or pk.get("sm_max_mhz", 1965.0))
     sm_now = float(clocks["sm_mhz"] or sm_max)
-    peak = SM_COUNT * LANES_PER_SM * sm_max * 1e6 / 1e12                 # Tlane-op/s at max clock
-    achieved = ops_per_ws * ws_exact / (rw_ms * 1e-3) / 1e12
+    peak = SM_COUNT * LANES_PER_SM * sm_max * 1e6 / 1e12                 # T FMA-pipe lane-op/s at max clock
+    fma_ops, fma_def = fma_ops_per_window_sample(W, cfg.alpha, cfg.n_iter)
+    kname = "umi_small_kernel" if W <= 49 else "umi_reweight_kernel"
+    achieved = fma_ops * ws_exact / (rw_ms * 1e-3) / 1e12
+    ncu = ncu_record(args.config, S, kname)
+    nominal = NOMINAL_PHASE2 + NOMINAL_PER_PASS * cfg.n_iter
+    survey_fma = SURVEY_FMA_PHASE2 + SURVEY_FMA_PER_PASS * cfg.n_iter
     roofline = {
-        "bound": "alu", "kernel": "umi_reweight_kernel",
-        "achieved": achieved, "peak": peak, "unit": "Tlane-op/s", "frac": achieved / peak,
-        "peak_def": "148 SMs x 4 schedulers x 32 lanes x 1 warp-instr/clk x sm_max_mhz (%s clocks)" % pk_kind,
+        "bound": "alu", "pipe": "fma", "kernel": kname + (" (fused phases 1-3)" if W <= 49 else ""),
+        "achieved": achieved, "peak": peak, "unit": "T FMA-pipe lane-op/s", "frac": achieved / peak,
+        "peak_def": "148 SMs x 128 FP32 lanes x sm_max_mhz (%s clocks); achieved = executed FMA-pipe lane-ops per "
+                    "window-sample [%s] x exact window-samples / kernel time" % (pk_kind, fma_def),
         "frac_at_measured_clock": achieved / (peak * sm_now / sm_max),
-        "ops_per_window_sample": ops_per_ws, "window_samples_per_launch": ws_exact,
-        "window_samples_nominal": S * N * W,
+        "fma_pipe_lane_ops_per_window_sample": fma_ops,
+        "window_samples_per_launch": ws_exact, "window_samples_nominal": S * N * W,
         "kernel_ms": rw_ms, "median_kernel_ms": med_ms, "kernel_share_of_step": rw_ms / (rw_ms + med_ms),
         "window_samples_per_s": ws_exact / (ms_per_step * 1e-3),
+        # cross-check from the committed ncu capture of this same launch configuration (None: none committed)
+        "ncu_fma_pipe_pct": None if ncu is None else ncu.get("fma_pipe_pct"),
+        "ncu_issue_active_pct": None if ncu is None else ncu.get("issue_active_pct"),
+        "ncu_kernel": None if ncu is None else ncu.get("kernel"),
+        "traffic": None if ncu is None else ncu.get("dram_bytes_read", 0) + ncu.get("dram_bytes_write", 0),
+        # side figures, NOT fractions of a hardware ceiling
+        "frac_survey_fma_count": survey_fma * ws_exact / (rw_ms * 1e-3) / 1e12 / peak,
+        "frac_nominal_issue": nominal * ws_exact / (rw_ms * 1e-3) / 1e12 / peak,
         "hbm_algorithmic_GBps": 8.0 * S * N / (ms_per_step * 1e-3) / 1e9, "hbm_peak_GBps": pk.get("hbm_gbs"),
-        "traffic": ncu_traffic(args.config, S),
+        "hbm_frac": 8.0 * S * N / (ms_per_step * 1e-3) / 1e9 / float(pk.get("hbm_gbs") or 6549.4),
     }
-    # What the kernel executes, as opposed to the 49 operations the method is charged with above: FMA-pipe
-    # lane-operations per window-sample as built (Phase 2: 2 with n+ from the median kernel; a pass: 5 when alpha is 1, 2 or 4 -- alpha*u is an
-    # integer add on the ALU pipe -- else 6) against the FMA pipe's 128 lanes/clk/SM.  ncu's
-    # sm__pipe_fma_cycles_active for the same launch is in profiles/ncu_full_r01.csv.
-    fma_ops = (2 if W > 49 else 3) + (5 if cfg.alpha in (1.0, 2.0, 4.0) and W > 49 else 6) * cfg.n_iter
-    roofline["executed"] = {"fma_pipe_lane_ops_per_window_sample": fma_ops,
-                            "fma_pipe_frac": fma_ops * ws_exact / (rw_ms * 1e-3) / 1e12 / peak,
-                            "peak_def": "148 SMs x 128 FP32 lanes x sm_max_mhz"}
-    if W <= 49:
-        roofline["kernel"] = "umi_small_kernel (fused phases 1-3)"
     cpu = None
     if not args.no_cpu_baseline:
         rate, _, cores = oracle_sample(cfg, flux_np, min(S, 16))

@@ -15,13 +15,14 @@
  *  - Every entry point returns a umi_status (int); nothing throws or aborts
  *    across this boundary.  Arguments are validated on the host before any
  *    work is enqueued.
- *  - No torch types, no hidden allocation that outlives a call (device
- *    scratch, where a call needs any, is stream-ordered: cudaMallocAsync /
- *    cudaFreeAsync on the caller's stream, see umi_detrend), no mutable
- *    global state: the library is re-entrant.  (Two exceptions, which hold no
- *    memory and no data: the host batch driver keeps its CUDA streams per host
- *    thread between calls, see umi_detrend_host; and the release threshold of
- *    the device's default memory pool is raised to 1 GiB.)
+ *  - No torch types.  The DEVICE entry points allocate nothing, create nothing and keep
+ *    no state: the only scratch their kernels share is trend_out itself, and any further
+ *    buffer is a caller-owned workspace (umi_detrend_gapped).  They are re-entrant and may
+ *    be called concurrently from several host threads on different streams.  The HOST
+ *    batch driver (umi_detrend_host, umi_flatten_host) has to own device buffers and
+ *    streams; it takes them from a memory pool and a stream free list the library creates
+ *    for itself per device (the device's default pool is never touched) and keeps them for
+ *    the next call until umi_shutdown().  Nothing reads the process environment.
  *  - "DEVICE pointer": memory of the current CUDA device, readable/writable by
  *    kernels launched on `stream`.  "HOST pointer": ordinary host memory
  *    (pinned memory makes the copies asynchronous and faster, but is not
@@ -35,8 +36,12 @@
  *    bit-exact always.  The trend of a star may differ in its last bits (~1e-7 relative) between calls
  *    with different batch sizes, because small batches run the split-window variant of the
  *    reweighting kernel, which sums the same terms in another order.
- *  - Supported dynamic range: within one tile of ~512 consecutive cadences,
- *    (max - min) * 16 * max(1, 1/alpha) must be finite in fp32.
+ *  - Supported dynamic range (windows longer than 49 samples): the passes run on samples
+ *    centred on the mid-range of the medians of 128 consecutive positions, so the 1e-5
+ *    bar on the trend is relative to the LARGEST |median| among those 128 positions (for a
+ *    light curve: the local flux); isolated samples of any finite magnitude (fill values,
+ *    glitches) cost the others no precision.  (max - min) * 16 * max(1, 1/alpha) over the
+ *    valid samples of those positions' windows must be finite in fp32.
  */
 #ifndef UMI_B200_H
 #define UMI_B200_H
@@ -87,14 +92,9 @@ int umi_window_len(double dt_days);
  *             Work is enqueued; the call does not synchronise.  The caller
  *             keeps all three buffers alive until the stream has drained.
  *
- * Scratch: when W > 49, n_iter > 0 and the batch holds more than 592 tiles of
- * 512 positions, the call takes 2 bytes per cadence from the device's default
- * memory pool with cudaMallocAsync on `stream` (the count n+ of Eq. 1, which
- * the first kernel hands to the second) and returns them with cudaFreeAsync
- * on `stream` before it returns; the pool's release threshold is raised to
- * 1 GiB (once per host thread) so that repeated calls reuse the memory.
- * Nothing allocated by the library outlives the work enqueued by the call.
- * A failed allocation -> UMI_ERR_CUDA, nothing enqueued.
+ * Scratch: none besides trend_out.  Between the two kernels of a call trend_out holds, per
+ * position, where in its window the median sample sits and the count n+ of Eq. 1; the
+ * second kernel overwrites both with the trend.  The call allocates nothing.
  *
  * c is fixed at 5.0.  Errors: see umi_status.
  */
@@ -175,8 +175,8 @@ int umi_detrend_family(const double* time, const float* flux,
  *   flat_out   DEVICE, float [n_stars*n_samples] or NULL: flux / trend.
  *   workspace  DEVICE, at least umi_gapped_workspace_bytes(n_stars, n_grid) bytes, owned by
  *              the caller, free to reuse once the stream has passed the call; too small or
- *              NULL -> UMI_ERR_INVALID_ARG.  It holds the two fp32 slot grids and the hot path's
- *              n+ scratch (10 bytes per slot): this entry point allocates nothing.
+ *              NULL -> UMI_ERR_INVALID_ARG.  It holds the two fp32 slot grids (flux, trend:
+ *              8 bytes per slot): this entry point allocates nothing.
  * Enqueues on `stream`; does not synchronise.
  */
 size_t umi_gapped_workspace_bytes(int64_t n_stars, int64_t n_grid);
@@ -194,13 +194,12 @@ int umi_detrend_gapped(const double* time, const float* flux,
  * ramp down by factors of 4, so that the first host->device copy and the last
  * device->host copy -- the only two no kernel hides -- are small), and
  * host->device copy, kernels and device->host copy of successive batches are
- * pipelined over `n_streams` CUDA streams (<= 0: 3) with one device buffer
- * set per stream, allocated and freed inside the call with cudaMallocAsync /
- * cudaFreeAsync (the call raises the release threshold of the device's
- * default memory pool to 1 GiB so that repeated calls reuse the buffers).
- * The streams themselves (at most 16 per host thread and device) are created
- * on first use and kept for the life of the process: creating and destroying
- * them per call cost 0.3 ms of an 8.7 ms job.
+ * pipelined over `n_streams` CUDA streams (<= 0: 3, at most 16) with one device
+ * buffer set per stream.  Buffers come from a memory pool the library creates for
+ * itself on the current device (cudaMemPoolCreate, release threshold 1 GiB: what a
+ * call frees is kept for the next one), streams from a free list; both are taken
+ * when the call starts, given back when it returns, and destroyed by umi_shutdown().
+ * Concurrent calls from several host threads are safe (each gets streams of its own).
  *
  *   time, flux, trend_out   HOST pointers, same shapes as above; time may be NULL.
  * The call returns after every batch has been copied back (it synchronises).
@@ -245,11 +244,20 @@ int umi_detrend_profile(const double* time, const float* flux,
  * arithmetic; host only).  Any pointer may be NULL.
  *   median_tile    positions per CTA of the Phase-1 (median) kernel
  *   median_sort_n  power-of-two length of the per-tile sort
- *   weight_tile    positions per CTA of the Phase-2/3 (reweighting) kernel in its throughput variant
- *                  (batches of at most 4 x 148 such tiles run the split-window variant: 1/8 of it)
+ *   weight_tile    positions per WARP tile of the Phase-2/3 (reweighting) kernel in its throughput variant
+ *                  (batches of at most 4 CTAs of four such tiles per SM run the split-window variant: 1/8 of it)
  * Returns UMI_OK, or INVALID_ARG / UNSUPPORTED for a bad W.
  */
 int umi_launch_geometry(int W, int* median_tile, int* median_sort_n, int* weight_tile);
+
+/*
+ * Releases what the HOST batch driver keeps between calls (its memory pools and idle
+ * streams, on every device it was used on).  Call it when no umi_*_host call is running;
+ * the library can be used again afterwards.  Returns UMI_OK, or UMI_ERR_CUDA if a
+ * destroy call failed.  The device entry points keep nothing, so programs that only use
+ * those never need it.
+ */
+int umi_shutdown(void);
 
 /* Static, never-freed string for a umi_status value. */
 const char* umi_status_string(int status);

@@ -23,7 +23,7 @@ UMI_WEIGHT_BISQUARE, UMI_WEIGHT_WELSCH = 0, 1
 
 EXPORTS = ("umi_window_len", "umi_detrend", "umi_detrend_ex", "umi_detrend_host", "umi_detrend_profile",
            "umi_flatten", "umi_flatten_host", "umi_detrend_family", "umi_detrend_gapped", "umi_gapped_workspace_bytes",
-           "umi_launch_geometry", "umi_status_string", "umi_version")
+           "umi_launch_geometry", "umi_status_string", "umi_version", "umi_shutdown")
 
 _lib = None
 
@@ -72,6 +72,8 @@ def lib():
     L.umi_status_string.argtypes = [ci]
     L.umi_version.restype = ci
     L.umi_version.argtypes = []
+    L.umi_shutdown.restype = ci
+    L.umi_shutdown.argtypes = []
     _lib = L
     return L
 
@@ -87,6 +89,11 @@ def umi_status_string(status):
 
 def umi_version():
     return int(lib().umi_version())
+
+
+def umi_shutdown():
+    """Release the host batch driver's memory pools and idle streams (include/umi.h)."""
+    _check(lib().umi_shutdown())
 
 
 def umi_window_len(dt_days):
@@ -114,6 +121,16 @@ def _cuda_2d(t, dtype, name):
     return t
 
 
+def _time_like(time, f):
+    import torch
+    if time is None:
+        return None
+    tt = _cuda_2d(time, torch.float64, "time")
+    if tt.shape != f.shape or tt.device != f.device:
+        raise ValueError("time must have flux's shape and device")
+    return tt
+
+
 def umi_detrend(time, flux, W, alpha=2.0, n_iter=5, out=None, stream=None, c=None, min_valid=None):
     """Device path.  `flux`: CUDA fp32 [S, N] (or [N]); `time`: None or CUDA fp64 of the
     same shape.  Enqueues on `stream` (default: torch's current stream) and returns the
@@ -121,42 +138,60 @@ def umi_detrend(time, flux, W, alpha=2.0, n_iter=5, out=None, stream=None, c=Non
     umi_detrend_ex (Table 4)."""
     import torch
     f = _cuda_2d(flux, torch.float32, "flux")
-    tptr = None
-    if time is not None:
-        tt = _cuda_2d(time, torch.float64, "time")
-        if tt.shape != f.shape or tt.device != f.device:
-            raise ValueError("time must have flux's shape and device")
-        tptr = tt.data_ptr()
-    if out is None:
-        out = torch.empty_like(f)
-    else:
+    tt = _time_like(time, f)
+    if out is not None:
         out = _cuda_2d(out, torch.float32, "out")
         if out.shape != f.shape or out.device != f.device:
             raise ValueError("out must have flux's shape and device")
     S, N = f.shape
-    with torch.cuda.device(f.device):
-        if stream is None:
-            stream = torch.cuda.current_stream(f.device)
-        sptr = stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
-        fptr = f.data_ptr() if f.numel() else None
-        optr = out.data_ptr() if out.numel() else None
+    with _OnStream(stream, f.device) as on:
+        if out is None:
+            out = torch.empty_like(f)
+        on.uses(f, tt, out)
         if S == 0 or N == 0:
             return out.view(flux.shape)
+        tptr = None if tt is None else tt.data_ptr()
         if c is None and min_valid is None:
-            st = lib().umi_detrend(tptr, fptr, S, N, int(W), float(alpha), int(n_iter), optr, sptr)
+            st = lib().umi_detrend(tptr, f.data_ptr(), S, N, int(W), float(alpha), int(n_iter), out.data_ptr(), on.ptr)
         else:
-            st = lib().umi_detrend_ex(tptr, fptr, S, N, int(W), float(alpha),
+            st = lib().umi_detrend_ex(tptr, f.data_ptr(), S, N, int(W), float(alpha),
                                       5.0 if c is None else float(c), int(n_iter),
-                                      -1 if min_valid is None else int(min_valid), optr, sptr)
+                                      -1 if min_valid is None else int(min_valid), out.data_ptr(), on.ptr)
     _check(st)
     return out.view(flux.shape)
 
 
-def _stream_ptr(stream, device):
-    import torch
-    if stream is None:
-        stream = torch.cuda.current_stream(device)
-    return stream.cuda_stream if hasattr(stream, "cuda_stream") else int(stream)
+class _OnStream:
+    """Allocations made inside the block belong to `stream` (torch's caching allocator hands memory
+    out per stream, so a tensor allocated on another stream could still be in use there), and tensors
+    the caller allocated elsewhere are recorded as used on it.  `stream`: None (torch's current
+    stream), a torch.cuda.Stream / ExternalStream, or a raw cudaStream_t as int."""
+
+    def __init__(self, stream, device):
+        import torch
+        if stream is None:
+            stream = torch.cuda.current_stream(device)
+        elif not hasattr(stream, "cuda_stream"):
+            stream = torch.cuda.ExternalStream(int(stream), device=device)
+        self.stream = stream
+        self.ptr = stream.cuda_stream
+        self._dev = torch.cuda.device(device)
+        self._ctx = torch.cuda.stream(stream)
+
+    def __enter__(self):
+        self._dev.__enter__()
+        self._ctx.__enter__()
+        return self
+
+    def __exit__(self, *exc):
+        self._ctx.__exit__(*exc)
+        self._dev.__exit__(*exc)
+        return False
+
+    def uses(self, *tensors):
+        for t in tensors:
+            if t is not None and t.numel():
+                t.record_stream(self.stream)
 
 
 def umi_flatten(time, flux, W, alpha=2.0, n_iter=5, c=5.0, min_valid=-1, stream=None):
@@ -164,19 +199,14 @@ def umi_flatten(time, flux, W, alpha=2.0, n_iter=5, c=5.0, min_valid=-1, stream=
     computed in the kernels' epilogue.  Same argument rules as umi_detrend."""
     import torch
     f = _cuda_2d(flux, torch.float32, "flux")
-    tptr = None
-    if time is not None:
-        tt = _cuda_2d(time, torch.float64, "time")
-        if tt.shape != f.shape or tt.device != f.device:
-            raise ValueError("time must have flux's shape and device")
-        tptr = tt.data_ptr()
-    trend, flat = torch.empty_like(f), torch.empty_like(f)
+    tt = _time_like(time, f)
     S, N = f.shape
-    if S and N:
-        with torch.cuda.device(f.device):
-            _check(lib().umi_flatten(tptr, f.data_ptr(), S, N, int(W), float(alpha), float(c), int(n_iter),
-                                     int(min_valid), trend.data_ptr(), flat.data_ptr(),
-                                     _stream_ptr(stream, f.device)))
+    with _OnStream(stream, f.device) as on:
+        trend, flat = torch.empty_like(f), torch.empty_like(f)
+        on.uses(f, tt)
+        if S and N:
+            _check(lib().umi_flatten(None if tt is None else tt.data_ptr(), f.data_ptr(), S, N, int(W), float(alpha),
+                                     float(c), int(n_iter), int(min_valid), trend.data_ptr(), flat.data_ptr(), on.ptr))
     return trend.view(flux.shape), flat.view(flux.shape)
 
 
@@ -186,21 +216,17 @@ def umi_detrend_family(time, flux, W, scale_kind=0, weight_kind=0, alpha=2.0, n_
     Returns (trend, scale) or (trend, scale, flat)."""
     import torch
     f = _cuda_2d(flux, torch.float32, "flux")
-    tptr = None
-    if time is not None:
-        tt = _cuda_2d(time, torch.float64, "time")
-        if tt.shape != f.shape or tt.device != f.device:
-            raise ValueError("time must have flux's shape and device")
-        tptr = tt.data_ptr()
-    trend, scale = torch.empty_like(f), torch.empty_like(f)
-    fl = torch.empty_like(f) if flat else None
+    tt = _time_like(time, f)
     S, N = f.shape
-    if S and N:
-        with torch.cuda.device(f.device):
-            _check(lib().umi_detrend_family(tptr, f.data_ptr(), S, N, int(W), int(scale_kind), int(weight_kind),
-                                            float(alpha), float(c), int(n_iter), int(min_valid),
-                                            trend.data_ptr(), scale.data_ptr(), fl.data_ptr() if flat else None,
-                                            _stream_ptr(stream, f.device)))
+    with _OnStream(stream, f.device) as on:
+        trend, scale = torch.empty_like(f), torch.empty_like(f)
+        fl = torch.empty_like(f) if flat else None
+        on.uses(f, tt)
+        if S and N:
+            _check(lib().umi_detrend_family(None if tt is None else tt.data_ptr(), f.data_ptr(), S, N, int(W),
+                                            int(scale_kind), int(weight_kind), float(alpha), float(c), int(n_iter),
+                                            int(min_valid), trend.data_ptr(), scale.data_ptr(),
+                                            fl.data_ptr() if flat else None, on.ptr))
     out = (trend.view(flux.shape), scale.view(flux.shape))
     return out + (fl.view(flux.shape),) if flat else out
 
@@ -213,7 +239,8 @@ def umi_detrend_gapped(time, flux, t0, dt, n_grid, W, alpha=2.0, n_iter=5, c=5.0
                        flat=False, workspace=None, stream=None):
     """Compacted rows with real time stamps (gap handling; include/umi.h).
     `time` CUDA fp64 [S, M], `flux` CUDA fp32 [S, M].  Returns trend, or (trend, flat).
-    `workspace`: optional CUDA uint8 tensor of at least umi_gapped_workspace_bytes bytes."""
+    `workspace`: optional CUDA uint8 tensor of at least umi_gapped_workspace_bytes bytes; when it is
+    not given, one is allocated on `stream`, so its release is ordered after the kernels that use it."""
     import torch
     f = _cuda_2d(flux, torch.float32, "flux")
     tt = _cuda_2d(time, torch.float64, "time")
@@ -221,19 +248,20 @@ def umi_detrend_gapped(time, flux, t0, dt, n_grid, W, alpha=2.0, n_iter=5, c=5.0
         raise ValueError("time must have flux's shape and device")
     S, M = f.shape
     need = umi_gapped_workspace_bytes(S, n_grid)
-    if workspace is None:
-        workspace = torch.empty(max(need, 1), dtype=torch.uint8, device=f.device)
-    elif not (isinstance(workspace, torch.Tensor) and workspace.is_cuda and workspace.is_contiguous()):
+    if workspace is not None and not (isinstance(workspace, torch.Tensor) and workspace.is_cuda and workspace.is_contiguous()):
         raise TypeError("workspace must be a contiguous CUDA tensor")
-    wbytes = workspace.numel() * workspace.element_size()
-    trend = torch.empty_like(f)
-    fl = torch.empty_like(f) if flat else None
-    if S and M:
-        with torch.cuda.device(f.device):
+    with _OnStream(stream, f.device) as on:
+        if workspace is None:
+            workspace = torch.empty(max(need, 1), dtype=torch.uint8, device=f.device)
+        wbytes = workspace.numel() * workspace.element_size()
+        trend = torch.empty_like(f)
+        fl = torch.empty_like(f) if flat else None
+        on.uses(f, tt, workspace)
+        if S and M:
             _check(lib().umi_detrend_gapped(tt.data_ptr(), f.data_ptr(), S, M, float(t0), float(dt), int(n_grid),
                                             int(W), float(alpha), float(c), int(n_iter), int(min_valid),
                                             trend.data_ptr(), fl.data_ptr() if flat else None,
-                                            workspace.data_ptr(), wbytes, _stream_ptr(stream, f.device)))
+                                            workspace.data_ptr(), wbytes, on.ptr))
     return (trend.view(flux.shape), fl.view(flux.shape)) if flat else trend.view(flux.shape)
 
 
@@ -242,22 +270,16 @@ def umi_detrend_profile(time, flux, W, alpha=2.0, n_iter=5, out=None, stream=Non
     Synchronises the stream (measurement aid)."""
     import torch
     f = _cuda_2d(flux, torch.float32, "flux")
-    tptr = None
-    if time is not None:
-        tt = _cuda_2d(time, torch.float64, "time")
-        if tt.shape != f.shape:
-            raise ValueError("time must have flux's shape")
-        tptr = tt.data_ptr()
-    if out is None:
-        out = torch.empty_like(f)
-    o = _cuda_2d(out, torch.float32, "out")
+    tt = _time_like(time, f)
     S, N = f.shape
     ms = (ctypes.c_float * 2)()
-    with torch.cuda.device(f.device):
-        if stream is None:
-            stream = torch.cuda.current_stream(f.device)
-        _check(lib().umi_detrend_profile(tptr, f.data_ptr(), S, N, int(W), float(alpha), float(c),
-                                         int(n_iter), int(min_valid), o.data_ptr(), stream.cuda_stream, ms))
+    with _OnStream(stream, f.device) as on:
+        if out is None:
+            out = torch.empty_like(f)
+        o = _cuda_2d(out, torch.float32, "out")
+        on.uses(f, tt, o)
+        _check(lib().umi_detrend_profile(None if tt is None else tt.data_ptr(), f.data_ptr(), S, N, int(W), float(alpha),
+                                         float(c), int(n_iter), int(min_valid), o.data_ptr(), on.ptr, ms))
     return out.view(flux.shape), float(ms[0]), float(ms[1])
 
 

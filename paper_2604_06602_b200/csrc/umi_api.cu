@@ -8,6 +8,7 @@
 #include <stdlib.h>
 
 #include <algorithm>
+#include <mutex>
 #include <vector>
 
 #include "umi.h"
@@ -16,7 +17,6 @@
 namespace {
 
 constexpr int64_t MAX_GRID = 0x7FFFFFFF;
-constexpr int TC_MAX_WINDOW = 1101;      /* tensor-core reweighting: B tile + samples <= ~45 KB of shared memory per CTA */
 
 /* sibling-estimator selection (F4); the default is the paper's path */
 struct Family {
@@ -28,7 +28,7 @@ struct Family {
 struct Geometry {
     int T1, NS;            /* median kernel: positions per tile, sort length */
     size_t smem1;
-    size_t smem2;          /* reweighting kernel */
+    int halo4;             /* reweighting kernel: staged floats per warp besides its tile (4 per float4 group) */
 };
 
 /* DESIGN.md, "Launch geometry": the sort length is the smallest power of two
@@ -44,14 +44,19 @@ Geometry geometry_for(int W)
     const int h = (W - 1) / 2;
     const int hal = (h + 3) & ~3;
     const int G = (3 + (hal - h) + 2 * h) / 4 + 1;
-    g.smem2 = (size_t)(umi::K2_TILE + 4 * G) * sizeof(float);
+    g.halo4 = 4 * G;
     return g;
 }
 
-bool tc_requested()
+/* SMs of the current device (sizes the "does this batch fill the GPU" decision); 148 on B200 */
+int sm_count()
 {
-    const char* e = getenv("UMI_B200_TC");
-    return e != nullptr && e[0] == '1';
+    int dev = 0, n = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n <= 0) {
+        (void)cudaGetLastError();
+        return 148;
+    }
+    return n;
 }
 
 int check_window(int W)
@@ -77,35 +82,12 @@ int validate(const float* flux, int64_t n_stars, int64_t n_cadences, int W, floa
     return check_window(W);
 }
 
-/* Stream-ordered allocations (the n+ scratch of launch_device, the buffers of the host driver) come from the
-   device's default memory pool.  Its release threshold is 0 by default, i.e. every synchronisation hands the
-   freed memory back to the driver and the next call maps it again (0.1-0.2 ms for 40 MB); raised once per
-   host thread and device to 1 GiB so that repeated calls reuse it. */
-void keep_pool_memory()
-{
-    thread_local int done_for = -1;
-    int dev = 0;
-    if (cudaGetDevice(&dev) != cudaSuccess) { (void)cudaGetLastError(); return; }
-    if (done_for == dev) return;
-    cudaMemPool_t pool = nullptr;
-    if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-        uint64_t thr = 0;
-        if (cudaMemPoolGetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr) == cudaSuccess &&
-            thr < (1ull << 30)) {
-            thr = 1ull << 30;
-            (void)cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
-        }
-    }
-    (void)cudaGetLastError();
-    done_for = dev;
-}
-
-/* Enqueue both kernels for device-resident buffers. */
+/* Enqueue the kernels of one call for device-resident buffers.  Allocates nothing: the only scratch the two
+   kernels share is trend_out itself (umi_internal.h, "hand-over word"). */
 int launch_device(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
                   int W, float alpha, float c, int n_iter, int min_valid, float* trend_out,
                   cudaStream_t stream, cudaEvent_t* ev = nullptr /* [3] or null */,
-                  float* flat_out = nullptr, const Family& fam = Family(),
-                  uint16_t* nplus_scratch = nullptr /* [n_stars*n_cadences], or null: allocated here when needed */)
+                  float* flat_out = nullptr, const Family& fam = Family())
 {
     if (n_stars == 0 || n_cadences == 0) return UMI_OK;
     Geometry g = geometry_for(W);
@@ -129,8 +111,8 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.c = c;
         rp.c_over_alpha = c / alpha;
         rp.split = 1;
+        rp.packed = 0;
         rp.scale_in = nullptr;
-        rp.nplus = nullptr;
         rp.scale_out = fam.scale_out;
         rp.weight_kind = fam.weight_kind;
         rp.scale_kind = fam.scale_kind;
@@ -143,35 +125,21 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         return UMI_OK;
     }
 
-    /* The paper's path with passes to run: the median kernel also writes n+ (Eq. 1's count, exact on the sorted
-       keys) into a stream-ordered scratch buffer of 2 bytes per cadence, which the reweighting kernel reads
-       instead of counting again.  Allocated and freed in stream order inside this call (default memory pool). */
-    struct StreamScratch {
-        void* p = nullptr;
-        cudaStream_t s = nullptr;
-        ~StreamScratch() { if (p != nullptr) (void)cudaFreeAsync(p, s); }
-    } scratch;
-    scratch.s = stream;
-    uint16_t* nplus = nullptr;
-    /* (not for batches small enough to take the split-window variant: there the call is latency-bound and the
-       allocation would cost as much as the kernels, 45 -> 88 us on config 1) */
-    const int64_t rw_tiles = n_stars * ((n_cadences + umi::K2_TILE - 1) / umi::K2_TILE);
-    if (!fam.on && n_iter > 0 && rw_tiles > 4 * 148 && nplus_scratch != nullptr) {
-        nplus = nplus_scratch;
-    } else if (!fam.on && n_iter > 0 && rw_tiles > 4 * 148) {
-        keep_pool_memory();
-        if (cuda_failed(cudaMallocAsync(&scratch.p, (size_t)n_stars * (size_t)n_cadences * sizeof(uint16_t), stream)))
-            return UMI_ERR_CUDA;
-        nplus = static_cast<uint16_t*>(scratch.p);
-    }
+    /* the family path also runs the second kernel with n_iter = 0 when only the upper-RMS scale is wanted */
+    const bool scale_only = fam.on && !mad && fam.scale_out != nullptr && n_iter == 0;
+    const bool second = n_iter > 0 || scale_only;
+    /* The paper's path with passes to run: the median kernel leaves, per position, where in its window the
+       median sample sits and n+ (Eq. 1's count, exact on the sorted keys) in trend_out; the reweighting
+       kernel reads both back and overwrites them with the trend. */
+    const int packed = (!fam.on && n_iter > 0) ? 1 : 0;
 
     umi::MedianParams mp;
     mp.time = time;
     mp.flux = flux;
     mp.out = trend_out;
-    mp.flat = (n_iter == 0) ? flat_out : nullptr;
+    mp.flat = second ? nullptr : flat_out;                  /* whichever kernel writes the final trend divides */
     mp.scale = mad ? fam.scale_out : nullptr;
-    mp.nplus = nplus;
+    mp.packed = packed;
     mp.N = n_cadences;
     mp.tiles_per_star = (n_cadences + g.T1 - 1) / g.T1;
     mp.n_blocks = n_stars * mp.tiles_per_star;
@@ -184,25 +152,24 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
     if (cuda_failed(umi::launch_median(mp, grid1, g.smem1, stream))) return UMI_ERR_CUDA;
     if (ev && cuda_failed(cudaEventRecord(ev[1], stream))) return UMI_ERR_CUDA;
 
-    /* the family path also runs the second kernel with n_iter = 0 when only the upper-RMS scale is wanted */
-    const bool scale_only = fam.on && !mad && fam.scale_out != nullptr && n_iter == 0;
-    if (scale_only) mp.flat = nullptr;
-    if (n_iter > 0 || scale_only) {
+    if (second) {
         umi::ReweightParams rp;
         rp.time = time;
         rp.flux = flux;
         rp.out = trend_out;
         rp.flat = flat_out;
         rp.N = n_cadences;
-        rp.tiles_per_star = (n_cadences + umi::K2_TILE - 1) / umi::K2_TILE;
-        rp.n_blocks = n_stars * rp.tiles_per_star;
         rp.split = 1;
-        if (!fam.on && rp.n_blocks <= 4 * 148) {
-            /* the grid would leave most of the 148 x 8 CTA slots empty: split every window over
+        rp.packed = packed;
+        int wtile = umi::K2_WARP_TILE;
+        rp.tiles_per_star = (n_cadences + wtile - 1) / wtile;
+        rp.n_blocks = n_stars * rp.tiles_per_star;
+        if (!fam.on && (rp.n_blocks + umi::K2_WARPS - 1) / umi::K2_WARPS <= 4 * (int64_t)sm_count()) {
+            /* the grid would leave most of the resident-CTA slots empty: split every window over
                K2_SPLIT lanes instead (latency, not throughput, is what is left to win) */
             rp.split = umi::K2_SPLIT;
-            const int tile = umi::K2_TILE / umi::K2_SPLIT;
-            rp.tiles_per_star = (n_cadences + tile - 1) / tile;
+            wtile = umi::K2_WARP_TILE / umi::K2_SPLIT;
+            rp.tiles_per_star = (n_cadences + wtile - 1) / wtile;
             rp.n_blocks = n_stars * rp.tiles_per_star;
         }
         rp.W = W;
@@ -211,27 +178,11 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.c = c;
         rp.c_over_alpha = c / alpha;
         rp.scale_in = mad ? fam.scale_out : nullptr;
-        rp.nplus = nplus;
         rp.scale_out = mad ? nullptr : fam.scale_out;
         rp.weight_kind = fam.weight_kind;
         rp.scale_kind = fam.scale_kind;
-        /* Experimental, off by default: weights on the CUDA cores, the two sums of Eq. 4 on the tensor cores
-           (umi_reweight_tc.cu: tcgen05.mma with the weights in TMEM).  Correct (same parity tests) but measured
-           slower than the all-CUDA-core kernel on config 2 (13.8 ms vs 8.78 ms), so it only
-           runs when UMI_B200_TC=1 is set in the environment. */
-        if (!fam.on && rp.split == 1 && n_iter > 0 && W <= TC_MAX_WINDOW && tc_requested()) {
-            rp.tiles_per_star = (n_cadences + umi::tc_tile() - 1) / umi::tc_tile();
-            rp.n_blocks = n_stars * rp.tiles_per_star;
-            if (rp.n_blocks <= MAX_GRID) {
-                if (cuda_failed(umi::launch_reweight_tc(rp, (unsigned)rp.n_blocks, stream))) return UMI_ERR_CUDA;
-                if (ev && cuda_failed(cudaEventRecord(ev[2], stream))) return UMI_ERR_CUDA;
-                return UMI_OK;
-            }
-            rp.tiles_per_star = (n_cadences + umi::K2_TILE - 1) / umi::K2_TILE;
-            rp.n_blocks = n_stars * rp.tiles_per_star;
-        }
-        const unsigned grid2 = (unsigned)std::min<int64_t>(rp.n_blocks, MAX_GRID);
-        const size_t smem2 = g.smem2 - (size_t)(umi::K2_TILE - umi::K2_TILE / rp.split) * sizeof(float);
+        const unsigned grid2 = (unsigned)std::min<int64_t>((rp.n_blocks + umi::K2_WARPS - 1) / umi::K2_WARPS, MAX_GRID);
+        const size_t smem2 = (size_t)umi::K2_WARPS * (size_t)(wtile + g.halo4) * sizeof(float);
         if (cuda_failed(umi::launch_reweight(rp, fam.on, grid2, smem2, stream))) return UMI_ERR_CUDA;
     }
     if (ev && cuda_failed(cudaEventRecord(ev[2], stream))) return UMI_ERR_CUDA;
@@ -292,8 +243,8 @@ int umi_detrend_family(const double* time, const float* flux, int64_t n_stars, i
 size_t umi_gapped_workspace_bytes(int64_t n_stars, int64_t n_grid)
 {
     if (n_stars <= 0 || n_grid <= 0) return 0;
-    /* two fp32 grids (flux, trend) and the uint16 n+ scratch of the hot path */
-    return (size_t)n_stars * (size_t)n_grid * (2 * sizeof(float) + sizeof(uint16_t));
+    /* two fp32 grids: flux on the slots, and the trend on the slots */
+    return (size_t)n_stars * (size_t)n_grid * (2 * sizeof(float));
 }
 
 int umi_detrend_gapped(const double* time, const float* flux, int64_t n_stars, int64_t n_samples,
@@ -324,9 +275,8 @@ int umi_detrend_gapped(const double* time, const float* flux, int64_t n_stars, i
         if (cuda_failed(cudaMemsetAsync(grid_flux, 0xFF, (size_t)n_stars * (size_t)n_grid * sizeof(float), s)))
             return UMI_ERR_CUDA;
         if (cuda_failed(umi::launch_regrid_scatter(gp, grid_flux, s))) return UMI_ERR_CUDA;
-        uint16_t* grid_nplus = reinterpret_cast<uint16_t*>(grid_trend + (size_t)n_stars * (size_t)n_grid);
         const int st2 = launch_device(nullptr, grid_flux, n_stars, n_grid, W, alpha, c, n_iter, min_valid,
-                                      grid_trend, s, nullptr, nullptr, Family(), grid_nplus);
+                                      grid_trend, s);
         if (st2 != UMI_OK) return st2;
     }
     if (cuda_failed(umi::launch_regrid_gather(gp, grid_trend, trend_out, flat_out, s))) return UMI_ERR_CUDA;
@@ -369,31 +319,72 @@ int umi_detrend(const double* time, const float* flux, int64_t n_stars, int64_t 
 
 namespace {
 
-/* Streams of the batch driver, kept per host thread and per device between calls: creating and destroying
-   three streams per call cost ~0.3 ms of a 8.7 ms config-2 job.  They are never destroyed (a destructor at
-   thread or process exit would call into a CUDA runtime that may already be gone); at most 16 per thread and
-   device.  This is the only state the library keeps; it holds no memory and no data. */
-struct StreamCache {
-    int dev = -1;
-    std::vector<cudaStream_t> streams;
+/* What the HOST batch driver keeps between calls, per device: a memory pool of its own for the per-stream
+   device buffers (cudaMemPoolCreate; the device's default pool and its attributes are never touched) and a
+   free list of CUDA streams (creating and destroying three streams per call cost ~0.3 ms of an 8.7 ms
+   config-2 job).  A call takes what it needs under the mutex and puts it back when it returns, so concurrent
+   callers never share a stream; umi_shutdown() destroys everything.  The DEVICE entry points use none of it. */
+constexpr int MAX_DEVICES = 64;
+struct HostDriverState {
+    std::mutex lock;
+    cudaMemPool_t pool[MAX_DEVICES] = {};
+    std::vector<cudaStream_t> idle[MAX_DEVICES];
 };
-
-bool cached_streams(int n, std::vector<cudaStream_t>& out)
+HostDriverState& driver_state()
 {
-    thread_local StreamCache* cache = new StreamCache();          /* leaked on purpose, see above */
-    int dev = 0;
-    if (cuda_failed(cudaGetDevice(&dev))) return false;
-    if (cache->dev != dev) {                                        /* another device: start over (old ones leak) */
-        cache->dev = dev;
-        cache->streams.clear();
+    static HostDriverState* st = new HostDriverState();     /* never destroyed: no CUDA call from a static destructor */
+    return *st;
+}
+
+/* the library's pool on device `dev` (created on first use; freed memory is kept up to 1 GiB for the next call) */
+cudaMemPool_t driver_pool(int dev)
+{
+    if (dev < 0 || dev >= MAX_DEVICES) return nullptr;
+    HostDriverState& st = driver_state();
+    std::lock_guard<std::mutex> guard(st.lock);
+    if (st.pool[dev] == nullptr) {
+        cudaMemPoolProps props = {};
+        props.allocType = cudaMemAllocationTypePinned;
+        props.handleTypes = cudaMemHandleTypeNone;
+        props.location.type = cudaMemLocationTypeDevice;
+        props.location.id = dev;
+        cudaMemPool_t pool = nullptr;
+        if (cuda_failed(cudaMemPoolCreate(&pool, &props))) return nullptr;
+        uint64_t thr = 1ull << 30;
+        (void)cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
+        (void)cudaGetLastError();
+        st.pool[dev] = pool;
     }
-    while ((int)cache->streams.size() < n) {
-        cudaStream_t st = nullptr;
-        if (cuda_failed(cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking))) return false;
-        cache->streams.push_back(st);
+    return st.pool[dev];
+}
+
+bool take_streams(int dev, int n, std::vector<cudaStream_t>& out)
+{
+    out.clear();
+    if (dev < 0 || dev >= MAX_DEVICES) return false;
+    HostDriverState& st = driver_state();
+    {
+        std::lock_guard<std::mutex> guard(st.lock);
+        while ((int)out.size() < n && !st.idle[dev].empty()) {
+            out.push_back(st.idle[dev].back());
+            st.idle[dev].pop_back();
+        }
     }
-    out.assign(cache->streams.begin(), cache->streams.begin() + n);
+    while ((int)out.size() < n) {
+        cudaStream_t s = nullptr;
+        if (cuda_failed(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking))) return false;
+        out.push_back(s);
+    }
     return true;
+}
+
+void return_streams(int dev, std::vector<cudaStream_t>& streams)
+{
+    if (dev < 0 || dev >= MAX_DEVICES) return;
+    HostDriverState& st = driver_state();
+    std::lock_guard<std::mutex> guard(st.lock);
+    for (cudaStream_t s : streams) st.idle[dev].push_back(s);
+    streams.clear();
 }
 
 /* the batch driver behind umi_detrend_host / umi_flatten_host: trend_out and flat_out are HOST pointers,
@@ -450,25 +441,27 @@ int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t 
         float* d_trend = nullptr;
         float* d_flat = nullptr;
         double* d_time = nullptr;
-        uint16_t* d_nplus = nullptr;   /* the n+ scratch of launch_device, per slot: an allocation inside every batch would
-                                          make the pool hand memory from one stream to another and serialise them */
     };
     std::vector<Slot> slots((size_t)n_streams);
-    keep_pool_memory();     /* the per-call buffers stay in the driver's stream-ordered pool between calls */
     const size_t elems = (size_t)stars_per_batch * (size_t)n_cadences;
     int status = UMI_OK;
 
+    int dev = 0;
+    if (cuda_failed(cudaGetDevice(&dev))) return UMI_ERR_CUDA;
+    cudaMemPool_t pool = driver_pool(dev);
+    if (pool == nullptr) return UMI_ERR_CUDA;
     std::vector<cudaStream_t> streams;
-    if (!cached_streams(n_streams, streams)) return UMI_ERR_CUDA;
+    if (!take_streams(dev, n_streams, streams)) {
+        return_streams(dev, streams);
+        return UMI_ERR_CUDA;
+    }
     for (size_t i = 0; i < slots.size(); ++i) slots[i].stream = streams[i];
     for (auto& s : slots) {
-        if (/* stream-ordered allocations: served from the driver's pool after the first call */
-            cuda_failed(cudaMallocAsync((void**)&s.d_flux, elems * sizeof(float), s.stream)) ||
-            cuda_failed(cudaMallocAsync((void**)&s.d_trend, elems * sizeof(float), s.stream)) ||
-            (flat_out != nullptr && cuda_failed(cudaMallocAsync((void**)&s.d_flat, elems * sizeof(float), s.stream))) ||
-            (time != nullptr && cuda_failed(cudaMallocAsync((void**)&s.d_time, elems * sizeof(double), s.stream))) ||
-            (W > umi::KS_MAX_WINDOW && n_iter > 0 &&
-             cuda_failed(cudaMallocAsync((void**)&s.d_nplus, elems * sizeof(uint16_t), s.stream)))) {
+        if (/* stream-ordered allocations from the library's own pool: served from memory it kept after the first call */
+            cuda_failed(cudaMallocFromPoolAsync((void**)&s.d_flux, elems * sizeof(float), pool, s.stream)) ||
+            cuda_failed(cudaMallocFromPoolAsync((void**)&s.d_trend, elems * sizeof(float), pool, s.stream)) ||
+            (flat_out != nullptr && cuda_failed(cudaMallocFromPoolAsync((void**)&s.d_flat, elems * sizeof(float), pool, s.stream))) ||
+            (time != nullptr && cuda_failed(cudaMallocFromPoolAsync((void**)&s.d_time, elems * sizeof(double), pool, s.stream)))) {
             status = UMI_ERR_CUDA;
             break;
         }
@@ -488,7 +481,7 @@ int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t 
             break;
         }
         status = launch_device(s.d_time, s.d_flux, ns, n_cadences, W, alpha, c, n_iter, min_valid, s.d_trend, s.stream,
-                               nullptr, s.d_flat, Family(), s.d_nplus);
+                               nullptr, s.d_flat);
         if (status != UMI_OK) break;
         if ((trend_out != nullptr &&
              cuda_failed(cudaMemcpyAsync(trend_out + off, s.d_trend, cnt * sizeof(float), cudaMemcpyDeviceToHost, s.stream))) ||
@@ -503,16 +496,33 @@ int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t 
         if (s.d_trend) (void)cudaFreeAsync(s.d_trend, s.stream);
         if (s.d_flat) (void)cudaFreeAsync(s.d_flat, s.stream);
         if (s.d_time) (void)cudaFreeAsync(s.d_time, s.stream);
-        if (s.d_nplus) (void)cudaFreeAsync(s.d_nplus, s.stream);
         if (cuda_failed(cudaStreamSynchronize(s.stream))) status = UMI_ERR_CUDA;
     }
     (void)cudaGetLastError();
+    return_streams(dev, streams);
     return status;
 }
 
 } // namespace
 
 extern "C" {
+
+int umi_shutdown(void)
+{
+    HostDriverState& st = driver_state();
+    std::lock_guard<std::mutex> guard(st.lock);
+    int status = UMI_OK;
+    for (int dev = 0; dev < MAX_DEVICES; ++dev) {
+        for (cudaStream_t s : st.idle[dev])
+            if (cuda_failed(cudaStreamDestroy(s))) status = UMI_ERR_CUDA;
+        st.idle[dev].clear();
+        if (st.pool[dev] != nullptr) {
+            if (cuda_failed(cudaMemPoolDestroy(st.pool[dev]))) status = UMI_ERR_CUDA;
+            st.pool[dev] = nullptr;
+        }
+    }
+    return status;
+}
 
 int umi_detrend_host(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
                      int W, float alpha, int n_iter, float* trend_out,
@@ -539,7 +549,7 @@ int umi_launch_geometry(int W, int* median_tile, int* median_sort_n, int* weight
     const Geometry g = geometry_for(W);
     if (median_tile) *median_tile = g.T1;
     if (median_sort_n) *median_sort_n = g.NS;
-    if (weight_tile) *weight_tile = umi::K2_TILE;
+    if (weight_tile) *weight_tile = umi::K2_WARP_TILE;
     return UMI_OK;
 }
 
@@ -554,6 +564,6 @@ const char* umi_status_string(int status)
     }
 }
 
-int umi_version(void) { return 200; /* 0.2.0 */ }
+int umi_version(void) { return 300; /* 0.3.0 */ }
 
 } /* extern "C" */

@@ -1,4 +1,5 @@
-/* umi_internal.h -- launch parameters shared by umi_kernels.cu and umi_api.cu (not installed). */
+/* umi_internal.h -- launch parameters and launch functions shared by the kernel files (umi_median.cu,
+   umi_reweight.cu, umi_small.cu, umi_regrid.cu) and umi_api.cu (not installed). */
 #ifndef UMI_INTERNAL_H
 #define UMI_INTERNAL_H
 
@@ -25,7 +26,7 @@ __host__ __device__ constexpr size_t k1_smem_bytes(int ns, bool mad = false, int
        + u32 sorted keys */
     const size_t bw = (size_t)ns / 32, nw = (size_t)k1_walkers(ns);
     const size_t bits = 4 * (nw * (bw + 1) + (nw / 32) * bw);
-    /* f32 medians [T], then u16 median ranks [T] and u16 window counts [T] (for n+), rounded to 16 bytes */
+    /* f32 medians [T], then u16 median ranks [T] and u16 window counts [T] (for n+ and the packed hand-over), rounded to 16 bytes */
     const size_t med = ((8 * (size_t)(t > 0 ? t : ns)) + 15) / 16 * 16;
     /* the MAD variant stages one more fp32 per position (the scale) behind everything else */
     return (size_t)ns * 10 + (bits > med ? bits : med) + 4 * (size_t)ns + (mad ? 4 * (size_t)ns : 0);
@@ -43,17 +44,27 @@ constexpr int KS_MAX_WINDOW = 49;                /* windows up to this length ta
 #define UMI_K2_THREADS 128
 #endif
 constexpr int K2_THREADS = UMI_K2_THREADS;       /* reweighting kernel */
+constexpr int K2_WARPS = K2_THREADS / 32;        /* every warp owns tiles of its own: no CTA-wide barrier in the kernel */
 constexpr int K2_NPOS = 4;                       /* consecutive positions per thread */
-constexpr int K2_TILE = K2_THREADS * K2_NPOS;    /* positions per CTA */
-constexpr int K2_SPLIT = 8;                      /* small batches: lanes per 4 positions (tile = K2_TILE / K2_SPLIT) */
+constexpr int K2_WARP_TILE = 32 * K2_NPOS;       /* positions per warp tile (throughput variant) */
+constexpr int K2_TILE = K2_THREADS * K2_NPOS;    /* positions per CTA and trip of its tile loop */
+constexpr int K2_SPLIT = 8;                      /* small batches: lanes per 4 positions (warp tile = K2_WARP_TILE / K2_SPLIT) */
+
+/* What the median kernel leaves in `out` for the reweighting kernel when passes follow (the paper's path):
+   one 32-bit word per position, 0xFFFFFFFF = no trend here (R4, R5), else
+       bits  0..15  offset of the median sample inside the window, 0 .. W-1 (the median IS a window sample)
+       bits 16..31  n+ of Eq. 1 (R7), counted exactly on the sorted keys.
+   The reweighting kernel has the window staged in shared memory and reads the median from there, so the
+   two kernels need no scratch buffer besides `out` itself. */
+constexpr uint32_t HANDOVER_NONE = 0xFFFFFFFFu;
 
 struct MedianParams {
     const double* time;      /* may be null */
     const float* flux;
-    float* out;              /* median, NaN where the position has no trend */
+    float* out;              /* median, NaN where the position has no trend; or the packed hand-over words (above) */
     float* flat;             /* null, or flux / median (only set when the call stops after Phase 1) */
     float* scale;            /* null, or MAD of the window (selects the MAD variant of the kernel) */
-    uint16_t* nplus;         /* null, or n+ = number of window samples strictly above the median (Eq. 1, R7) */
+    int packed;              /* 1: write the hand-over word (median offset | n+ << 16) instead of the median value */
     int64_t N;               /* cadences per star */
     int64_t tiles_per_star;
     int64_t n_blocks;        /* n_stars * tiles_per_star */
@@ -63,17 +74,17 @@ struct MedianParams {
 struct ReweightParams {
     const double* time;
     const float* flux;
-    float* out;              /* in: median from the median kernel; out: trend */
+    float* out;              /* in: from the median kernel (hand-over words if `packed`, else medians); out: trend */
     float* flat;             /* null, or flux / trend (PAPER.md:155 normalisation), NaN where trend is NaN */
     const float* scale_in;   /* family kernels: null, or s per position (replaces Phase 2) */
     float* scale_out;        /* family kernels: null, or receives s per position */
-    const uint16_t* nplus;   /* null, or n+ per position from the median kernel: Phase 2 then only sums squares */
+    int packed;              /* 1: `out` holds hand-over words (the paper's path), 0: fp32 medians (sibling estimators) */
     int split;               /* reweighting kernel: 1, or K2_SPLIT for batches too small to fill the GPU */
     int weight_kind;         /* family kernels: WEIGHT_BISQUARE / WEIGHT_WELSCH */
     int scale_kind;          /* fused short-window kernel only */
     int64_t N;
-    int64_t tiles_per_star;
-    int64_t n_blocks;
+    int64_t tiles_per_star;  /* reweighting kernel: WARP tiles per star */
+    int64_t n_blocks;        /* n_stars * tiles_per_star */
     int W, n_iter;
     float alpha, c;
     float c_over_alpha;      /* c / alpha, formed on the host: the sentinel's distance factor ("Sentinel") */
@@ -83,11 +94,6 @@ struct ReweightParams {
 cudaError_t launch_median(const MedianParams& prm, unsigned grid, size_t smem, cudaStream_t stream);
 /* family = false: the paper's path (scale_in/scale_out/weight_kind ignored); true: the sibling-estimator variants */
 cudaError_t launch_reweight(const ReweightParams& prm, bool family, unsigned grid, size_t smem, cudaStream_t stream);
-/* umi_reweight_tc.cu: Phases 2-3 with the two sums of Eq. 4 on the tensor cores (tcgen05 / TMEM) */
-int tc_chunks(int W);
-size_t tc_smem_bytes(int W);
-int tc_tile();
-cudaError_t launch_reweight_tc(const ReweightParams& prm, unsigned grid, cudaStream_t stream);
 /* fused kernel for W <= KS_MAX_WINDOW; wt = compiled wire count (9, 17, 25, 33 or 49) >= W */
 cudaError_t launch_small(const ReweightParams& prm, bool family, int min_valid, int wt, unsigned grid, cudaStream_t stream);
 

@@ -382,12 +382,13 @@ umi_median_kernel(MedianParams prm)
                 /* emit position p (R4, R5) */
                 const bool own = rank[p + h] < nvu;
                 const bool has = own && n >= prm.min_valid && n > 0;
-                float m = __int_as_float(0x7FC00000);
-                if (has) m = key_to_float((uint32_t)(srt[rho] >> 32));
-                medbuf[p] = m;
-                if (!MAD && prm.nplus != nullptr) {                 /* for n+, counted after the walk (never asked of the MAD build) */
+                if (!MAD && prm.packed) {                           /* hand-over word, assembled after the walk (never asked of the MAD build) */
                     rhobuf[p] = has ? (uint16_t)rho : (uint16_t)0xFFFFu;
                     cntbuf[p] = (uint16_t)n;
+                } else {
+                    float m = __int_as_float(0x7FC00000);
+                    if (has) m = key_to_float((uint32_t)(srt[rho] >> 32));
+                    medbuf[p] = m;
                 }
                 if constexpr (MAD) sclbuf[p] = has ? mad : __int_as_float(0x7FC00000);
                 if (++p >= pend) break;
@@ -446,23 +447,28 @@ umi_median_kernel(MedianParams prm)
         __syncthreads();
 
         float* orow = prm.out + star * prm.N + j0;
-        for (int p = tid; p < Tact; p += K1_THREADS) orow[p] = medbuf[p];
-        if (!MAD && prm.nplus != nullptr) {
-            /* n+ of Eq. 1 (R7), all threads, off the walkers' serial chain: the n - 1 - (n-1)/2 members above
-               the median in rank, less those that tie with it in value (they follow it directly in sorted order) */
-            uint16_t* nrow = prm.nplus + star * prm.N + j0;
+        if (!MAD && prm.packed) {
+            /* Hand-over word for the reweighting kernel (umi_internal.h), all threads, off the walkers' serial
+               chain: where in its window the median sample sits (union index - position, 0 .. W-1), and n+ of
+               Eq. 1 (R7) = the n - 1 - (n-1)/2 members above the median in rank, less those that tie with it
+               in value (they follow it directly in sorted order). */
+            uint32_t* wrow = reinterpret_cast<uint32_t*>(orow);
             for (int p = tid; p < Tact; p += K1_THREADS) {
                 const int rho = rhobuf[p];
-                int np = 0;
+                uint32_t word = HANDOVER_NONE;
                 if (rho != 0xFFFF) {
                     const int n = cntbuf[p];
-                    const uint32_t kmed = (uint32_t)(srt[rho] >> 32);
-                    np = n - 1 - ((n - 1) >> 1);
+                    const uint64_t ent = srt[rho];
+                    const uint32_t kmed = (uint32_t)(ent >> 32);
+                    int np = n - 1 - ((n - 1) >> 1);
                     for (int r = rho + 1; r < nvu && (uint32_t)(srt[r] >> 32) == kmed; ++r)
                         np -= (((uint32_t)srt[r] - (uint32_t)p) < (uint32_t)W) ? 1 : 0;
+                    word = ((uint32_t)ent - (uint32_t)p) | ((uint32_t)np << 16);
                 }
-                nrow[p] = (uint16_t)np;
+                wrow[p] = word;
             }
+        } else {
+            for (int p = tid; p < Tact; p += K1_THREADS) orow[p] = medbuf[p];
         }
         if constexpr (MAD) {
             float* srow = prm.scale + star * prm.N + j0;

@@ -2,12 +2,20 @@
  * umi_reweight.cu -- Phase 2 + Phase 3 (Eq. 1-4): upper-RMS scale and
  * n_iter asymmetric Tukey-bisquare passes, starting from the Phase-1 median.
  *
- * CTA = one star x 512 positions; a thread owns 4 consecutive positions and streams
- * the W+3 samples they share from shared memory with one 128-bit load per 16
- * (sample, position) evaluations; all accumulators stay in registers, there are no
- * reductions.  Invalid samples are replaced in shared memory by a finite per-tile
- * sentinel far below the tile minimum, which Eq. 1 never counts and Eq. 3 always
- * gives weight 0, so the inner loop carries no validity predicate.
+ * Every WARP owns tiles of its own: 128 consecutive positions of one star, a thread owning 4
+ * consecutive positions.  The warp stages its tile and the W-1 halo into its private slice of
+ * shared memory, so the kernel has no CTA-wide barrier at all (__syncwarp only) and a warp whose
+ * tile lies in a gap does not hold the other three up.  A thread streams the W+3 samples its 4
+ * windows share with one 128-bit load per 16 (sample, position) evaluations; all accumulators stay
+ * in registers, there are no reductions.  Invalid samples are replaced in shared memory by a finite
+ * per-tile sentinel far below the tile minimum, which Eq. 1 never counts and Eq. 3 always gives
+ * weight 0, so the inner loop carries no validity predicate.
+ *
+ * What the median kernel hands over (umi_internal.h): one word per position = where in its window
+ * the median sample sits | n+ << 16.  The median is read from the staged samples, n+ (Eq. 1's
+ * count, exact on the sorted keys) leaves Phase 2 with a sum of squares only, and the staged
+ * samples are centred on the mid-range of the tile's MEDIANS -- a robust reference: one wild
+ * sample (a -9999 fill value, a 1e6 glitch) moves neither it nor the precision of the others.
  *
  * Inner loop: per (sample, position), on u' = -u
  *     u' = x*(-k) + mu*k            k = 1/(c s)
@@ -17,14 +25,10 @@
  *     n  = e*e - 1  (<= 0);  w = n*n;  S += w;  R += w*x'            Eq. 4: mu' <- R/S
  * The fma/mul/add steps run as sm_100a packed fp32x2 instructions (FFMA2/FMUL2/FADD2) on two
  * consecutive samples at a time; the edge groups use the scalar float form of the same arithmetic.
- * Phase 2 takes n+ from the median kernel when the launch provides it and then only sums squares.
  * Nothing here is shared with oracle/.
  */
 #include "umi_device.cuh"
 
-#ifndef UMI_K2_PACKED
-#define UMI_K2_PACKED 1
-#endif
 #ifndef UMI_K2_MIN_CTAS
 #define UMI_K2_MIN_CTAS 5
 #endif
@@ -79,7 +83,6 @@ __device__ __forceinline__ void eval_welsch(float x, float k, float c0, float na
     R = fmaf(w, x, R);
 }
 
-#if UMI_K2_PACKED
 /* Phase 3 on one 128-bit group: 4 samples (two fp32x2 pairs) x 4 positions = 8 pair
    evaluations, written stage by stage so that the 8 dependency chains interleave.
    kn2 = (-k, -k), cn2 = (mu k, mu k): the group works on u' = -u.  Exactly one of u' and
@@ -125,7 +128,6 @@ __device__ __forceinline__ void eval_weight_group(f32x2 x01, f32x2 x23, const f3
         R2[q] = ffma2(w2[2 * q + 1], x23, R2[q]);
     }
 }
-#endif
 
 } // namespace
 
@@ -141,28 +143,28 @@ template <int MODE, int SPLIT, int APOW>
 __global__ void __launch_bounds__(K2_THREADS, (APOW >= 0 && SPLIT == 1) ? UMI_K2_MIN_CTAS_POW2 : UMI_K2_MIN_CTAS)
 umi_reweight_kernel(ReweightParams prm)
 {
-    constexpr int TILE = K2_TILE / SPLIT;
+    constexpr int TILE = K2_WARP_TILE / SPLIT;          /* positions per warp tile */
     extern __shared__ __align__(16) unsigned char smem_raw[];
-    float* xs = reinterpret_cast<float*>(smem_raw);
-    __shared__ float s_red[2 * (K2_THREADS / 32)];
 
-    const int tid = threadIdx.x;
-    const int pt = tid / SPLIT;                         /* which 4 positions of the tile */
-    const int sl = tid % SPLIT;                         /* which slice of their windows */
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const int pt = lane / SPLIT;                        /* which 4 positions of the tile */
+    const int sl = lane % SPLIT;                        /* which slice of their windows */
     const int W = prm.W;
     const int h = (W - 1) >> 1;
     const int hal = (h + 3) & ~3;
     const int delta = hal - h;
     const int G = (3 + delta + 2 * h) / 4 + 1;          /* float4 groups per thread */
-    const int nx = TILE + 4 * G;                        /* staged floats */
+    const int nx = TILE + 4 * G;                        /* staged floats per warp (a multiple of 4) */
     const int g_lo = (3 + delta + 3) >> 2;              /* first group fully inside all 4 windows */
     const int g_hi = (delta + 2 * h - 3) >= 0 ? ((delta + 2 * h - 3) >> 2) : -1;   /* last such group */
     /* first interior group of this lane's slice: the smallest g >= g_lo with g = sl (mod SPLIT) */
     const int g_first = (SPLIT == 1) ? g_lo : g_lo + ((sl - g_lo % SPLIT) + SPLIT) % SPLIT;
     const float nalpha = -prm.alpha;
     const float qnan = __int_as_float(0x7FC00000);
+    float* xs = reinterpret_cast<float*>(smem_raw) + warp * nx;     /* this warp's slice */
 
-    for (int64_t bid = blockIdx.x; bid < prm.n_blocks; bid += gridDim.x) {
+    for (int64_t bid = (int64_t)blockIdx.x * K2_WARPS + warp; bid < prm.n_blocks; bid += (int64_t)gridDim.x * K2_WARPS) {
         const int64_t star = bid / prm.tiles_per_star;
         const int64_t tile = bid - star * prm.tiles_per_star;
         const int64_t j0 = tile * TILE;
@@ -174,23 +176,55 @@ umi_reweight_kernel(ReweightParams prm)
 
         /* stage the union, NaN marks invalid; tile min / max of the valid samples */
         float tmin = INFINITY, tmax = -INFINITY;
-        for (int u = tid; u < nx; u += K2_THREADS) {
+        for (int u = lane; u < nx; u += 32) {
             float x = 0.f;
             const bool ok = load_sample(trow, frow, prm.N, jbase + u, x);
             if (ok) { tmin = fminf(tmin, x); tmax = fmaxf(tmax, x); }
             xs[u] = ok ? x : qnan;
         }
+        __syncwarp();
+
+        /* per-position state: 4 consecutive positions, local index 4*pt + q.  The median: read from the staged
+           window at the offset the median kernel handed over (with n+), or an fp32 value (sibling estimators) */
+        float mu[K2_NPOS], kk[K2_NPOS], cs[K2_NPOS];
+        float nplus[K2_NPOS] = {0.f, 0.f, 0.f, 0.f};
+        bool act[K2_NPOS];
+        bool any_act = false;
+        unsigned has_med = 0u;                              /* bit q: position q has a median, i.e. a trend */
+        float mmin = INFINITY, mmax = -INFINITY;            /* range of the tile's medians */
+#pragma unroll
+        for (int q = 0; q < K2_NPOS; ++q) {
+            const int jl = 4 * pt + q;                      /* position inside the tile (32-bit from here on) */
+            float med = qnan;
+            if (jl < nrow) {
+                if (MODE == 0 || prm.packed) {
+                    const uint32_t word = reinterpret_cast<const uint32_t*>(otile)[jl];
+                    if (word != HANDOVER_NONE) {
+                        med = xs[jl + delta + (int)(word & 0xFFFFu)];   /* window of jl = staged [jl + delta, jl + delta + 2h] */
+                        nplus[q] = (float)(word >> 16);
+                    }
+                } else {
+                    med = otile[jl];
+                }
+            }
+            act[q] = (med == med);
+            has_med |= act[q] ? (1u << q) : 0u;
+            any_act = any_act || act[q];
+            mu[q] = act[q] ? med : 0.f;
+            if (act[q]) { mmin = fminf(mmin, med); mmax = fmaxf(mmax, med); }
+            kk[q] = 0.f;
+            cs[q] = 0.f;
+            if constexpr (MODE != 0) {                              /* no trend, no scale */
+                if (prm.scale_in == nullptr && prm.scale_out != nullptr && jl < nrow && !act[q] && sl == 0)
+                    prm.scale_out[star * prm.N + j0 + jl] = qnan;
+            }
+        }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) {
             tmin = fminf(tmin, __shfl_xor_sync(0xFFFFFFFFu, tmin, o));
             tmax = fmaxf(tmax, __shfl_xor_sync(0xFFFFFFFFu, tmax, o));
-        }
-        if ((tid & 31) == 0) { s_red[(tid >> 5) * 2] = tmin; s_red[(tid >> 5) * 2 + 1] = tmax; }
-        __syncthreads();
-#pragma unroll
-        for (int w = 0; w < K2_THREADS / 32; ++w) {
-            tmin = fminf(tmin, s_red[2 * w]);
-            tmax = fmaxf(tmax, s_red[2 * w + 1]);
+            mmin = fminf(mmin, __shfl_xor_sync(0xFFFFFFFFu, mmin, o));
+            mmax = fmaxf(mmax, __shfl_xor_sync(0xFFFFFFFFu, mmax, o));
         }
         /* sentinel: alpha*(mu - x)/(c s) >= 2 for every window of the tile, since
            mu >= tmin and s <= 0.6745 (tmax - tmin)  ("Sentinel") */
@@ -202,40 +236,21 @@ umi_reweight_kernel(ReweightParams prm)
                 sent = tmin - (MODE == 2 ? 24.f : 2.f) * prm.c_over_alpha * (tmax - tmin);
             sent = fmaxf(sent, -3.0e38f);
         }
-        /* everything below works on samples centred on the middle of the tile's range: Eq. 4 is then
-           mu' = sum(w x') / sum(w) with |x'| small, i.e. exact to fp32 without a separate sum of w*u */
-        const float xref = (tmin <= tmax) ? 0.5f * tmin + 0.5f * tmax : 0.f;
+        /* Everything below works on samples centred on the middle of the range of the tile's MEDIANS: Eq. 4 is
+           then mu' = sum(w x') / sum(w) with |x'| small for every sample that can carry weight, i.e. exact to
+           fp32 without a separate sum of w*u.  The medians are robust, so a wild sample (a fill value, a
+           glitch of any size) keeps its own magnitude and leaves the precision of the others alone. */
+        const float xref = (mmin <= mmax) ? 0.5f * mmin + 0.5f * mmax : 0.f;
         const float xabs = (tmin <= tmax) ? fmaxf(fabsf(sent - xref), fabsf(tmax - xref)) : 0.f;   /* max |x'| staged */
-        for (int u = tid; u < nx; u += K2_THREADS) {
+        __syncwarp();                                       /* every lane has read its medians from xs */
+        for (int u = lane; u < nx; u += 32) {
             const float x = xs[u];
             xs[u] = ((x != x) ? sent : x) - xref;
         }
-        __syncthreads();
-
-        /* per-position state: 4 consecutive positions, local index 4*tid + q */
-        float mu[K2_NPOS], kk[K2_NPOS], cs[K2_NPOS];
-        float nplus[K2_NPOS] = {0.f, 0.f, 0.f, 0.f};      /* n+ from the median kernel, when it was asked for one */
-        bool act[K2_NPOS];
-        bool any_act = false;
-        unsigned has_med = 0u;                              /* bit q: position q has a median, i.e. a trend */
 #pragma unroll
-        for (int q = 0; q < K2_NPOS; ++q) {
-            const int jl = 4 * pt + q;                      /* position inside the tile (32-bit from here on) */
-            const float med = (jl < nrow) ? otile[jl] - xref : qnan;
-            act[q] = (med == med);
-            has_med |= act[q] ? (1u << q) : 0u;
-            any_act = any_act || act[q];
-            mu[q] = act[q] ? med : 0.f;
-            if constexpr (MODE == 0) {
-                if (prm.nplus != nullptr) nplus[q] = (act[q] && jl < nrow) ? (float)prm.nplus[star * prm.N + j0 + jl] : 0.f;
-            }
-            kk[q] = 0.f;
-            cs[q] = 0.f;
-            if constexpr (MODE != 0) {                              /* no trend, no scale */
-                if (prm.scale_in == nullptr && prm.scale_out != nullptr && jl < nrow && !act[q])
-                    prm.scale_out[star * prm.N + j0 + jl] = qnan;
-            }
-        }
+        for (int q = 0; q < K2_NPOS; ++q) mu[q] = act[q] ? mu[q] - xref : 0.f;
+        __syncwarp();
+
         const float4* xs4 = reinterpret_cast<const float4*>(xs) + pt;
 
         if (__any_sync(0xFFFFFFFFu, any_act)) {
@@ -244,7 +259,7 @@ umi_reweight_kernel(ReweightParams prm)
 #pragma unroll
             for (int q = 0; q < K2_NPOS; ++q) { ss[q] = 0.f; cnt[q] = 0.f; }
             const bool given = (MODE != 0) && prm.scale_in != nullptr;
-            const bool counted = (MODE == 0) && UMI_K2_PACKED && prm.nplus != nullptr;   /* n+ already known */
+            const bool counted = (MODE == 0);               /* n+ came with the median */
             for (int g = sl; g < (given ? 0 : G); g += SPLIT) {
                 if (counted && g >= g_lo && g <= g_hi) {            /* interior groups: packed loop below */
                     if constexpr (SPLIT == 1) g = g_hi;
@@ -267,7 +282,6 @@ umi_reweight_kernel(ReweightParams prm)
                         }
                 }
             }
-#if UMI_K2_PACKED
             if (counted) {
                 /* With n+ known (the median kernel counts it exactly, on the sorted keys), Eq. 1 is a sum of
                    squares only: d = x - med on sample pairs (FADD2), max(d, 0) as a signed-integer maximum on
@@ -299,7 +313,6 @@ umi_reweight_kernel(ReweightParams prm)
                     ss[q] += s0 + s1;
                 }
             }
-#endif
             if constexpr (SPLIT > 1) {
 #pragma unroll
                 for (int q = 0; q < K2_NPOS; ++q)
@@ -347,7 +360,6 @@ umi_reweight_kernel(ReweightParams prm)
                 float S[K2_NPOS], R[K2_NPOS], c0[K2_NPOS];
 #pragma unroll
                 for (int q = 0; q < K2_NPOS; ++q) { S[q] = 0.f; R[q] = 0.f; c0[q] = -mu[q] * kk[q]; }
-#if UMI_K2_PACKED
                 f32x2 S2[K2_NPOS], R2[K2_NPOS], kn2[K2_NPOS], cn2[K2_NPOS];
                 const f32x2 nalpha2 = pack2(nalpha, nalpha);
 #pragma unroll
@@ -357,7 +369,6 @@ umi_reweight_kernel(ReweightParams prm)
                     kn2[q] = pack2(-kk[q], -kk[q]);                 /* exact negations: u' = -u bit for bit */
                     cn2[q] = pack2(-c0[q], -c0[q]);
                 }
-#endif
                 /* edge groups: samples that belong to some but not all of the 4 windows -- and, in the
                    alpha = 2^m builds, every group of a warp whose -u could overflow (`risky`, never seen on
                    real data): this scalar loop forms alpha*u by a multiply */
@@ -390,9 +401,7 @@ umi_reweight_kernel(ReweightParams prm)
 #pragma unroll
                             for (int r = 0; r < 4; ++r) eval_welsch(xv[r], kk[q], c0[q], nalpha, S[q], R[q]);
                     }
-                } else {
-#if UMI_K2_PACKED
-                if constexpr (APOW >= 0) {
+                } else if constexpr (APOW >= 0) {
                     if (!risky) {
 #pragma unroll K2_UNROLL_POW2
                         for (int g = g_first; g <= g_hi; g += SPLIT) {
@@ -407,21 +416,8 @@ umi_reweight_kernel(ReweightParams prm)
                         eval_weight_group<-1>(v2.x, v2.y, kn2, cn2, nalpha2, S2, R2);
                     }
                 }
-#else
-#pragma unroll 2
-                for (int g = g_first; g <= g_hi; g += SPLIT) {
-                    const float4 v = xs4[g];
-                    const float xv[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-                    for (int q = 0; q < K2_NPOS; ++q)
-#pragma unroll
-                        for (int r = 0; r < 4; ++r) eval_weight(xv[r], kk[q], c0[q], nalpha, S[q], R[q]);
-                }
-#endif
-                }
 #pragma unroll
                 for (int q = 0; q < K2_NPOS; ++q) {
-#if UMI_K2_PACKED
                     if constexpr (MODE != 2) {
                         float s0, s1, r0, r1;
                         unpack2(S2[q], s0, s1);
@@ -429,7 +425,6 @@ umi_reweight_kernel(ReweightParams prm)
                         S[q] += s0 + s1;
                         R[q] += r0 + r1;
                     }
-#endif
                     if constexpr (SPLIT > 1) {
 #pragma unroll
                         for (int o = SPLIT / 2; o > 0; o >>= 1) {
@@ -442,37 +437,38 @@ umi_reweight_kernel(ReweightParams prm)
             }
         }
 
+        /* the trend; with n_iter = 0 (sibling estimators asked for the scale only) `out` keeps the median
+           the selection kernel wrote, bit for bit */
+        float* flrow = prm.flat != nullptr ? prm.flat + star * prm.N + j0 : nullptr;
 #pragma unroll
         for (int q = 0; q < K2_NPOS; ++q) {
             const int jl = 4 * pt + q;
-            if (jl < nrow && ((has_med >> q) & 1u) && sl == 0) otile[jl] = mu[q] + xref;
-        }
-        if (prm.flat != nullptr) {                                  /* PAPER.md:155 normalisation */
-            float* flrow = prm.flat + star * prm.N + j0;
-#pragma unroll
-            for (int q = 0; q < K2_NPOS; ++q) {
-                const int jl = 4 * pt + q;
-                /* own sample = staged index hal + 4*tid + q (valid whenever the median is not NaN) */
-                if (jl < nrow && sl == 0) flrow[jl] = ((has_med >> q) & 1u) ? __ldg(frow + j0 + jl) / (mu[q] + xref) : qnan;
+            if (jl < nrow && sl == 0) {
+                const bool has = (has_med >> q) & 1u;
+                float tr = mu[q] + xref;
+                if (MODE != 0 && prm.n_iter == 0) tr = otile[jl];
+                else otile[jl] = has ? tr : qnan;
+                if (flrow != nullptr)                               /* PAPER.md:155 normalisation */
+                    flrow[jl] = has ? __ldg(frow + j0 + jl) / tr : qnan;
             }
         }
-        __syncthreads();
+        __syncwarp();                                       /* the slice is free for the next tile */
     }
 }
 
 cudaError_t launch_reweight(const ReweightParams& prm, bool family, unsigned grid, size_t smem, cudaStream_t stream)
 {
     const int ap = alpha_pow2(prm.alpha);
-    if (!family && prm.split == K2_SPLIT) {
-        if (ap == 1) umi_reweight_kernel<0, K2_SPLIT, 1><<<grid, K2_THREADS, smem, stream>>>(prm);
-        else umi_reweight_kernel<0, K2_SPLIT, -1><<<grid, K2_THREADS, smem, stream>>>(prm);
-    } else if (!family) {
-        if (ap == 0) umi_reweight_kernel<0, 1, 0><<<grid, K2_THREADS, smem, stream>>>(prm);
-        else if (ap == 1) umi_reweight_kernel<0, 1, 1><<<grid, K2_THREADS, smem, stream>>>(prm);
-        else if (ap == 2) umi_reweight_kernel<0, 1, 2><<<grid, K2_THREADS, smem, stream>>>(prm);
-        else umi_reweight_kernel<0, 1, -1><<<grid, K2_THREADS, smem, stream>>>(prm);
-    } else if (prm.weight_kind == WEIGHT_WELSCH) umi_reweight_kernel<2, 1, -1><<<grid, K2_THREADS, smem, stream>>>(prm);
-    else umi_reweight_kernel<1, 1, -1><<<grid, K2_THREADS, smem, stream>>>(prm);
+    void (*k2)(ReweightParams) = nullptr;
+    if (!family && prm.split == K2_SPLIT) k2 = (ap == 1) ? umi_reweight_kernel<0, K2_SPLIT, 1> : umi_reweight_kernel<0, K2_SPLIT, -1>;
+    else if (!family) k2 = (ap == 0) ? umi_reweight_kernel<0, 1, 0> : (ap == 1) ? umi_reweight_kernel<0, 1, 1>
+                         : (ap == 2) ? umi_reweight_kernel<0, 1, 2> : umi_reweight_kernel<0, 1, -1>;
+    else k2 = (prm.weight_kind == WEIGHT_WELSCH) ? umi_reweight_kernel<2, 1, -1> : umi_reweight_kernel<1, 1, -1>;
+    if (smem > 48 * 1024) {               /* W > ~2900: four warp slices of W + 131 floats pass the default limit */
+        const cudaError_t e = cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e != cudaSuccess) return e;
+    }
+    k2<<<grid, K2_THREADS, smem, stream>>>(prm);
     return cudaGetLastError();
 }
 
