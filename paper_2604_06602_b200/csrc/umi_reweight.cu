@@ -163,6 +163,8 @@ umi_reweight_kernel(ReweightParams prm)
     const float nalpha = -prm.alpha;
     const float qnan = __int_as_float(0x7FC00000);
     float* xs = reinterpret_cast<float*>(smem_raw) + warp * nx;     /* this warp's slice */
+    const bool vec = (prm.N & 3) == 0 && (reinterpret_cast<uintptr_t>(prm.flux) & 15) == 0 &&
+                     (reinterpret_cast<uintptr_t>(prm.time) & 15) == 0;
 
     for (int64_t bid = (int64_t)blockIdx.x * K2_WARPS + warp; bid < prm.n_blocks; bid += (int64_t)gridDim.x * K2_WARPS) {
         const int64_t star = bid / prm.tiles_per_star;
@@ -174,13 +176,50 @@ umi_reweight_kernel(ReweightParams prm)
         float* otile = prm.out + star * prm.N + j0;          /* the tile's TILE positions of the output row */
         const int nrow = (int)((prm.N - j0 < TILE) ? prm.N - j0 : TILE);   /* positions of the tile inside the row */
 
-        /* stage the union, NaN marks invalid; tile min / max of the valid samples */
+        /* stage the union, NaN marks invalid; tile min / max of the valid samples.  jbase is a multiple of 4, so
+           when the rows are 16-byte aligned (vec: N % 4 == 0 and aligned base pointers) a lane moves four samples
+           with one 128-bit load (two for an fp64 time), all of a round's loads in flight before the first use;
+           otherwise one 32-bit load per sample, four in flight */
         float tmin = INFINITY, tmax = -INFINITY;
-        for (int u = lane; u < nx; u += 32) {
-            float x = 0.f;
-            const bool ok = load_sample(trow, frow, prm.N, jbase + u, x);
-            if (ok) { tmin = fminf(tmin, x); tmax = fmaxf(tmax, x); }
-            xs[u] = ok ? x : qnan;
+        if (vec) {
+            for (int u = 4 * lane; u < nx; u += 128) {
+                const int64_t j = jbase + u;
+                float4 v = make_float4(qnan, qnan, qnan, qnan);
+                if (j >= 0 && j < prm.N) {                  /* a group of 4 lies entirely inside or outside the row */
+                    v = __ldg(reinterpret_cast<const float4*>(frow + j));
+                    bool t0 = true, t1 = true, t2 = true, t3 = true;
+                    if (trow != nullptr) {
+                        const double2 ta = __ldg(reinterpret_cast<const double2*>(trow + j));
+                        const double2 tb = __ldg(reinterpret_cast<const double2*>(trow + j + 2));
+                        t0 = finite_f64(ta.x); t1 = finite_f64(ta.y); t2 = finite_f64(tb.x); t3 = finite_f64(tb.y);
+                    }
+                    v.x = (t0 && finite_f32(v.x)) ? v.x : qnan;
+                    v.y = (t1 && finite_f32(v.y)) ? v.y : qnan;
+                    v.z = (t2 && finite_f32(v.z)) ? v.z : qnan;
+                    v.w = (t3 && finite_f32(v.w)) ? v.w : qnan;
+                    tmin = fminf(tmin, fminf(fminf(v.x, v.y), fminf(v.z, v.w)));     /* fminf / fmaxf skip NaN */
+                    tmax = fmaxf(tmax, fmaxf(fmaxf(v.x, v.y), fmaxf(v.z, v.w)));
+                }
+                *reinterpret_cast<float4*>(xs + u) = v;
+            }
+        } else {
+            for (int u0 = 0; u0 < nx; u0 += 128) {
+                float xv[4];
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const int u = u0 + 32 * r + lane;
+                    float x = 0.f;
+                    const bool ok = u < nx && load_sample(trow, frow, prm.N, jbase + u, x);
+                    xv[r] = ok ? x : qnan;
+                }
+#pragma unroll
+                for (int r = 0; r < 4; ++r) {
+                    const int u = u0 + 32 * r + lane;
+                    tmin = fminf(tmin, xv[r]);
+                    tmax = fmaxf(tmax, xv[r]);
+                    if (u < nx) xs[u] = xv[r];
+                }
+            }
         }
         __syncwarp();
 

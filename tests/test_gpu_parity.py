@@ -264,12 +264,19 @@ def test_wild_samples_cost_the_others_no_precision(umi, n_stars, W):
     for b in range(n_stars):
         for val in (-9999.0, -1.0e6, 1.0e5):
             x[b, rng.integers(0, 2100, 3)] = val
-    rep = _both(umi, x, W)
-    assert rep.max_rel <= 1e-6          # measured ~1e-7: the outliers are invisible to the inliers
+    _both(umi, x, W)                                    # the 1e-5 bar everywhere, wild windows included
+    # tighter where the wild samples carry no weight (trend next to the inliers): the error must be what it is
+    # on clean data, ~1e-7.  (A window holding both a +1e5 spike and a -9999 gives the latter a weight of ~0.8
+    # on a scale of ~2e4: its trend is a cancellation between 1 and -9999, where 1e-6 is fp32's own limit.)
+    ref = orc.detrend(x, W)
+    got = _gpu(umi, x, W).astype(np.float64)
+    calm = np.isfinite(ref.trend64) & (np.abs(ref.trend64 - 1.0) < 0.1) & ~ref.near_cutoff.astype(bool)
+    assert calm.sum() > 0.5 * x.size
+    assert (np.abs(got[calm] - ref.trend64[calm]) <= 5e-7 * np.abs(ref.trend64[calm])).all()
     # deepening below-median samples leaves the scale, hence the trend, where it was (reading G2)
     y = x.copy()
     y[y < -100.0] *= 1.0e20
-    got_x, got_y = _gpu(umi, x, W), _gpu(umi, y, W)
+    got_x, got_y = got.astype(np.float32), _gpu(umi, y, W)
     keep = np.isfinite(got_x) & (np.abs(x) < 100.0)
     assert np.allclose(got_x[keep], got_y[keep], rtol=2e-6, atol=0.0)
 
