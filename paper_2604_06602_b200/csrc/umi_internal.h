@@ -48,7 +48,10 @@ constexpr int K2_WARPS = K2_THREADS / 32;        /* every warp owns tiles of its
 constexpr int K2_NPOS = 4;                       /* consecutive positions per thread */
 constexpr int K2_WARP_TILE = 32 * K2_NPOS;       /* positions per warp tile (throughput variant) */
 constexpr int K2_TILE = K2_THREADS * K2_NPOS;    /* positions per CTA and trip of its tile loop */
-constexpr int K2_SPLIT = 8;                      /* small batches: lanes per 4 positions (warp tile = K2_WARP_TILE / K2_SPLIT) */
+#ifndef UMI_K2_SPLIT
+#define UMI_K2_SPLIT 8
+#endif
+constexpr int K2_SPLIT = UMI_K2_SPLIT;                    /* small batches: lanes per 4 positions (warp tile = K2_WARP_TILE / K2_SPLIT) */
 
 /* What the median kernel leaves in `out` for the reweighting kernel when passes follow (the paper's path):
    one 32-bit word per position, 0xFFFFFFFF = no trend here (R4, R5), else

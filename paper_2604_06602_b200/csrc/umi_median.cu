@@ -150,6 +150,8 @@ umi_median_kernel(MedianParams prm)
     const int tid = threadIdx.x;
     const int lane = tid & 31;
 
+    pdl_launch_dependents();        /* the reweighting kernel may be scheduled once every CTA of this grid has started */
+
     for (int64_t bid = blockIdx.x; bid < prm.n_blocks; bid += gridDim.x) {
         const int64_t star = bid / prm.tiles_per_star;
         const int64_t tile = bid - star * prm.tiles_per_star;

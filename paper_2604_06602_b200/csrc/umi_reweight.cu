@@ -38,16 +38,12 @@
 #ifndef UMI_K2_UNROLL
 #define UMI_K2_UNROLL 8
 #endif
-#ifndef UMI_K2_UNROLL_POW2
-#define UMI_K2_UNROLL_POW2 8
-#endif
 
 namespace umi {
 
 namespace {
 
 constexpr int K2_UNROLL = UMI_K2_UNROLL;
-constexpr int K2_UNROLL_POW2 = UMI_K2_UNROLL_POW2;
 
 /* Phase 2, Eq. 1: strictly-above-median residuals (R7). */
 __device__ __forceinline__ void eval_scale(float x, float med, float& ss, float& cnt)
@@ -84,7 +80,9 @@ __device__ __forceinline__ void eval_welsch(float x, float k, float c0, float na
 }
 
 /* Phase 3 on one 128-bit group: 4 samples (two fp32x2 pairs) x 4 positions = 8 pair
-   evaluations, written stage by stage so that the 8 dependency chains interleave.
+   evaluations, written stage by stage so that the 8 dependency chains interleave.  x01[q], x23[q]: the group's
+   two sample pairs as position q sees them (all four the same in an interior group; in an edge group the
+   samples outside window q are replaced by the sentinel, whose weight is exactly 0).
    kn2 = (-k, -k), cn2 = (mu k, mu k): the group works on u' = -u.  Exactly one of u' and
    alpha*u = -alpha*u' is <= 0, and it is -|u_eff| of Eq. 2; as signed integers a non-positive float
    sorts below every positive one, and among non-positive floats the larger magnitude is the larger
@@ -93,15 +91,15 @@ __device__ __forceinline__ void eval_welsch(float x, float k, float c0, float na
    (was: FMNMX for |u_eff| and a second FMNMX for the clamp).  1 - min(|u_eff|,1)^2 is then >= 0
    by construction, and bitwise the value max(1 - u_eff^2, 0) had. */
 template <int APOW>
-__device__ __forceinline__ void eval_weight_group(f32x2 x01, f32x2 x23, const f32x2 (&kn2)[K2_NPOS],
-                                                  const f32x2 (&cn2)[K2_NPOS], f32x2 nalpha2,
+__device__ __forceinline__ void eval_weight_group(const f32x2 (&x01)[K2_NPOS], const f32x2 (&x23)[K2_NPOS],
+                                                  const f32x2 (&kn2)[K2_NPOS], const f32x2 (&cn2)[K2_NPOS], f32x2 nalpha2,
                                                   f32x2 (&S2)[K2_NPOS], f32x2 (&R2)[K2_NPOS])
 {
     f32x2 a2[2 * K2_NPOS], w2[2 * K2_NPOS];
 #pragma unroll
     for (int q = 0; q < K2_NPOS; ++q) {
-        a2[2 * q] = ffma2(x01, kn2[q], cn2[q]);                    /* -u */
-        a2[2 * q + 1] = ffma2(x23, kn2[q], cn2[q]);
+        a2[2 * q] = ffma2(x01[q], kn2[q], cn2[q]);                 /* -u */
+        a2[2 * q + 1] = ffma2(x23[q], kn2[q], cn2[q]);
     }
     const f32x2 mone2 = pack2(-1.f, -1.f);
 #pragma unroll
@@ -123,9 +121,29 @@ __device__ __forceinline__ void eval_weight_group(f32x2 x01, f32x2 x23, const f3
 #pragma unroll
     for (int q = 0; q < K2_NPOS; ++q) {
         S2[q] = fadd2(S2[q], fadd2(w2[2 * q], w2[2 * q + 1]));
-        /* sum w x on the sample pairs themselves (shared by the 4 positions), so that u need not stay live */
-        R2[q] = ffma2(w2[2 * q], x01, R2[q]);
-        R2[q] = ffma2(w2[2 * q + 1], x23, R2[q]);
+        /* sum w x on the sample pairs themselves (shared by the 4 positions in an interior group), so that u need not stay live */
+        R2[q] = ffma2(w2[2 * q], x01[q], R2[q]);
+        R2[q] = ffma2(w2[2 * q + 1], x23[q], R2[q]);
+    }
+}
+
+/* Phase 2 with n+ known (the median kernel counts it exactly, on the sorted keys): Eq. 1 is a sum of squares only.
+   d = x - med on sample pairs (FADD2), max(d, 0) as a signed-integer maximum on the ALU pipe, ss += d*d (FFMA2):
+   two FMA-pipe lane-operations and one ALU instruction per sample. */
+__device__ __forceinline__ void eval_scale_group(const f32x2 (&x01)[K2_NPOS], const f32x2 (&x23)[K2_NPOS],
+                                                 const f32x2 (&nmed2)[K2_NPOS], f32x2 (&ss2)[K2_NPOS])
+{
+#pragma unroll
+    for (int q = 0; q < K2_NPOS; ++q) {
+#pragma unroll
+        for (int hh = 0; hh < 2; ++hh) {
+            const f32x2 d2 = fadd2(hh ? x23[q] : x01[q], nmed2[q]);
+            float d0, d1;
+            unpack2(d2, d0, d1);
+            const f32x2 p2 = pack2(__int_as_float(max(__float_as_int(d0), 0)),
+                                   __int_as_float(max(__float_as_int(d1), 0)));
+            ss2[q] = ffma2(p2, p2, ss2[q]);
+        }
     }
 }
 
@@ -222,6 +240,7 @@ umi_reweight_kernel(ReweightParams prm)
             }
         }
         __syncwarp();
+        pdl_wait_for_primary();                             /* the median kernel's words are complete and visible from here on */
 
         /* per-position state: 4 consecutive positions, local index 4*pt + q.  The median: read from the staged
            window at the offset the median kernel handed over (with n+), or an fp32 value (sibling estimators) */
@@ -280,11 +299,12 @@ umi_reweight_kernel(ReweightParams prm)
            fp32 without a separate sum of w*u.  The medians are robust, so a wild sample (a fill value, a
            glitch of any size) keeps its own magnitude and leaves the precision of the others alone. */
         const float xref = (mmin <= mmax) ? 0.5f * mmin + 0.5f * mmax : 0.f;
-        const float xabs = (tmin <= tmax) ? fmaxf(fabsf(sent - xref), fabsf(tmax - xref)) : 0.f;   /* max |x'| staged */
+        const float xsent = sent - xref;                    /* the sentinel as staged */
+        const float xabs = (tmin <= tmax) ? fmaxf(fabsf(xsent), fabsf(tmax - xref)) : 0.f;         /* max |x'| staged */
         __syncwarp();                                       /* every lane has read its medians from xs */
         for (int u = lane; u < nx; u += 32) {
             const float x = xs[u];
-            xs[u] = ((x != x) ? sent : x) - xref;
+            xs[u] = (x != x) ? xsent : x - xref;
         }
 #pragma unroll
         for (int q = 0; q < K2_NPOS; ++q) mu[q] = act[q] ? mu[q] - xref : 0.f;
@@ -293,55 +313,71 @@ umi_reweight_kernel(ReweightParams prm)
         const float4* xs4 = reinterpret_cast<const float4*>(xs) + pt;
 
         if (__any_sync(0xFFFFFFFFu, any_act)) {
+            /* Edge groups hold samples that belong to some but not all of the thread's 4 windows.  They run the
+               same packed arithmetic as the interior groups on MASKED samples: position q sees the (centred)
+               sentinel in place of a sample outside its window -- never above a median, weight exactly 0 -- so
+               no (sample, position) evaluation is predicated.  The lane's edge groups: g < g_lo and g > g_hi. */
+            /* Split-window variant: the lane's groups g = sl, sl + SPLIT, ... < G in three runs: [sl, g_first) low
+               edge groups; [g_first, g_tail) interior groups, a multiple of 8 of them, through the unrolled loop;
+               [g_tail, G) the rest -- up to 7 interior groups and the high edge groups -- through the same rolled,
+               masked loop as the low edge groups (one copy of that loop body). */
+            constexpr int UNR = K2_UNROLL;
+            int g_tail = g_first;
+            if (g_first <= g_hi) g_tail += ((g_hi - g_first) / SPLIT + 1) / UNR * (UNR * SPLIT);
+            const unsigned two_h = 2u * (unsigned)h;
+            auto masked_group = [&](int g, f32x2 (&x01)[K2_NPOS], f32x2 (&x23)[K2_NPOS]) {
+                const float4 v = xs4[g];
+#pragma unroll
+                for (int q = 0; q < K2_NPOS; ++q) {
+                    const int o = 4 * g - delta - q;                    /* offset of v.x inside window q */
+                    x01[q] = pack2((unsigned)o <= two_h ? v.x : xsent, (unsigned)(o + 1) <= two_h ? v.y : xsent);
+                    x23[q] = pack2((unsigned)(o + 2) <= two_h ? v.z : xsent, (unsigned)(o + 3) <= two_h ? v.w : xsent);
+                }
+            };
+            auto shared_group = [&](int g, f32x2 (&x01)[K2_NPOS], f32x2 (&x23)[K2_NPOS]) {
+                const ulonglong2 v2 = reinterpret_cast<const ulonglong2*>(xs4)[g];
+#pragma unroll
+                for (int q = 0; q < K2_NPOS; ++q) { x01[q] = v2.x; x23[q] = v2.y; }
+            };
+
             /* ---- Phase 2 (Eq. 1) ---- */
             float ss[K2_NPOS], cnt[K2_NPOS];
 #pragma unroll
             for (int q = 0; q < K2_NPOS; ++q) { ss[q] = 0.f; cnt[q] = 0.f; }
             const bool given = (MODE != 0) && prm.scale_in != nullptr;
-            const bool counted = (MODE == 0);               /* n+ came with the median */
-            for (int g = sl; g < (given ? 0 : G); g += SPLIT) {
-                if (counted && g >= g_lo && g <= g_hi) {            /* interior groups: packed loop below */
-                    if constexpr (SPLIT == 1) g = g_hi;
-                    continue;
-                }
-                const float4 v = xs4[g];
-                const float xv[4] = {v.x, v.y, v.z, v.w};
-                if (g >= g_lo && g <= g_hi) {
-#pragma unroll
-                    for (int q = 0; q < K2_NPOS; ++q)
-#pragma unroll
-                        for (int r = 0; r < 4; ++r) eval_scale(xv[r], mu[q], ss[q], cnt[q]);
-                } else {
-#pragma unroll
-                    for (int q = 0; q < K2_NPOS; ++q)
-#pragma unroll
-                        for (int r = 0; r < 4; ++r) {
-                            const int o = 4 * g + r - delta - q;
-                            if (o >= 0 && o <= 2 * h) eval_scale(xv[r], mu[q], ss[q], cnt[q]);
-                        }
-                }
-            }
-            if (counted) {
-                /* With n+ known (the median kernel counts it exactly, on the sorted keys), Eq. 1 is a sum of
-                   squares only: d = x - med on sample pairs (FADD2), max(d, 0) as a signed-integer maximum on
-                   the ALU pipe, ss += d*d (FFMA2).  Two FMA-pipe lane-operations and one ALU instruction per
-                   sample instead of three and one. */
-                f32x2 nmed2[K2_NPOS], ss2[K2_NPOS];
+            if constexpr (MODE == 0) {                              /* n+ came with the median: a sum of squares is left */
+                f32x2 nmed2[K2_NPOS], ss2[K2_NPOS], x01[K2_NPOS], x23[K2_NPOS];
 #pragma unroll
                 for (int q = 0; q < K2_NPOS; ++q) { nmed2[q] = pack2(-mu[q], -mu[q]); ss2[q] = pack2(0.f, 0.f); }
+                if constexpr (SPLIT == 1) {
+                    for (int g = 0; g < G; ++g) {                   /* edge groups, one (sample, position) at a time */
+                        if (g == g_lo && g_hi >= g_lo) g = g_hi + 1;
+                        if (g >= G) break;
+                        const float4 v = xs4[g];
+                        const float xv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                        for (int q = 0; q < K2_NPOS; ++q)
+#pragma unroll
+                            for (int r = 0; r < 4; ++r)
+                                if ((unsigned)(4 * g + r - delta - q) <= two_h) eval_scale(xv[r], mu[q], ss[q], cnt[q]);
+                    }
 #pragma unroll 8
-                for (int g = g_first; g <= g_hi; g += SPLIT) {
-                    const ulonglong2 v2 = reinterpret_cast<const ulonglong2*>(xs4)[g];
+                    for (int g = g_lo; g <= g_hi; ++g) {
+                        shared_group(g, x01, x23);
+                        eval_scale_group(x01, x23, nmed2, ss2);
+                    }
+                } else {
+                    for (int g = sl; g < G; g += SPLIT) {
+                        if (g == g_first) g = g_tail;
+                        if (g >= G) break;
+                        masked_group(g, x01, x23);
+                        eval_scale_group(x01, x23, nmed2, ss2);
+                    }
+                    for (int g0 = g_first; g0 < g_tail; g0 += UNR * SPLIT) {
 #pragma unroll
-                    for (int q = 0; q < K2_NPOS; ++q) {
-#pragma unroll
-                        for (int hh = 0; hh < 2; ++hh) {
-                            const f32x2 d2 = fadd2(hh ? v2.y : v2.x, nmed2[q]);
-                            float d0, d1;
-                            unpack2(d2, d0, d1);
-                            const f32x2 p2 = pack2(__int_as_float(max(__float_as_int(d0), 0)),
-                                                   __int_as_float(max(__float_as_int(d1), 0)));
-                            ss2[q] = ffma2(p2, p2, ss2[q]);
+                        for (int j = 0; j < UNR; ++j) {
+                            shared_group(g0 + j * SPLIT, x01, x23);
+                            eval_scale_group(x01, x23, nmed2, ss2);
                         }
                     }
                 }
@@ -351,6 +387,16 @@ umi_reweight_kernel(ReweightParams prm)
                     unpack2(ss2[q], s0, s1);
                     ss[q] += s0 + s1;
                 }
+            } else {                                                /* sibling estimators: count and sum, one sample at a time */
+                for (int g = sl; g < (given ? 0 : G); g += SPLIT) {
+                    const float4 v = xs4[g];
+                    const float xv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                    for (int q = 0; q < K2_NPOS; ++q)
+#pragma unroll
+                        for (int r = 0; r < 4; ++r)
+                            if ((unsigned)(4 * g + r - delta - q) <= two_h) eval_scale(xv[r], mu[q], ss[q], cnt[q]);
+                }
             }
             if constexpr (SPLIT > 1) {
 #pragma unroll
@@ -358,10 +404,10 @@ umi_reweight_kernel(ReweightParams prm)
 #pragma unroll
                     for (int o = SPLIT / 2; o > 0; o >>= 1) {
                         ss[q] += __shfl_xor_sync(0xFFFFFFFFu, ss[q], o);
-                        cnt[q] += __shfl_xor_sync(0xFFFFFFFFu, cnt[q], o);
+                        if constexpr (MODE != 0) cnt[q] += __shfl_xor_sync(0xFFFFFFFFu, cnt[q], o);
                     }
             }
-            if (counted) {
+            if constexpr (MODE == 0) {
 #pragma unroll
                 for (int q = 0; q < K2_NPOS; ++q) cnt[q] = nplus[q];
             }
@@ -387,19 +433,19 @@ umi_reweight_kernel(ReweightParams prm)
                 kk[q] = on ? 1.f / cs[q] : 0.f;
             }
 
-            /* alpha = 2^APOW loop only where -u = k (mu' - x') cannot overflow: |x'|, |mu'| <= xabs */
+            /* the packed loops form -u = k (mu' - x') without a guard, and the alpha = 2^APOW form of alpha*u would
+               wrap an overflowed -u to a small value: warps in which it could overflow (|x'|, |mu'| <= xabs; never
+               seen on real data) run every group through the scalar loop, which multiplies and predicates */
             bool risky = false;
-            if constexpr (APOW >= 0) {
 #pragma unroll
-                for (int q = 0; q < K2_NPOS; ++q) risky = risky || !(kk[q] * xabs < 1.2676506e30f);   /* 2^100 */
-                risky = __any_sync(0xFFFFFFFFu, risky);
-            }
+            for (int q = 0; q < K2_NPOS; ++q) risky = risky || !(kk[q] * xabs < 1.2676506e30f);   /* 2^100 */
+            risky = __any_sync(0xFFFFFFFFu, risky);
             /* ---- Phase 3 (Eq. 2-4), s held fixed (R9), exactly n_iter passes (R10) ---- */
             for (int it = 0; it < prm.n_iter; ++it) {
                 float S[K2_NPOS], R[K2_NPOS], c0[K2_NPOS];
 #pragma unroll
                 for (int q = 0; q < K2_NPOS; ++q) { S[q] = 0.f; R[q] = 0.f; c0[q] = -mu[q] * kk[q]; }
-                f32x2 S2[K2_NPOS], R2[K2_NPOS], kn2[K2_NPOS], cn2[K2_NPOS];
+                f32x2 S2[K2_NPOS], R2[K2_NPOS], kn2[K2_NPOS], cn2[K2_NPOS], x01[K2_NPOS], x23[K2_NPOS];
                 const f32x2 nalpha2 = pack2(nalpha, nalpha);
 #pragma unroll
                 for (int q = 0; q < K2_NPOS; ++q) {
@@ -408,62 +454,67 @@ umi_reweight_kernel(ReweightParams prm)
                     kn2[q] = pack2(-kk[q], -kk[q]);                 /* exact negations: u' = -u bit for bit */
                     cn2[q] = pack2(-c0[q], -c0[q]);
                 }
-                /* edge groups: samples that belong to some but not all of the 4 windows -- and, in the
-                   alpha = 2^m builds, every group of a warp whose -u could overflow (`risky`, never seen on
-                   real data): this scalar loop forms alpha*u by a multiply */
-                for (int g = sl; g < G; g += SPLIT) {
-                    if (!(APOW >= 0 && risky) && g >= g_lo && g <= g_hi) {
-                        if constexpr (SPLIT == 1) g = g_hi;
-                        continue;
-                    }
-                    const float4 v = xs4[g];
-                    const float xv[4] = {v.x, v.y, v.z, v.w};
-#pragma unroll
-                    for (int q = 0; q < K2_NPOS; ++q)
-#pragma unroll
-                        for (int r = 0; r < 4; ++r) {
-                            const int o = 4 * g + r - delta - q;
-                            if (o >= 0 && o <= 2 * h) {
-                                if constexpr (MODE == 2) eval_welsch(xv[r], kk[q], c0[q], nalpha, S[q], R[q]);
-                                else eval_weight(xv[r], kk[q], c0[q], nalpha, S[q], R[q]);
-                            }
+                const bool scalar_all = (MODE == 2) || risky;
+                if (SPLIT == 1 || scalar_all) {
+                    /* one (sample, position) at a time, predicated: every group of a Welsch or `risky` warp; in the
+                       throughput variant also the two or three edge groups (measured against the masked form
+                       below: 6.95 vs 7.00 ms at W = 361, 53.1 vs 54.9 at W = 217, 46.9 vs 47.3 at W = 2161 -- a
+                       second packed loop body costs more in instruction cache than it saves in issue slots) */
+                    for (int g = sl; g < G; g += SPLIT) {
+                        if (!scalar_all && g >= g_lo && g <= g_hi) {
+                            g = g_hi;                               /* (SPLIT == 1 here) */
+                            continue;
                         }
-                }
-                /* interior groups: every sample belongs to all 4 windows */
-                if constexpr (MODE == 2) {
-#pragma unroll 2
-                    for (int g = g_first; g <= g_hi; g += SPLIT) {
                         const float4 v = xs4[g];
                         const float xv[4] = {v.x, v.y, v.z, v.w};
 #pragma unroll
                         for (int q = 0; q < K2_NPOS; ++q)
 #pragma unroll
-                            for (int r = 0; r < 4; ++r) eval_welsch(xv[r], kk[q], c0[q], nalpha, S[q], R[q]);
+                            for (int r = 0; r < 4; ++r)
+                                if ((unsigned)(4 * g + r - delta - q) <= two_h) {
+                                    if constexpr (MODE == 2) eval_welsch(xv[r], kk[q], c0[q], nalpha, S[q], R[q]);
+                                    else eval_weight(xv[r], kk[q], c0[q], nalpha, S[q], R[q]);
+                                }
                     }
-                } else if constexpr (APOW >= 0) {
-                    if (!risky) {
-#pragma unroll K2_UNROLL_POW2
-                        for (int g = g_first; g <= g_hi; g += SPLIT) {
-                            const ulonglong2 v2 = reinterpret_cast<const ulonglong2*>(xs4)[g];
-                            eval_weight_group<APOW>(v2.x, v2.y, kn2, cn2, nalpha2, S2, R2);
-                        }
-                    }
-                } else {
+                }
+                if constexpr (MODE != 2) {
+                    if (!scalar_all) {
+                        if constexpr (SPLIT == 1) {
 #pragma unroll K2_UNROLL
-                    for (int g = g_first; g <= g_hi; g += SPLIT) {
-                        const ulonglong2 v2 = reinterpret_cast<const ulonglong2*>(xs4)[g];
-                        eval_weight_group<-1>(v2.x, v2.y, kn2, cn2, nalpha2, S2, R2);
+                            for (int g = g_lo; g <= g_hi; ++g) {       /* interior groups: every sample belongs to all 4 windows */
+                                shared_group(g, x01, x23);
+                                eval_weight_group<APOW>(x01, x23, kn2, cn2, nalpha2, S2, R2);
+                            }
+                        } else {
+                            /* split-window variant: a lane has ~1/SPLIT of the groups, so the edge groups weigh SPLIT
+                               times more: masked, packed, in the rolled loop that also takes what the unrolled one
+                               leaves over (config 1: 30.7 -> 26.6 us) */
+                            for (int g = sl; g < G; g += SPLIT) {
+                                if (g == g_first) g = g_tail;
+                                if (g >= G) break;
+                                masked_group(g, x01, x23);
+                                eval_weight_group<APOW>(x01, x23, kn2, cn2, nalpha2, S2, R2);
+                            }
+                            for (int g0 = g_first; g0 < g_tail; g0 += UNR * SPLIT) {
+#pragma unroll
+                                for (int j = 0; j < UNR; ++j) {
+                                    shared_group(g0 + j * SPLIT, x01, x23);
+                                    eval_weight_group<APOW>(x01, x23, kn2, cn2, nalpha2, S2, R2);
+                                }
+                            }
+                        }
+#pragma unroll
+                        for (int q = 0; q < K2_NPOS; ++q) {
+                            float s0, s1, r0, r1;
+                            unpack2(S2[q], s0, s1);
+                            unpack2(R2[q], r0, r1);
+                            S[q] += s0 + s1;
+                            R[q] += r0 + r1;
+                        }
                     }
                 }
 #pragma unroll
                 for (int q = 0; q < K2_NPOS; ++q) {
-                    if constexpr (MODE != 2) {
-                        float s0, s1, r0, r1;
-                        unpack2(S2[q], s0, s1);
-                        unpack2(R2[q], r0, r1);
-                        S[q] += s0 + s1;
-                        R[q] += r0 + r1;
-                    }
                     if constexpr (SPLIT > 1) {
 #pragma unroll
                         for (int o = SPLIT / 2; o > 0; o >>= 1) {
@@ -507,7 +558,24 @@ cudaError_t launch_reweight(const ReweightParams& prm, bool family, unsigned gri
         const cudaError_t e = cudaFuncSetAttribute(k2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    k2<<<grid, K2_THREADS, smem, stream>>>(prm);
+    /* programmatic dependent launch behind the median kernel (umi_device.cuh): the prologue of this grid --
+       launch, staging of the samples -- overlaps the tail of that one */
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(grid);
+    cfg.blockDim = dim3(K2_THREADS);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = stream;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+#ifdef UMI_NO_PDL_WAIT
+    cfg.numAttrs = 0;
+#else
+    cfg.numAttrs = 1;
+#endif
+    const cudaError_t e = cudaLaunchKernelEx(&cfg, k2, prm);
+    if (e != cudaSuccess) return e;
     return cudaGetLastError();
 }
 
