@@ -103,7 +103,7 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.out = trend_out;
         rp.flat = flat_out;
         rp.N = n_cadences;
-        rp.tiles_per_star = (n_cadences + umi::KS_TILE - 1) / umi::KS_TILE;
+        rp.tiles_per_star = (n_cadences + umi::KS_WARP_TILE - 1) / umi::KS_WARP_TILE;
         rp.n_blocks = n_stars * rp.tiles_per_star;
         rp.W = W;
         rp.n_iter = n_iter;
@@ -117,7 +117,7 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         rp.weight_kind = fam.weight_kind;
         rp.scale_kind = fam.scale_kind;
         const int wt = W <= 9 ? 9 : W <= 17 ? 17 : W <= 25 ? 25 : W <= 33 ? 33 : 49;
-        const unsigned grid = (unsigned)std::min<int64_t>(rp.n_blocks, MAX_GRID);
+        const unsigned grid = (unsigned)std::min<int64_t>((rp.n_blocks + umi::KS_WARPS - 1) / umi::KS_WARPS, MAX_GRID);
         if (ev && (cuda_failed(cudaEventRecord(ev[0], stream)) || cuda_failed(cudaEventRecord(ev[1], stream))))
             return UMI_ERR_CUDA;
         if (cuda_failed(umi::launch_small(rp, fam.on, min_valid, wt, grid, stream))) return UMI_ERR_CUDA;

@@ -37,7 +37,8 @@ constexpr int SCALE_UPPER_RMS = 0, SCALE_MAD = 1;
 constexpr int WEIGHT_BISQUARE = 0, WEIGHT_WELSCH = 1;
 
 constexpr int KS_THREADS = 128;                  /* fused small-window kernel: 4 consecutive positions per thread */
-constexpr int KS_TILE = 4 * KS_THREADS;          /* positions per CTA */
+constexpr int KS_WARPS = KS_THREADS / 32;        /* every warp owns tiles of its own, as in the reweighting kernel */
+constexpr int KS_WARP_TILE = 128;                /* positions per warp tile */
 constexpr int KS_MAX_WINDOW = 49;                /* windows up to this length take the fused kernel */
 
 #ifndef UMI_K2_THREADS
@@ -97,7 +98,8 @@ struct ReweightParams {
 cudaError_t launch_median(const MedianParams& prm, unsigned grid, size_t smem, cudaStream_t stream);
 /* family = false: the paper's path (scale_in/scale_out/weight_kind ignored); true: the sibling-estimator variants */
 cudaError_t launch_reweight(const ReweightParams& prm, bool family, unsigned grid, size_t smem, cudaStream_t stream);
-/* fused kernel for W <= KS_MAX_WINDOW; wt = compiled wire count (9, 17, 25, 33 or 49) >= W */
+/* fused kernel for W <= KS_MAX_WINDOW; wt = compiled wire count (9, 17, 25, 33 or 49) >= W; prm.tiles_per_star and
+   prm.n_blocks count WARP tiles of KS_WARP_TILE positions, grid = CTAs of KS_WARPS warps */
 cudaError_t launch_small(const ReweightParams& prm, bool family, int min_valid, int wt, unsigned grid, cudaStream_t stream);
 
 /* umi_regrid.cu: gap handling by time stamps (R20) */
