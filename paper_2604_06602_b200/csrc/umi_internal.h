@@ -23,13 +23,13 @@ __host__ __device__ constexpr int k1_walkers(int ns) { return (UMI_K1_WALKER_BUD
 __host__ __device__ constexpr size_t k1_smem_bytes(int ns, bool mad = false, int t = 0)
 {
     /* u64 sorted entries + u16 ranks + max(rank bitsets [NW][NS/32+1] + scan offsets [NW/32][NS/32], f32 medians)
-       + u32 sorted keys */
+       + u32 sorted keys, one pad word per 32 */
     const size_t bw = (size_t)ns / 32, nw = (size_t)k1_walkers(ns);
     const size_t bits = 4 * (nw * (bw + 1) + (nw / 32) * bw);
     /* f32 medians [T], then u16 median ranks [T] and u16 window counts [T] (for n+ and the packed hand-over), rounded to 16 bytes */
     const size_t med = ((8 * (size_t)(t > 0 ? t : ns)) + 15) / 16 * 16;
     /* the MAD variant stages one more fp32 per position (the scale) behind everything else */
-    return (size_t)ns * 10 + (bits > med ? bits : med) + 4 * (size_t)ns + (mad ? 4 * (size_t)ns : 0);
+    return (size_t)ns * 10 + (bits > med ? bits : med) + 4 * ((size_t)ns + (size_t)ns / 32) + (mad ? 4 * (size_t)ns : 0);
 }
 
 /* sibling estimators; values match include/umi.h */

@@ -34,9 +34,54 @@ namespace {
    multiset, and the ranks of tied entries are assigned after the sort (see the kernel). */
 __device__ __forceinline__ void cmp_swap(uint32_t& a, uint32_t& b, bool up)
 {
-    const uint32_t mn = min(a, b), mx = max(a, b);
-    a = up ? mn : mx;
-    b = up ? mx : mn;
+    const uint32_t lo = up ? min(a, b) : max(a, b);                 /* one VIMNMX each: the direction is its predicate operand */
+    const uint32_t hi = up ? max(a, b) : min(a, b);
+    a = lo;
+    b = hi;
+}
+
+/* index of sorted key i in skey[]: one pad word per 32 keys, so that the probes of the rank search -- all at
+   i = -1 (mod 32) in its first steps -- fall into different banks (they were 75 % of the kernel's bank conflicts) */
+__device__ __forceinline__ int skey_at(int i) { return i + (i >> 5); }
+
+/* E consecutive slots of one star row starting at cadence j (j = 0 mod 4 when vec): keys, KEY_INVALID where invalid */
+template <int E>
+__device__ __forceinline__ int load_keys(const double* __restrict__ trow, const float* __restrict__ frow, int64_t N, int64_t j,
+                                         bool vec, uint32_t (&key)[E])
+{
+    int nvalid = 0;
+    if (vec) {
+#pragma unroll
+        for (int e = 0; e < E; e += 4) {
+            const int64_t jj = j + e;
+            float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+            bool in = jj >= 0 && jj < N;                            /* a group of 4 lies entirely inside or outside the row */
+            bool t0 = in, t1 = in, t2 = in, t3 = in;
+            if (in) {
+                v = __ldg(reinterpret_cast<const float4*>(frow + jj));
+                if (trow != nullptr) {
+                    const double2 ta = __ldg(reinterpret_cast<const double2*>(trow + jj));
+                    const double2 tb = __ldg(reinterpret_cast<const double2*>(trow + jj + 2));
+                    t0 = finite_f64(ta.x); t1 = finite_f64(ta.y); t2 = finite_f64(tb.x); t3 = finite_f64(tb.y);
+                }
+            }
+            t0 = t0 && finite_f32(v.x); t1 = t1 && finite_f32(v.y); t2 = t2 && finite_f32(v.z); t3 = t3 && finite_f32(v.w);
+            key[e] = t0 ? float_to_key(v.x) : KEY_INVALID;
+            key[e + 1] = t1 ? float_to_key(v.y) : KEY_INVALID;
+            key[e + 2] = t2 ? float_to_key(v.z) : KEY_INVALID;
+            key[e + 3] = t3 ? float_to_key(v.w) : KEY_INVALID;
+            nvalid += (int)t0 + (int)t1 + (int)t2 + (int)t3;
+        }
+    } else {
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+            float x = 0.f;
+            const bool ok = load_sample(trow, frow, N, j + e, x);
+            nvalid += ok ? 1 : 0;
+            key[e] = ok ? float_to_key(x) : KEY_INVALID;
+        }
+    }
+    return nvalid;
 }
 
 /* One bitonic stage (merge size K, stride J) on keys i = tid*E + e held in v[e] (blocked). */
@@ -118,7 +163,7 @@ struct MadRange {
 };
 
 template <int E, bool MAD>
-__global__ void __launch_bounds__(K1_THREADS, E == 4 ? 6 : 0)   /* NS = 1024: 6 CTAs/SM fit in shared memory, keep the registers at 40 */
+__global__ void __launch_bounds__(K1_THREADS, E == 4 ? 6 : E == 8 ? 5 : E == 16 ? 3 : 1)   /* as many CTAs per SM as their shared memory allows (NS = 1024: 6, 2048: 5, 4096: 3, 8192: 1) */
 umi_median_kernel(MedianParams prm)
 {
     constexpr int NS = K1_THREADS * E;
@@ -140,7 +185,7 @@ umi_median_kernel(MedianParams prm)
     float* medbuf = reinterpret_cast<float*>(bits);                 /* ... aliased: [T] medians of the tile */
     uint16_t* rhobuf = reinterpret_cast<uint16_t*>(medbuf + prm.T); /* ... [T] median ranks and [T] window counts behind them */
     uint16_t* cntbuf = rhobuf + prm.T;
-    uint32_t* skey = reinterpret_cast<uint32_t*>(smem_raw + k1_smem_bytes(NS, false, prm.T)) - NS;   /* [NS] sorted keys */
+    uint32_t* skey = reinterpret_cast<uint32_t*>(smem_raw + k1_smem_bytes(NS, false, prm.T)) - (NS + NS / 32);   /* [NS + NS/32] sorted keys, padded (skey_at) */
     float* sclbuf = reinterpret_cast<float*>(smem_raw + k1_smem_bytes(NS, false, prm.T));   /* MAD only: [T] scales */
     __shared__ int s_nvu;
 
@@ -149,6 +194,8 @@ umi_median_kernel(MedianParams prm)
     const int h = (W - 1) >> 1;
     const int tid = threadIdx.x;
     const int lane = tid & 31;
+    const bool rows_vec = (prm.N & 3) == 0 && (reinterpret_cast<uintptr_t>(prm.flux) & 15) == 0 &&
+                          (reinterpret_cast<uintptr_t>(prm.time) & 15) == 0;
 
     pdl_launch_dependents();        /* the reweighting kernel may be scheduled once every CTA of this grid has started */
 
@@ -168,14 +215,12 @@ umi_median_kernel(MedianParams prm)
 
         /* 1. load E consecutive union entries and sort their 32-bit keys */
         uint32_t v[E];
-        int nvalid = 0;
+        const bool vec = rows_vec && ((jbase + (int64_t)tid * E) & 3) == 0;
+        int nvalid = load_keys<E>(trow, frow, prm.N, jbase + (int64_t)tid * E, vec, v);
+        uint32_t own[E <= 8 ? E : 1];                               /* the entries' own keys, kept across the sort when they fit */
+        if constexpr (E <= 8) {
 #pragma unroll
-        for (int e = 0; e < E; ++e) {
-            const int u = tid * E + e;
-            float x = 0.f;
-            const bool ok = load_sample(trow, frow, prm.N, jbase + u, x);
-            nvalid += ok ? 1 : 0;
-            v[e] = ok ? float_to_key(x) : KEY_INVALID;
+            for (int e = 0; e < E; ++e) own[e] = v[e];
         }
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) nvalid += __shfl_xor_sync(0xFFFFFFFFu, nvalid, o);
@@ -184,25 +229,23 @@ umi_median_kernel(MedianParams prm)
         bitonic_sort_blocked<E>(v, reinterpret_cast<uint32_t*>(srt), tid);
 
 #pragma unroll
-        for (int e = 0; e < E; e += 4)
-            *reinterpret_cast<uint4*>(skey + tid * E + e) = make_uint4(v[e], v[e + 1], v[e + 2], v[e + 3]);
+        for (int e = 0; e < E; ++e) skey[skey_at(tid * E + e)] = v[e];
         __syncthreads();                                            /* also: every read of the exchange buffer is done */
 
         /* rank of every entry = lower bound of its key among the sorted keys + its turn among the entries
            with that key (a counter per key value, borrowed from the still all-zero bitset area and zeroed
            again below).  Tied entries carry the same value, so which of them gets which rank changes
            nothing that is computed from ranks.  Invalid entries get a rank above every valid one. */
+        if constexpr (E > 8) (void)load_keys<E>(trow, frow, prm.N, jbase + (int64_t)tid * E, vec, v);   /* the same words again (L1 / L2) */
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             const int u = tid * E + e;
-            float x = 0.f;
-            const bool ok = load_sample(trow, frow, prm.N, jbase + u, x);   /* the same words again (L1 / L2) */
-            if (ok) {
-                const uint32_t key = float_to_key(x);
+            const uint32_t key = (E <= 8) ? own[(E <= 8) ? e : 0] : v[e];
+            if (key != KEY_INVALID) {
                 int pos = 0;
 #pragma unroll
                 for (int step = NS / 2; step > 0; step >>= 1)
-                    pos += (skey[pos + step - 1] < key) ? step : 0;
+                    pos += (skey[skey_at(pos + step - 1)] < key) ? step : 0;
                 const int r = pos + (int)atomicAdd(&bits[pos], 1u);
                 v[e] = (uint32_t)pos;
                 rank[u] = (uint16_t)r;
