@@ -107,6 +107,46 @@ def detrend_gapped(time, flux, t0, dt, n_grid, W, alpha=2.0, n_iter=5, c=5.0, mi
     return trend, median
 
 
+def detrend_gapped_ex(time, flux, t0, dt, n_grid, W, alpha=2.0, n_iter=5, c=5.0, min_valid=None,
+                      break_slots=-1, min_segment=0, edge_cut=0):
+    """Brute force for the segmented gap handling (reading R23), written with whole-row masks and
+    np.split instead of the oracle's running counters: valid samples (as in detrend_gapped) are cut
+    where np.diff(slot) - 1 > break_slots, pieces shorter than min_segment are thrown away, a window
+    is the piece's samples within h slots, samples closer than edge_cut slots to a piece's end get NaN."""
+    time = np.atleast_2d(np.asarray(time, dtype=np.float64))
+    flux = np.atleast_2d(np.asarray(flux, dtype=np.float32))
+    S, M = flux.shape
+    h = (W - 1) // 2
+    if min_valid is None:
+        min_valid = max(1, W // 3)
+    trend = np.full((S, M), np.nan)
+    median = np.full((S, M), np.nan)
+    for b in range(S):
+        with np.errstate(invalid="ignore"):
+            k = np.rint((time[b] - t0) / dt)
+        ok = np.isfinite(time[b]) & (k >= 0) & (k < n_grid)
+        same_as_next = np.zeros(M, dtype=bool)
+        same_as_next[:-1] = np.isfinite(time[b, :-1]) & np.isfinite(time[b, 1:]) & (k[:-1] == k[1:])
+        ok &= ~same_as_next & np.isfinite(flux[b])
+        idx = np.flatnonzero(ok)
+        if idx.size == 0:
+            continue
+        ks = k[idx].astype(np.int64)
+        cuts = np.flatnonzero(np.diff(ks) - 1 > break_slots) + 1 if break_slots >= 0 else np.array([], dtype=np.int64)
+        for piece_idx, piece_k in zip(np.split(idx, cuts), np.split(ks, cuts)):
+            if piece_idx.size < min_segment:
+                continue
+            x_all = flux[b][piece_idx].astype(np.float64)
+            for i, ki in zip(piece_idx, piece_k):
+                if ki - piece_k[0] < edge_cut or piece_k[-1] - ki < edge_cut:
+                    continue
+                x = x_all[np.abs(piece_k - ki) <= h]
+                if x.size < min_valid:
+                    continue
+                trend[b, i], median[b, i], _ = location(x, alpha, c, n_iter)
+    return trend, median
+
+
 def location_family(x, scale_kind="upper_rms", weight_kind="bisquare", alpha=2.0, c=5.0, n_iter=5):
     """Sibling estimators (F4): scale_kind "mad" = np.median-style MAD (lower middle, R21),
     weight_kind "welsch" = exp(-u_eff^2) (R22).  Returns (mu, median, s)."""

@@ -401,6 +401,132 @@ int umi_oracle_gapped(const double *time, const float *flux,
 }
 
 /*
+ * Gap handling with segments (next row F2, second part; "gap handling", PAPER.md:192
+ * "minimum segment length ... W/3"; reading R23).  On top of umi_oracle_gapped (R20):
+ *   - the valid samples of a row, in order, are cut into SEGMENTS wherever more than break_slots
+ *     empty slots lie between two consecutive valid samples (break_slots < 0: never);
+ *   - a segment with fewer than min_segment valid samples is dropped: NaN out, in no window;
+ *   - the window of a sample holds samples of its OWN segment only (|slot difference| <= h);
+ *   - a sample whose slot lies less than edge_cut slots from the first or the last slot of its
+ *     segment gets NaN out, but still takes part in the windows of the others.
+ * break_slots < 0, min_segment <= 0, edge_cut <= 0 is umi_oracle_gapped.
+ */
+int umi_oracle_gapped_ex(const double *time, const float *flux,
+                         int64_t n_stars, int64_t n_samples,
+                         double t0, double dt, int64_t n_grid,
+                         int W, double alpha, double c, int n_iter, int min_valid,
+                         int64_t break_slots, int64_t min_segment, int64_t edge_cut,
+                         double cutoff_tol,
+                         double *trend64, float *trend32, float *median,
+                         double *scale, int32_t *n_valid, int32_t *n_plus,
+                         uint8_t *near_cutoff)
+{
+    if (!time || !flux || n_stars < 0 || n_samples < 0 || n_grid < 0 || W < 1 || (W & 1) == 0 ||
+        n_iter < 0 || !(alpha > 0.0) || !(c > 0.0) || !(dt > 0.0) || !isfinite(dt) || !isfinite(t0))
+        return 1;
+    const int mv = resolve_min_valid(W, min_valid);
+    const int64_t h = (W - 1) / 2;
+    const int64_t total = n_stars * n_samples;
+    const size_t cnt = (size_t)(total > 0 ? total : 1);
+    int64_t *slot = (int64_t *)malloc(cnt * sizeof(int64_t));   /* -1 = invalid */
+    int64_t *seg = (int64_t *)malloc(cnt * sizeof(int64_t));    /* segment number inside the row, -1 = none */
+    uint8_t *cut = (uint8_t *)malloc(cnt);                       /* 1 = inside the edge cut */
+    if (!slot || !seg || !cut) { free(slot); free(seg); free(cut); return 1; }
+    for (int64_t b = 0; b < n_stars; ++b) {
+        const double *trow = time + b * n_samples;
+        const float *frow = flux + b * n_samples;
+        int64_t *srow = slot + b * n_samples, *grow = seg + b * n_samples;
+        uint8_t *crow = cut + b * n_samples;
+        /* (R20) slot of every sample, as in umi_oracle_gapped */
+        for (int64_t i = 0; i < n_samples; ++i) {
+            srow[i] = -1;
+            if (!isfinite(trow[i])) continue;
+            double k = rint((trow[i] - t0) / dt);
+            if (!(k >= 0.0) || !(k < (double)n_grid)) continue;
+            srow[i] = (int64_t)k;
+        }
+        for (int64_t i = 0; i < n_samples; ++i) {
+            int64_t k = srow[i];
+            if (k >= 0 && i + 1 < n_samples && isfinite(trow[i + 1])) {
+                double kn = rint((trow[i + 1] - t0) / dt);
+                if (kn == (double)k) srow[i] = -1;
+            }
+        }
+        for (int64_t i = 0; i < n_samples; ++i)
+            if (!isfinite(frow[i])) srow[i] = -1;
+        /* (R23) segments: a new one starts after more than break_slots empty slots */
+        int64_t cur = -1, prev_slot = 0;
+        for (int64_t i = 0; i < n_samples; ++i) {
+            grow[i] = -1;
+            crow[i] = 0;
+            if (srow[i] < 0) continue;
+            if (cur < 0 || (break_slots >= 0 && srow[i] - prev_slot - 1 > break_slots)) ++cur;
+            grow[i] = cur;
+            prev_slot = srow[i];
+        }
+        /* per segment: count, first and last slot; short segments dropped, edges marked */
+        for (int64_t i = 0; i < n_samples;) {
+            if (grow[i] < 0) { ++i; continue; }
+            int64_t j = i, last = i, count = 0;
+            for (; j < n_samples; ++j) {
+                if (grow[j] < 0) continue;
+                if (grow[j] != grow[i]) break;
+                ++count;
+                last = j;
+            }
+            if (min_segment > 0 && count < min_segment) {
+                for (int64_t m = i; m <= last; ++m)
+                    if (grow[m] == grow[i]) { srow[m] = -1; }
+                for (int64_t m = i; m <= last; ++m)
+                    if (srow[m] < 0) grow[m] = -1;
+            } else if (edge_cut > 0) {
+                for (int64_t m = i; m <= last; ++m)
+                    if (grow[m] >= 0 && (srow[m] - srow[i] < edge_cut || srow[last] - srow[m] < edge_cut)) crow[m] = 1;
+            }
+            i = j;
+        }
+    }
+    int bad = 0;
+#pragma omp parallel
+    {
+        double *work = (double *)malloc((size_t)2 * (size_t)W * sizeof(double));
+#pragma omp for schedule(dynamic, 256)
+        for (int64_t q = 0; q < total; ++q) {
+            if (!work) {
+#pragma omp atomic write
+                bad = 1;
+                continue;
+            }
+            const int64_t b = q / n_samples, i = q % n_samples;
+            const float *frow = flux + b * n_samples;
+            const int64_t *srow = slot + b * n_samples, *grow = seg + b * n_samples;
+            const int64_t ki = srow[i];
+            int n = 0;
+            if (ki >= 0) {
+                for (int64_t j = i - h; j <= i + h; ++j) {
+                    if (j < 0 || j >= n_samples || srow[j] < 0 || grow[j] != grow[i]) continue;
+                    int64_t d = srow[j] - ki;
+                    if (d < 0) d = -d;
+                    if (d <= h) work[n++] = (double)frow[j];
+                }
+            }
+            if (n_valid) n_valid[q] = n;
+            double t64;
+            oracle_location(work, n, ki >= 0 && !cut[q], alpha, c, n_iter, mv, cutoff_tol, work + W,
+                            &t64, median ? median + q : NULL, scale ? scale + q : NULL,
+                            n_plus ? n_plus + q : NULL, near_cutoff ? near_cutoff + q : NULL);
+            if (trend64) trend64[q] = t64;
+            if (trend32) trend32[q] = (float)t64;
+        }
+        free(work);
+    }
+    free(slot);
+    free(seg);
+    free(cut);
+    return bad;
+}
+
+/*
  * Sibling estimators (F4): every position of every star with the chosen scale and weight.
  * scale_kind 0 / weight_kind 0 is umi_oracle_detrend.  n_plus is not produced for the MAD.
  */

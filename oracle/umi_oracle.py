@@ -70,6 +70,12 @@ def lib():
             ctypes.c_double, ctypes.c_double, ctypes.c_int64,
             ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
             ctypes.c_double] + outs
+        L.umi_oracle_gapped_ex.restype = ctypes.c_int
+        L.umi_oracle_gapped_ex.argtypes = [
+            _c_double_p, _c_float_p, ctypes.c_int64, ctypes.c_int64,
+            ctypes.c_double, ctypes.c_double, ctypes.c_int64,
+            ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
+            ctypes.c_int64, ctypes.c_int64, ctypes.c_int64, ctypes.c_double] + outs
         _lib = L
     return _lib
 
@@ -180,6 +186,25 @@ def gapped(time, flux, t0, dt, n_grid, W, alpha=2.0, n_iter=5, c=5.0, min_valid=
         int(W), float(alpha), float(c), int(n_iter), int(min_valid), float(cutoff_tol), *_out_ptrs(r))
     if rc != 0:
         raise ValueError("umi_oracle_gapped: invalid arguments")
+    return r
+
+
+def gapped_ex(time, flux, t0, dt, n_grid, W, alpha=2.0, n_iter=5, c=5.0, min_valid=-1,
+              break_slots=-1, min_segment=0, edge_cut=0, cutoff_tol=1e-5) -> OracleResult:
+    """gapped() with segments (reading R23): rows are cut where more than break_slots empty slots lie between
+    valid samples, segments shorter than min_segment are dropped, windows stay inside a segment, and samples
+    closer than edge_cut slots to a segment end get NaN."""
+    flux, time, tp = _prep(flux, time)
+    if tp is None:
+        raise ValueError("time is required")
+    S, M = flux.shape
+    r = _alloc((S, M))
+    rc = lib().umi_oracle_gapped_ex(
+        tp, flux.ctypes.data_as(_c_float_p), S, M, float(t0), float(dt), int(n_grid),
+        int(W), float(alpha), float(c), int(n_iter), int(min_valid),
+        int(break_slots), int(min_segment), int(edge_cut), float(cutoff_tol), *_out_ptrs(r))
+    if rc != 0:
+        raise ValueError("umi_oracle_gapped_ex: invalid arguments")
     return r
 
 

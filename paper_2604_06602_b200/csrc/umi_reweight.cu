@@ -454,9 +454,9 @@ umi_reweight_kernel(ReweightParams prm)
                     kn2[q] = pack2(-kk[q], -kk[q]);                 /* exact negations: u' = -u bit for bit */
                     cn2[q] = pack2(-c0[q], -c0[q]);
                 }
-                const bool scalar_all = (MODE == 2) || risky;
+                const bool scalar_all = risky;
                 if (SPLIT == 1 || scalar_all) {
-                    /* one (sample, position) at a time, predicated: every group of a Welsch or `risky` warp; in the
+                    /* one (sample, position) at a time, predicated: every group of a `risky` warp; in the
                        throughput variant also the two or three edge groups (measured against the masked form
                        below: 6.95 vs 7.00 ms at W = 361, 53.1 vs 54.9 at W = 217, 46.9 vs 47.3 at W = 2161 -- a
                        second packed loop body costs more in instruction cache than it saves in issue slots) */
@@ -477,7 +477,19 @@ umi_reweight_kernel(ReweightParams prm)
                                 }
                     }
                 }
-                if constexpr (MODE != 2) {
+                if constexpr (MODE == 2) {
+                    if (!scalar_all) {                              /* Welsch: MUFU-bound, one sample at a time */
+#pragma unroll 2
+                        for (int g = g_lo; g <= g_hi; ++g) {
+                            const float4 v = xs4[g];
+                            const float xv[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                            for (int q = 0; q < K2_NPOS; ++q)
+#pragma unroll
+                                for (int r = 0; r < 4; ++r) eval_welsch(xv[r], kk[q], c0[q], nalpha, S[q], R[q]);
+                        }
+                    }
+                } else {
                     if (!scalar_all) {
                         if constexpr (SPLIT == 1) {
 #pragma unroll K2_UNROLL

@@ -569,3 +569,65 @@ def test_mad_is_inflated_by_a_deep_dip_but_upper_rms_is_not():
     m0, m1 = (orc.family(v[None, :], 201, orc.SCALE_MAD, 0, n_iter=0).scale[0, 100] for v in (x, y))
     assert a0 == a1
     assert m1 > 1.5 * m0
+
+
+# ------------------------------------------------------------------ F2, second part: segments (reading R23)
+def _segment_case(seed, S=2, N=700):
+    from workloads import lightcurves as lc
+    grid = lc.random_series(seed, S, N, nan_frac=0.03, inf_frac=0.0)
+    rng = np.random.default_rng(seed)
+    for b in range(S):                                     # a few wide gaps and one island of 5 samples
+        for _ in range(3):
+            a = int(rng.integers(50, N - 120))
+            grid[b, a:a + int(rng.integers(15, 60))] = np.nan
+        a = int(rng.integers(200, N - 200))
+        grid[b, a - 30:a + 35] = np.nan
+        grid[b, a:a + 5] = 1.0 + 1e-3 * rng.standard_normal(5).astype(np.float32)
+    return lc.compact(grid, 0.02, t0=3.5, jitter=0.2, seed=seed) + (N,)
+
+
+@pytest.mark.parametrize("W,brk,mseg,ecut", [(21, 10, 0, 0), (21, 10, 8, 0), (21, 12, 8, 3), (51, 25, 17, 0),
+                                              (51, 40, 0, 7), (9, 0, 3, 1), (21, 3, 0, 0), (21, -1, 0, 4)])
+def test_gapped_segments_brute_force(W, brk, mseg, ecut):
+    # independent numpy brute force (np.split on the slot differences) incl. break_slots < h, where the
+    # "own segment only" clause of R23 is what keeps a window from reaching across a short gap
+    t, f, slot, N = _segment_case(100 + W + brk)
+    got = orc.gapped_ex(t, f, 3.5, 0.02, N, W, break_slots=brk, min_segment=mseg, edge_cut=ecut)
+    bt, bm = brute.detrend_gapped_ex(t, f, 3.5, 0.02, N, W, break_slots=brk, min_segment=mseg, edge_cut=ecut)
+    assert np.array_equal(np.isnan(got.trend64), np.isnan(bt))
+    ok = ~np.isnan(bt)
+    assert np.array_equal(got.median[ok], bm[ok].astype(np.float32))
+    assert np.allclose(got.trend64[ok], bt[ok], rtol=1e-12, atol=0.0)
+
+
+def test_gapped_segments_reduce_to_plain_gap_handling():
+    t, f, slot, N = _segment_case(7)
+    base = orc.gapped(t, f, 3.5, 0.02, N, 21)
+    off = orc.gapped_ex(t, f, 3.5, 0.02, N, 21)                       # nothing switched on
+    assert np.array_equal(base.trend64, off.trend64, equal_nan=True)
+    # breaks at least h slots wide cannot be crossed by a window anyway: only the bookkeeping differs
+    wide = orc.gapped_ex(t, f, 3.5, 0.02, N, 21, break_slots=10)
+    assert np.array_equal(base.trend64, wide.trend64, equal_nan=True)
+    # a break narrower than h does change windows: with break_slots = 0 every missing slot ends a segment
+    narrow = orc.gapped_ex(t, f, 3.5, 0.02, N, 21, break_slots=0, min_valid=1)
+    both = ~np.isnan(base.trend64) & ~np.isnan(narrow.trend64)
+    assert (base.trend64[both] != narrow.trend64[both]).any()
+
+
+def test_gapped_segments_hand_example():
+    # slots 0..9, a 4-slot hole, 14..16, another hole, 30..49: break at > 3 empty slots gives segments of
+    # 10, 3 and 20 samples; min_segment = 4 drops the middle one; edge_cut = 2 blanks two slots at every end
+    k = np.r_[0:10, 14:17, 30:50].astype(np.float64)
+    t = (10.0 + 0.5 * k)[None, :]
+    f = (1.0 + 0.01 * np.sin(k))[None, :].astype(np.float32)
+    r = orc.gapped_ex(t, f, 10.0, 0.5, 50, 5, break_slots=3, min_segment=4, edge_cut=2, min_valid=1)
+    nan = np.isnan(r.trend64[0])
+    expect = np.ones(33, bool)
+    expect[2:8] = False                      # slots 2..7 of the first segment
+    expect[15:31] = False                    # slots 32..47 of the last one
+    assert np.array_equal(nan, expect)
+    # the first window that survives: slots 0..4 (the cut samples still count)
+    assert r.n_valid[0, 2] == 5 and r.median[0, 2] == np.sort(f[0, 0:5])[2]
+    # without the minimum length the island is a segment of its own and never sees its neighbours
+    r2 = orc.gapped_ex(t, f, 10.0, 0.5, 50, 9, break_slots=3, min_valid=1)
+    assert list(r2.n_valid[0, 10:13]) == [3, 3, 3]
