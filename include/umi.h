@@ -188,6 +188,29 @@ int umi_detrend_gapped(const double* time, const float* flux,
                        void* workspace, size_t workspace_bytes, void* stream);
 
 /*
+ * The same with SEGMENTS (reading R23; "gap handling", "minimum
+ * segment length ... W/3"): the valid samples of a row are cut into segments wherever more than
+ * break_slots empty slots lie between two consecutive ones, and
+ *   min_segment  a segment with fewer valid samples is dropped: NaN out, in no window (<= 0: off);
+ *   edge_cut     samples less than edge_cut slots from the first or the last slot of their segment get
+ *                NaN (trend and flat) but still take part in the windows of the others (<= 0: off);
+ *   break_slots  < 0: the row is one segment.  Windows are never clipped at a break, which is exact
+ *                whenever no window can reach across one: break_slots >= (W-1)/2 is required,
+ *                0 <= break_slots < (W-1)/2 -> UMI_ERR_UNSUPPORTED.  (For a break of half a day on a
+ *                half-day window, the usual choice, break_slots = W - 1.)
+ * With all three off this is umi_detrend_gapped.  Needs umi_gapped_ex_workspace_bytes (17 bytes per
+ * slot) when any of them is on, else umi_gapped_workspace_bytes; n_grid <= 2^31 - 1.
+ */
+size_t umi_gapped_ex_workspace_bytes(int64_t n_stars, int64_t n_grid);
+int umi_detrend_gapped_ex(const double* time, const float* flux,
+                          int64_t n_stars, int64_t n_samples,
+                          double t0, double dt, int64_t n_grid,
+                          int W, float alpha, float c, int n_iter, int min_valid,
+                          int64_t break_slots, int64_t min_segment, int64_t edge_cut,
+                          float* trend_out, float* flat_out,
+                          void* workspace, size_t workspace_bytes, void* stream);
+
+/*
  * Batch driver (the paper streams 50-star batches): the same
  * computation with HOST buffers.  Stars are cut into batches of
  * `stars_per_batch` (<= 0: a body of ~32 MiB batches between a ramp up and a

@@ -23,7 +23,8 @@ UMI_WEIGHT_BISQUARE, UMI_WEIGHT_WELSCH = 0, 1
 
 EXPORTS = ("umi_window_len", "umi_detrend", "umi_detrend_ex", "umi_detrend_host", "umi_detrend_profile",
            "umi_flatten", "umi_flatten_host", "umi_detrend_family", "umi_detrend_gapped", "umi_gapped_workspace_bytes",
-           "umi_launch_geometry", "umi_status_string", "umi_version", "umi_shutdown")
+           "umi_launch_geometry", "umi_status_string", "umi_version", "umi_shutdown",
+           "umi_detrend_gapped_ex", "umi_gapped_ex_workspace_bytes")
 
 _lib = None
 
@@ -66,6 +67,11 @@ def lib():
     L.umi_detrend_gapped.restype = ci
     L.umi_detrend_gapped.argtypes = [vp, vp, i64, i64, ctypes.c_double, ctypes.c_double, i64,
                                      ci, cf, cf, ci, ci, vp, vp, vp, ctypes.c_size_t, vp]
+    L.umi_gapped_ex_workspace_bytes.restype = ctypes.c_size_t
+    L.umi_gapped_ex_workspace_bytes.argtypes = [i64, i64]
+    L.umi_detrend_gapped_ex.restype = ci
+    L.umi_detrend_gapped_ex.argtypes = [vp, vp, i64, i64, ctypes.c_double, ctypes.c_double, i64,
+                                        ci, cf, cf, ci, ci, i64, i64, i64, vp, vp, vp, ctypes.c_size_t, vp]
     L.umi_launch_geometry.restype = ci
     L.umi_launch_geometry.argtypes = [ci] + [ctypes.POINTER(ci)] * 3
     L.umi_status_string.restype = ctypes.c_char_p
@@ -235,11 +241,16 @@ def umi_gapped_workspace_bytes(n_stars, n_grid):
     return int(lib().umi_gapped_workspace_bytes(int(n_stars), int(n_grid)))
 
 
+def umi_gapped_ex_workspace_bytes(n_stars, n_grid):
+    return int(lib().umi_gapped_ex_workspace_bytes(int(n_stars), int(n_grid)))
+
+
 def umi_detrend_gapped(time, flux, t0, dt, n_grid, W, alpha=2.0, n_iter=5, c=5.0, min_valid=-1,
-                       flat=False, workspace=None, stream=None):
+                       flat=False, workspace=None, stream=None, break_slots=-1, min_segment=0, edge_cut=0):
     """Compacted rows with real time stamps (gap handling; include/umi.h).
     `time` CUDA fp64 [S, M], `flux` CUDA fp32 [S, M].  Returns trend, or (trend, flat).
-    `workspace`: optional CUDA uint8 tensor of at least umi_gapped_workspace_bytes bytes; when it is
+    break_slots / min_segment / edge_cut: segments (umi_detrend_gapped_ex; all off by default).
+    `workspace`: optional CUDA uint8 tensor of at least umi_gapped[_ex]_workspace_bytes bytes; when it is
     not given, one is allocated on `stream`, so its release is ordered after the kernels that use it."""
     import torch
     f = _cuda_2d(flux, torch.float32, "flux")
@@ -247,7 +258,8 @@ def umi_detrend_gapped(time, flux, t0, dt, n_grid, W, alpha=2.0, n_iter=5, c=5.0
     if tt.shape != f.shape or tt.device != f.device:
         raise ValueError("time must have flux's shape and device")
     S, M = f.shape
-    need = umi_gapped_workspace_bytes(S, n_grid)
+    segments = break_slots >= 0 or min_segment > 0 or edge_cut > 0
+    need = umi_gapped_ex_workspace_bytes(S, n_grid) if segments else umi_gapped_workspace_bytes(S, n_grid)
     if workspace is not None and not (isinstance(workspace, torch.Tensor) and workspace.is_cuda and workspace.is_contiguous()):
         raise TypeError("workspace must be a contiguous CUDA tensor")
     with _OnStream(stream, f.device) as on:
@@ -258,10 +270,11 @@ def umi_detrend_gapped(time, flux, t0, dt, n_grid, W, alpha=2.0, n_iter=5, c=5.0
         fl = torch.empty_like(f) if flat else None
         on.uses(f, tt, workspace)
         if S and M:
-            _check(lib().umi_detrend_gapped(tt.data_ptr(), f.data_ptr(), S, M, float(t0), float(dt), int(n_grid),
-                                            int(W), float(alpha), float(c), int(n_iter), int(min_valid),
-                                            trend.data_ptr(), fl.data_ptr() if flat else None,
-                                            workspace.data_ptr(), wbytes, on.ptr))
+            _check(lib().umi_detrend_gapped_ex(tt.data_ptr(), f.data_ptr(), S, M, float(t0), float(dt), int(n_grid),
+                                               int(W), float(alpha), float(c), int(n_iter), int(min_valid),
+                                               int(break_slots), int(min_segment), int(edge_cut),
+                                               trend.data_ptr(), fl.data_ptr() if flat else None,
+                                               workspace.data_ptr(), wbytes, on.ptr))
     return (trend.view(flux.shape), fl.view(flux.shape)) if flat else trend.view(flux.shape)
 
 

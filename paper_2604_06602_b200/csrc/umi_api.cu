@@ -247,17 +247,29 @@ size_t umi_gapped_workspace_bytes(int64_t n_stars, int64_t n_grid)
     return (size_t)n_stars * (size_t)n_grid * (2 * sizeof(float));
 }
 
-int umi_detrend_gapped(const double* time, const float* flux, int64_t n_stars, int64_t n_samples,
-                       double t0, double dt, int64_t n_grid,
-                       int W, float alpha, float c, int n_iter, int min_valid,
-                       float* trend_out, float* flat_out,
-                       void* workspace, size_t workspace_bytes, void* stream)
+size_t umi_gapped_ex_workspace_bytes(int64_t n_stars, int64_t n_grid)
+{
+    if (n_stars <= 0 || n_grid <= 0) return 0;
+    /* the two grids, 8 bytes per slot for the segment scan, one edge-cut byte per slot */
+    return (size_t)n_stars * (size_t)n_grid * (2 * sizeof(float) + 2 * sizeof(int32_t) + 1);
+}
+
+int umi_detrend_gapped_ex(const double* time, const float* flux, int64_t n_stars, int64_t n_samples,
+                          double t0, double dt, int64_t n_grid,
+                          int W, float alpha, float c, int n_iter, int min_valid,
+                          int64_t break_slots, int64_t min_segment, int64_t edge_cut,
+                          float* trend_out, float* flat_out,
+                          void* workspace, size_t workspace_bytes, void* stream)
 {
     if (time == nullptr || n_grid < 0 || !(dt > 0.0) || !isfinite(dt) || !isfinite(t0)) return UMI_ERR_INVALID_ARG;
     const int st = validate(flux, n_stars, n_samples, W, alpha, c, n_iter, trend_out);
     if (st != UMI_OK) return st;
+    if (n_grid > 0x7FFFFFFF) return UMI_ERR_UNSUPPORTED;              /* slots are 32-bit in the segment scan */
+    const bool segments = break_slots >= 0 || min_segment > 0 || edge_cut > 0;
+    /* windows are never clipped at a break: a break the window could reach across is refused (umi.h) */
+    if (break_slots >= 0 && break_slots < (W - 1) / 2) return UMI_ERR_UNSUPPORTED;
     if (n_stars == 0 || n_samples == 0) return UMI_OK;
-    const size_t need = umi_gapped_workspace_bytes(n_stars, n_grid);
+    const size_t need = segments ? umi_gapped_ex_workspace_bytes(n_stars, n_grid) : umi_gapped_workspace_bytes(n_stars, n_grid);
     if (need > 0 && (workspace == nullptr || workspace_bytes < need)) return UMI_ERR_INVALID_ARG;
     cudaStream_t s = static_cast<cudaStream_t>(stream);
     umi::RegridParams gp;
@@ -268,19 +280,35 @@ int umi_detrend_gapped(const double* time, const float* flux, int64_t n_stars, i
     gp.n_grid = n_grid;
     gp.t0 = t0;
     gp.dt = dt;
+    const size_t slots = (size_t)n_stars * (size_t)n_grid;
     float* grid_flux = static_cast<float*>(workspace);
-    float* grid_trend = grid_flux + (size_t)n_stars * (size_t)n_grid;
+    float* grid_trend = grid_flux + slots;
+    void* scan = grid_trend + slots;                                  /* 8 bytes per slot, 8-byte aligned */
+    uint8_t* grid_cut = segments ? static_cast<uint8_t*>(scan) + slots * 8 : nullptr;
     if (n_grid > 0) {
         /* 0xFFFFFFFF is a NaN: every slot starts invalid */
-        if (cuda_failed(cudaMemsetAsync(grid_flux, 0xFF, (size_t)n_stars * (size_t)n_grid * sizeof(float), s)))
-            return UMI_ERR_CUDA;
+        if (cuda_failed(cudaMemsetAsync(grid_flux, 0xFF, slots * sizeof(float), s))) return UMI_ERR_CUDA;
         if (cuda_failed(umi::launch_regrid_scatter(gp, grid_flux, s))) return UMI_ERR_CUDA;
+        if (segments && cuda_failed(umi::launch_regrid_segments(grid_flux, grid_cut, scan, n_stars, n_grid, break_slots,
+                                                                min_segment, edge_cut, s)))
+            return UMI_ERR_CUDA;
         const int st2 = launch_device(nullptr, grid_flux, n_stars, n_grid, W, alpha, c, n_iter, min_valid,
                                       grid_trend, s);
         if (st2 != UMI_OK) return st2;
     }
-    if (cuda_failed(umi::launch_regrid_gather(gp, grid_trend, trend_out, flat_out, s))) return UMI_ERR_CUDA;
+    if (cuda_failed(umi::launch_regrid_gather(gp, grid_trend, n_grid > 0 ? grid_cut : nullptr, trend_out, flat_out, s)))
+        return UMI_ERR_CUDA;
     return UMI_OK;
+}
+
+int umi_detrend_gapped(const double* time, const float* flux, int64_t n_stars, int64_t n_samples,
+                       double t0, double dt, int64_t n_grid,
+                       int W, float alpha, float c, int n_iter, int min_valid,
+                       float* trend_out, float* flat_out,
+                       void* workspace, size_t workspace_bytes, void* stream)
+{
+    return umi_detrend_gapped_ex(time, flux, n_stars, n_samples, t0, dt, n_grid, W, alpha, c, n_iter, min_valid,
+                                 -1, 0, 0, trend_out, flat_out, workspace, workspace_bytes, stream);
 }
 
 int umi_detrend_profile(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,

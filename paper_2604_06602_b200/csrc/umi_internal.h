@@ -111,9 +111,14 @@ struct RegridParams {
 };
 /* grid_flux[n_stars, n_grid] must already be NaN-filled */
 cudaError_t launch_regrid_scatter(const RegridParams& prm, float* grid_flux, cudaStream_t stream);
-/* trend_out[b, i] = grid_trend[b, slot] (NaN for invalid samples); flat_out (nullable) = flux / trend */
-cudaError_t launch_regrid_gather(const RegridParams& prm, const float* grid_trend, float* trend_out,
+/* trend_out[b, i] = grid_trend[b, slot] (NaN for invalid samples, and where grid_cut (nullable) marks the slot);
+   flat_out (nullable) = flux / trend */
+cudaError_t launch_regrid_gather(const RegridParams& prm, const float* grid_trend, const uint8_t* grid_cut, float* trend_out,
                                  float* flat_out, cudaStream_t stream);
+/* segments on the slot grid (reading R23): erases short segments from grid_flux, marks edge slots in grid_cut
+   [n_stars, n_grid]; scratch: 8 bytes per slot */
+cudaError_t launch_regrid_segments(float* grid_flux, uint8_t* grid_cut, void* scratch, int64_t n_stars, int64_t n_grid,
+                                   int64_t break_slots, int64_t min_segment, int64_t edge_cut, cudaStream_t stream);
 
 } // namespace umi
 

@@ -92,7 +92,7 @@ umi_regrid_scatter_kernel(RegridParams prm, float* __restrict__ grid_flux)
 }
 
 __global__ void __launch_bounds__(RG_THREADS)
-umi_regrid_gather_kernel(RegridParams prm, const float* __restrict__ grid_trend,
+umi_regrid_gather_kernel(RegridParams prm, const float* __restrict__ grid_trend, const uint8_t* __restrict__ grid_cut,
                          float* __restrict__ trend_out, float* __restrict__ flat_out)
 {
     const float qnan = __int_as_float(0x7FC00000);
@@ -116,6 +116,7 @@ umi_regrid_gather_kernel(RegridParams prm, const float* __restrict__ grid_trend,
                 const int64_t i = base + r * RG_THREADS + threadIdx.x;
                 const int64_t k = sample_slot(t[r], trow, i, prm.M, prm.t0, prm.dt, prm.n_grid);
                 tr[r] = (k >= 0 && finite_f32(x[r])) ? __ldg(grow + k) : qnan;
+                if (grid_cut != nullptr && k >= 0 && __ldg(grid_cut + b * prm.n_grid + k)) tr[r] = qnan;   /* (R23) edge cut */
             }
 #pragma unroll
             for (int r = 0; r < RG_ITEMS; ++r) {
@@ -123,6 +124,83 @@ umi_regrid_gather_kernel(RegridParams prm, const float* __restrict__ grid_trend,
                 if (i >= prm.M) continue;
                 trend_out[b * prm.M + i] = tr[r];
                 if (flat_out != nullptr) flat_out[b * prm.M + i] = (tr[r] == tr[r]) ? x[r] / tr[r] : qnan;
+            }
+        }
+    }
+}
+
+/*
+ * Segments (reading R23), on the slot grid after the scatter: the valid slots of a row are
+ * cut into segments wherever more than break_slots empty slots lie between two of them; a segment with fewer
+ * than min_segment valid slots is erased from grid_flux (NaN: in no window, no trend); grid_cut[k] = 1 for the
+ * valid slots less than edge_cut slots from their segment's first or last slot (the gather blanks those).
+ * One warp per row, 32 slots at a time, two passes: forward (first slot and index inside the segment, kept in
+ * `scratch`), backward (last slot and size of the segment).  Windows need no clipping: the entry point only
+ * accepts break_slots >= h, and a window of half-width h cannot reach across more than h - 1 empty slots.
+ */
+__global__ void __launch_bounds__(128)
+umi_regrid_segments_kernel(float* __restrict__ grid_flux, uint8_t* __restrict__ grid_cut, int2* __restrict__ scratch,
+                           int64_t n_stars, int64_t n_grid, int64_t break_slots, int64_t min_segment, int64_t edge_cut)
+{
+    const int lane = threadIdx.x & 31;
+    const unsigned lt = (1u << lane) - 1u, le = lt | (1u << lane), gt = ~le;
+    const float qnan = __int_as_float(0x7FC00000);
+    for (int64_t b = (int64_t)blockIdx.x * 4 + (threadIdx.x >> 5); b < n_stars; b += (int64_t)gridDim.x * 4) {
+        float* frow = grid_flux + b * n_grid;
+        uint8_t* crow = grid_cut + b * n_grid;
+        int2* srow = scratch + b * n_grid;
+        /* forward: (first slot of the segment, index inside it) of every valid slot */
+        bool have_prev = false;
+        int64_t prev_slot = 0, cur_first = 0, cur_cnt = 0;
+        for (int64_t base = 0; base < n_grid; base += 32) {
+            const int64_t k = base + lane;
+            const bool valid = k < n_grid && finite_f32(frow[k]);
+            const unsigned vb = __ballot_sync(0xFFFFFFFFu, valid);
+            const int p = 31 - __clz((int)(vb & lt));                               /* previous valid lane, -1: none */
+            const bool none = p < 0 && !have_prev;
+            const int64_t ps = p >= 0 ? base + p : prev_slot;
+            const bool start = valid && (none || (break_slots >= 0 && k - ps - 1 > break_slots));
+            const unsigned sb = __ballot_sync(0xFFFFFFFFu, start);
+            if (valid) {
+                const int st = 31 - __clz((int)(sb & le));                          /* start lane of my segment, -1: before this chunk */
+                int2 rec;
+                if (st >= 0) { rec.x = (int)(base + st); rec.y = __popc(vb & le & ~((1u << st) - 1u)) - 1; }
+                else { rec.x = (int)cur_first; rec.y = (int)cur_cnt + __popc(vb & lt); }
+                srow[k] = rec;
+            }
+            if (vb) { prev_slot = base + 31 - __clz((int)vb); have_prev = true; }
+            if (sb) { const int ls = 31 - __clz((int)sb); cur_first = base + ls; cur_cnt = __popc(vb & ~((1u << ls) - 1u)); }
+            else cur_cnt += __popc(vb);
+        }
+        __syncwarp();
+        /* backward: (last slot, size) of the segment; short segments erased, edges marked */
+        bool have_next = false;
+        int64_t next_slot = 0, cur_last = 0, cur_total = 0;
+        for (int64_t base = ((n_grid - 1) / 32) * 32; base >= 0; base -= 32) {
+            const int64_t k = base + lane;
+            const bool valid = k < n_grid && finite_f32(frow[k]);
+            const unsigned vb = __ballot_sync(0xFFFFFFFFu, valid);
+            const int nx = __ffs((int)(vb & gt)) - 1;                               /* next valid lane, -1: none */
+            const bool none = nx < 0 && !have_next;
+            const int64_t ns = nx >= 0 ? base + nx : next_slot;
+            const bool end = valid && (none || (break_slots >= 0 && ns - k - 1 > break_slots));
+            const unsigned eb = __ballot_sync(0xFFFFFFFFu, end);
+            int2 rec = make_int2(0, 0);
+            if (valid) rec = srow[k];
+            const int en = __ffs((int)(eb & ~lt)) - 1;                              /* end lane of my segment, -1: after this chunk */
+            const int idx_at_end = __shfl_sync(0xFFFFFFFFu, rec.y, en >= 0 ? en : 0);
+            const int64_t last = en >= 0 ? base + en : cur_last;
+            const int64_t total = en >= 0 ? (int64_t)idx_at_end + 1 : cur_total;
+            if (k < n_grid) {
+                const bool drop = valid && min_segment > 0 && total < min_segment;
+                if (drop) frow[k] = qnan;
+                crow[k] = (valid && !drop && edge_cut > 0 && (k - rec.x < edge_cut || last - k < edge_cut)) ? 1 : 0;
+            }
+            if (vb) { next_slot = base + __ffs((int)vb) - 1; have_next = true; }
+            if (eb) {
+                const int fe = __ffs((int)eb) - 1;
+                cur_last = base + fe;
+                cur_total = (int64_t)__shfl_sync(0xFFFFFFFFu, rec.y, fe) + 1;
             }
         }
     }
@@ -146,11 +224,21 @@ cudaError_t launch_regrid_scatter(const RegridParams& prm, float* grid_flux, cud
     return cudaGetLastError();
 }
 
-cudaError_t launch_regrid_gather(const RegridParams& prm, const float* grid_trend, float* trend_out,
+cudaError_t launch_regrid_gather(const RegridParams& prm, const float* grid_trend, const uint8_t* grid_cut, float* trend_out,
                                  float* flat_out, cudaStream_t stream)
 {
-    umi_regrid_gather_kernel<<<regrid_grid(prm.n_stars, prm.M), RG_THREADS, 0, stream>>>(prm, grid_trend,
+    umi_regrid_gather_kernel<<<regrid_grid(prm.n_stars, prm.M), RG_THREADS, 0, stream>>>(prm, grid_trend, grid_cut,
                                                                                          trend_out, flat_out);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_regrid_segments(float* grid_flux, uint8_t* grid_cut, void* scratch, int64_t n_stars, int64_t n_grid,
+                                   int64_t break_slots, int64_t min_segment, int64_t edge_cut, cudaStream_t stream)
+{
+    int64_t ctas = (n_stars + 3) / 4;
+    if (ctas > 0x7FFFFFFF) ctas = 0x7FFFFFFF;
+    umi_regrid_segments_kernel<<<(unsigned)ctas, 128, 0, stream>>>(grid_flux, grid_cut, static_cast<int2*>(scratch), n_stars,
+                                                                    n_grid, break_slots, min_segment, edge_cut);
     return cudaGetLastError();
 }
 

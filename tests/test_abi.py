@@ -98,6 +98,11 @@ def test_validation_happens_on_the_host():
     assert fam(S=0, scale=None) == umi.UMI_OK
     assert umi.umi_gapped_workspace_bytes(3, 100) == 2400     # two fp32 grids
     assert umi.umi_gapped_workspace_bytes(0, 100) == 0
+    assert umi.umi_gapped_ex_workspace_bytes(3, 100) == 3 * 100 * 17
+    gex = lambda **k: L.umi_detrend_gapped_ex(one, one, 1, 10, 0.0, 0.5, 12, k.get("W", 5), 2.0, 5.0, 5, -1, k.get("brk", -1), k.get("mseg", 0),
+                                               k.get("ecut", 0), one, None, k.get("ws", one), k.get("wsb", 1 << 20), None)
+    assert gex(W=51, brk=24) == umi.UMI_ERR_UNSUPPORTED       # a break a window could reach across
+    assert gex(mseg=3, wsb=12 * 8) == umi.UMI_ERR_INVALID_ARG   # segments need the larger workspace
     for s in range(5):
         assert umi.umi_status_string(s)
     assert "UMI_OK" in umi.umi_status_string(0)

@@ -116,6 +116,56 @@ def test_gapped_tess_batch_stars_compacted(umi):
     _check_flat(flat.cpu().numpy(), f, ref)
 
 
+def _segment_rows(seed, S, N, dt):
+    grid = lc.random_series(seed, S, N, nan_frac=0.03, inf_frac=0.0)
+    rng = np.random.default_rng(seed)
+    for b in range(S):                                      # wide gaps, and an island of a few samples
+        for _ in range(4):
+            a = int(rng.integers(50, N - 400))
+            grid[b, a:a + int(rng.integers(30, 380))] = np.nan
+        a = int(rng.integers(400, N - 400))
+        grid[b, a - 200:a + 210] = np.nan
+        grid[b, a:a + 9] = 1.0
+    return lc.compact(grid, dt, t0=7.25, jitter=0.2, seed=seed)
+
+
+@pytest.mark.parametrize("W,brk,mseg,ecut", [(25, 12, 12, 0), (25, 24, 0, 5), (51, 25, 17, 3), (361, 180, 120, 0),
+                                              (361, 360, 120, 40), (361, -1, 0, 25), (217, 400, 72, 1)])
+def test_gapped_segments_match_oracle(umi, W, brk, mseg, ecut):
+    # reading R23: segments at gaps wider than break_slots, minimum segment length, edge cut
+    import torch
+    dt = 2.0 / 1440
+    S, N = (5, 6001) if W > 49 else (3, 3001)
+    t, f, slot = _segment_rows(600 + W + max(brk, 0), S, N, dt)
+    ref = orc.gapped_ex(t, f, 7.25, dt, N, W, break_slots=brk, min_segment=mseg, edge_cut=ecut)
+    td, fd = _cuda(t, np.float64), _cuda(f, np.float32)
+    med = umi.umi_detrend_gapped(td, fd, 7.25, dt, N, W, n_iter=0, break_slots=brk, min_segment=mseg, edge_cut=ecut)
+    trend, flat = umi.umi_detrend_gapped(td, fd, 7.25, dt, N, W, flat=True, break_slots=brk, min_segment=mseg, edge_cut=ecut)
+    torch.cuda.synchronize()
+    parity.compare_median(med.cpu().numpy(), ref.median)
+    parity.compare_trend(trend.cpu().numpy(), ref)
+    _check_flat(flat.cpu().numpy(), f, ref)
+    if ecut > 0 or W == 25:                                               # the options did remove something the plain path keeps
+        plain = orc.gapped(t, f, 7.25, dt, N, W)
+        assert (np.isnan(ref.trend64) & ~np.isnan(plain.trend64)).any()
+
+
+def test_gapped_segments_argument_rules(umi):
+    import torch
+    t, f, slot = _segment_rows(3, 2, 2001, 0.01)
+    td, fd = _cuda(t, np.float64), _cuda(f, np.float32)
+    with pytest.raises(umi.UmiError) as e:                                # a break a window could reach across
+        umi.umi_detrend_gapped(td, fd, 7.25, 0.01, 2001, 51, break_slots=24)
+    assert e.value.status == umi.UMI_ERR_UNSUPPORTED
+    with pytest.raises(umi.UmiError):                                     # the plain workspace is too small for segments
+        umi.umi_detrend_gapped(td, fd, 7.25, 0.01, 2001, 51, min_segment=17,
+                               workspace=torch.empty(umi.umi_gapped_workspace_bytes(2, 2001), dtype=torch.uint8, device="cuda"))
+    a = umi.umi_detrend_gapped(td, fd, 7.25, 0.01, 2001, 51)
+    b = umi.umi_detrend_gapped(td, fd, 7.25, 0.01, 2001, 51, break_slots=10 ** 9)     # one segment: nothing changes
+    torch.cuda.synchronize()
+    assert torch.equal(torch.nan_to_num(a), torch.nan_to_num(b)) and torch.equal(torch.isnan(a), torch.isnan(b))
+
+
 # ------------------------------------------------------------------ F4: sibling estimators
 def _family_case(umi, x, W, sk, wk, alpha=2.0, c=5.0, n_iter=5, time=None):
     import torch
