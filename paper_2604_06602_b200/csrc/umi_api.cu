@@ -92,6 +92,13 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
     if (n_stars == 0 || n_cadences == 0) return UMI_OK;
     Geometry g = geometry_for(W);
     const bool mad = fam.on && fam.scale_kind == umi::SCALE_MAD;
+    /* small batches (fewer median tiles than SMs; config 1 has 30): a 512-key sort with tiles of at least 128
+       positions gives four times the CTAs and a shorter serial chain in each (latency is what is left to win) */
+    if (W - 1 + 128 <= 512 && n_stars * ((n_cadences + g.T1 - 1) / g.T1) < (int64_t)sm_count()) {
+        g.NS = 512;
+        g.T1 = 512 - (W - 1);
+        g.smem1 = umi::k1_smem_bytes(g.NS, false, g.T1);
+    }
     if (mad) g.smem1 = umi::k1_smem_bytes(g.NS, true, g.T1);
     if (min_valid < 0) min_valid = std::max(1, W / 3);      /* PAPER.md:192 (R4) */
 

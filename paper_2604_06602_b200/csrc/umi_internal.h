@@ -13,7 +13,10 @@ namespace umi {
 #define UMI_K1_THREADS 256
 #endif
 constexpr int K1_THREADS = UMI_K1_THREADS;       /* median kernel */
-constexpr int K1_MIN_SORT = 1024;                /* smallest per-tile sort length */
+#ifndef UMI_K1_MIN_SORT
+#define UMI_K1_MIN_SORT 1024
+#endif
+constexpr int K1_MIN_SORT = UMI_K1_MIN_SORT;     /* smallest per-tile sort length */
 /* walkers per tile of the median kernel and its dynamic shared memory (bytes) */
 #ifndef UMI_K1_WALKER_BUDGET
 #define UMI_K1_WALKER_BUDGET 131072

@@ -50,9 +50,9 @@ __device__ __forceinline__ int load_keys(const double* __restrict__ trow, const 
                                          bool vec, uint32_t (&key)[E])
 {
     int nvalid = 0;
-    if (vec) {
+    if (E % 4 == 0 && vec) {
 #pragma unroll
-        for (int e = 0; e < E; e += 4) {
+        for (int e = 0; e + 3 < E; e += 4) {
             const int64_t jj = j + e;
             float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
             bool in = jj >= 0 && jj < N;                            /* a group of 4 lies entirely inside or outside the row */
@@ -111,21 +111,29 @@ __device__ __forceinline__ void bitonic_stage(uint32_t (&v)[E], uint32_t* buf, i
     } else {
         /* partner in another warp: exchange through shared memory */
         __syncthreads();
-#pragma unroll
-        for (int e = 0; e < E; e += 4)
-            *reinterpret_cast<uint4*>(buf + tid * E + e) = make_uint4(v[e], v[e + 1], v[e + 2], v[e + 3]);
-        __syncthreads();
         const bool up = ((tid * E) & K) == 0;
         const bool low = ((tid * E) & J) == 0;
         const bool keep_min = (low == up);
         const uint32_t* other = buf + ((tid * E) ^ J);
+        if constexpr (E % 4 == 0) {
 #pragma unroll
-        for (int e = 0; e < E; e += 4) {
-            const uint4 o4 = *reinterpret_cast<const uint4*>(other + e);
-            v[e] = keep_min ? min(v[e], o4.x) : max(v[e], o4.x);
-            v[e + 1] = keep_min ? min(v[e + 1], o4.y) : max(v[e + 1], o4.y);
-            v[e + 2] = keep_min ? min(v[e + 2], o4.z) : max(v[e + 2], o4.z);
-            v[e + 3] = keep_min ? min(v[e + 3], o4.w) : max(v[e + 3], o4.w);
+            for (int e = 0; e < E; e += 4)
+                *reinterpret_cast<uint4*>(buf + tid * E + e) = make_uint4(v[e], v[e + 1], v[e + 2], v[e + 3]);
+            __syncthreads();
+#pragma unroll
+            for (int e = 0; e < E; e += 4) {
+                const uint4 o4 = *reinterpret_cast<const uint4*>(other + e);
+                v[e] = keep_min ? min(v[e], o4.x) : max(v[e], o4.x);
+                v[e + 1] = keep_min ? min(v[e + 1], o4.y) : max(v[e + 1], o4.y);
+                v[e + 2] = keep_min ? min(v[e + 2], o4.z) : max(v[e + 2], o4.z);
+                v[e + 3] = keep_min ? min(v[e + 3], o4.w) : max(v[e + 3], o4.w);
+            }
+        } else {                                                    /* E = 2 (NS = 512, small batches) */
+            *reinterpret_cast<uint2*>(buf + tid * E) = make_uint2(v[0], v[1]);
+            __syncthreads();
+            const uint2 o2 = *reinterpret_cast<const uint2*>(other);
+            v[0] = keep_min ? min(v[0], o2.x) : max(v[0], o2.x);
+            v[1] = keep_min ? min(v[1], o2.y) : max(v[1], o2.y);
         }
     }
 }
@@ -163,7 +171,7 @@ struct MadRange {
 };
 
 template <int E, bool MAD>
-__global__ void __launch_bounds__(K1_THREADS, E == 4 ? 6 : E == 8 ? 5 : E == 16 ? 3 : 1)   /* as many CTAs per SM as their shared memory allows (NS = 1024: 6, 2048: 5, 4096: 3, 8192: 1) */
+__global__ void __launch_bounds__(K1_THREADS, E <= 4 ? 6 : E == 8 ? 5 : E == 16 ? 3 : 1)   /* as many CTAs per SM as their shared memory allows (NS = 1024: 6, 2048: 5, 4096: 3, 8192: 1) */
 umi_median_kernel(MedianParams prm)
 {
     constexpr int NS = K1_THREADS * E;
@@ -535,6 +543,7 @@ cudaError_t launch_median(const MedianParams& prm, unsigned grid, size_t smem, c
     void (*k1)(MedianParams) = nullptr;
     const bool mad = prm.scale != nullptr;
     switch (prm.NS / K1_THREADS) {
+    case 2: k1 = mad ? umi_median_kernel<2, true> : umi_median_kernel<2, false>; break;
     case 4: k1 = mad ? umi_median_kernel<4, true> : umi_median_kernel<4, false>; break;
     case 8: k1 = mad ? umi_median_kernel<8, true> : umi_median_kernel<8, false>; break;
     case 16: k1 = mad ? umi_median_kernel<16, true> : umi_median_kernel<16, false>; break;
