@@ -54,11 +54,7 @@ __device__ __forceinline__ bool load_sample(const double* __restrict__ trow,
    not depend on the median kernel -- while the median kernel's last CTAs are still running; it waits here before
    it touches what the median kernel wrote.  Both instructions do nothing in a launch without the attribute. ---- */
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
-#ifdef UMI_NO_PDL_WAIT
-__device__ __forceinline__ void pdl_wait_for_primary() {}
-#else
 __device__ __forceinline__ void pdl_wait_for_primary() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-#endif
 
 /* ---- sm_100a packed fp32x2 arithmetic (FFMA2 / FMUL2 / FADD2): two fp32 in one 64-bit register pair ---- */
 typedef unsigned long long f32x2;                    /* two fp32 in one 64-bit register pair */

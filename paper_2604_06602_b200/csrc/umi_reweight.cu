@@ -581,11 +581,7 @@ cudaError_t launch_reweight(const ReweightParams& prm, bool family, unsigned gri
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr;
-#ifdef UMI_NO_PDL_WAIT
-    cfg.numAttrs = 0;
-#else
     cfg.numAttrs = 1;
-#endif
     const cudaError_t e = cudaLaunchKernelEx(&cfg, k2, prm);
     if (e != cudaSuccess) return e;
     return cudaGetLastError();

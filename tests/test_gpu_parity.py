@@ -361,3 +361,25 @@ def test_concurrent_calls_from_two_host_threads(umi):
         parity.compare_trend(outs[k], refs[k])
     umi.umi_shutdown()
     parity.compare_trend(umi.umi_detrend_host(None, xs[0], cfg.W), refs[0])      # usable again afterwards
+
+
+@pytest.mark.parametrize("W", [25, 361])
+def test_rows_that_are_not_16_byte_aligned(umi, W):
+    # the kernels stage with 128-bit loads when the rows are 16-byte aligned (N = 0 mod 4 and aligned base pointers);
+    # a view that starts 4 bytes into its buffer must take the 32-bit path and give the same bits
+    import torch
+    x = lc.random_series(5000 + W, 160, 2100, nan_frac=0.01, inf_frac=0.0)
+    t = np.tile(np.arange(2100, dtype=np.float64), (160, 1))
+    t[3, 40:90] = np.nan
+    ref = orc.detrend(x, W, time=t)
+    aligned = umi.umi_detrend(torch.from_numpy(t).cuda(), torch.from_numpy(x).cuda(), W)
+    fbuf = torch.empty(x.size + 1, dtype=torch.float32, device="cuda")
+    tbuf = torch.empty(t.size + 1, dtype=torch.float64, device="cuda")
+    fv, tv = fbuf[1:].view(160, 2100), tbuf[1:].view(160, 2100)
+    fv.copy_(torch.from_numpy(x))
+    tv.copy_(torch.from_numpy(t))
+    assert fv.data_ptr() % 16 == 4 and tv.data_ptr() % 16 == 8
+    shifted = umi.umi_detrend(tv, fv, W)
+    torch.cuda.synchronize()
+    parity.compare_trend(shifted.cpu().numpy(), ref)
+    assert torch.equal(torch.nan_to_num(aligned), torch.nan_to_num(shifted))
