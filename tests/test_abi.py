@@ -127,3 +127,17 @@ def test_binding_rejects_host_tensors_on_the_device_path():
     import torch
     with pytest.raises(TypeError):
         umi.umi_detrend(None, torch.zeros(2, 8), 3)
+
+
+def test_bakeoff_library_is_separate_and_exports_its_candidates():
+    # the measured alternatives (csrc/bakeoff/) build into their own library and never into the product one
+    from paper_2604_06602_b200 import build
+    B = ctypes.CDLL(build.build_bakeoff())
+    for name in ("umi_bakeoff_median_radix", "umi_bakeoff_median_warp_sorted", "umi_bakeoff_reweight_warp_window"):
+        assert hasattr(B, name)
+    L = ctypes.CDLL(build.build())
+    assert not hasattr(L, "umi_bakeoff_median_radix")
+    one = ctypes.c_void_p(16)
+    B.umi_bakeoff_median_radix.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
+    assert B.umi_bakeoff_median_radix(one, 1, 10, 4, one, None) == 1        # even window: refused on the host
+    assert B.umi_bakeoff_median_radix(one, 0, 10, 361, one, None) == 0      # empty batch: nothing enqueued
