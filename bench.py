@@ -44,7 +44,7 @@ UNIT = "cadences/s"
 # that figure is not a fraction of any hardware ceiling.
 SM_COUNT = 148
 LANES_PER_SM = 128          # FP32 lanes of the FMA pipe per SM (4 SMSPs x 32)
-FMA_OPS_SMALL = (3, 6)      # fused short-window kernel: Phase 2 (sub, fma, count), a pass (general-alpha form)
+FMA_OPS_SMALL = (3, 6, 5)   # fused short-window kernel: Phase 2 (sub, fma, count), a pass (general alpha), a pass (alpha = 2)
 NOMINAL_PHASE2, NOMINAL_PER_PASS = 4, 9
 SURVEY_FMA_PHASE2, SURVEY_FMA_PER_PASS = 2, 6
 
@@ -52,7 +52,7 @@ SURVEY_FMA_PHASE2, SURVEY_FMA_PER_PASS = 2, 6
 def fma_ops_per_window_sample(W, alpha, n_iter):
     """(executed FMA-pipe lane-operations per window-sample, description) for the kernel that runs this W."""
     if W <= 49:
-        p2, pp = FMA_OPS_SMALL
+        p2, pp = FMA_OPS_SMALL[0], (FMA_OPS_SMALL[2] if alpha == 2.0 else FMA_OPS_SMALL[1])
         return p2 + pp * n_iter, "%d (Phase 2) + %d x %d passes, fused short-window kernel" % (p2, pp, n_iter)
     pp = 5 if alpha in (1.0, 2.0, 4.0) else 6
     return 2 + pp * n_iter, "2 (Phase 2) + %d x %d passes, alpha %s" % (pp, n_iter, "= 2^m: integer-add form" if pp == 5 else "general")

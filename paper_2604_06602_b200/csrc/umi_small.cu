@@ -228,7 +228,7 @@ __device__ __noinline__ void small_position(const float* win, int W, float sent,
    hold WT + 3 samples per thread and get the registers they need */
 constexpr int ks_min_ctas(int wt, bool family) { return wt <= 9 ? 6 : wt <= 17 ? 5 : wt <= 25 ? (family ? 5 : 6) : wt <= 33 ? 4 : 3; }
 
-template <int WT, bool FAMILY>
+template <int WT, bool FAMILY, int APOW>
 __global__ void __launch_bounds__(KS_THREADS, ks_min_ctas(WT, FAMILY))
 umi_small_kernel(const __grid_constant__ ReweightParams prm, int min_valid)   /* (__grid_constant__: small_position takes prm by reference) */
 {
@@ -440,12 +440,31 @@ umi_small_kernel(const __grid_constant__ ReweightParams prm, int min_valid)   /*
                 cs[q] = on[q] ? prm.c * sc : 0.f;
                 k[q] = on[q] ? 1.f / cs[q] : 0.f;
             }
+            /* APOW >= 0 (alpha = 2^APOW): the pairs form alpha*u by an integer add (umi_device.cuh), which would wrap an
+               overflowed -u = k (mu - x) to a small value; warps in which it could overflow (|x|, |mu| <= amax; never seen
+               on real data) take a rolled scalar loop over the staged window instead, which multiplies */
+            bool risky = false;
+            if constexpr (APOW >= 0) {
+                const float amax = 2.f * fmaxf(fabsf(sent), fmaxf(fabsf(tmin), fabsf(tmax)));
+#pragma unroll
+                for (int q = 0; q < 4; ++q) risky = risky || !(k[q] * amax < 1.2676506e30f);   /* 2^100 */
+                risky = __any_sync(0xFFFFFFFFu, risky);
+            }
             /* ---- Phase 3 (Eq. 2-4) ---- */
             for (int it = 0; it < prm.n_iter; ++it) {
                 float S[4], R[4], c0k[4];
 #pragma unroll
                 for (int q = 0; q < 4; ++q) { S[q] = 0.f; R[q] = 0.f; c0k[q] = -mu[q] * k[q]; }
-                if (FAMILY && prm.weight_kind == WEIGHT_WELSCH) {
+                if (APOW >= 0 && risky) {
+#pragma unroll 1
+                    for (int i = 0; i < WT + 3; ++i) {
+                        const float xr = xs[4 * lane + i];
+                        const float x = finite_f32(xr) ? xr : sent;
+#pragma unroll
+                        for (int q = 0; q < 4; ++q)
+                            if (i >= q && i < q + WT) eval_u<false>(x, k[q], c0k[q], nalpha, S[q], R[q]);
+                    }
+                } else if (FAMILY && prm.weight_kind == WEIGHT_WELSCH) {
 #pragma unroll
                     for (int q = 0; q < 4; ++q)
 #pragma unroll
@@ -463,8 +482,8 @@ umi_small_kernel(const __grid_constant__ ReweightParams prm, int min_valid)   /*
 #pragma unroll
                         for (int j = 0; j < NPAIR; ++j) {
                             const f32x2 x2 = pack2(s[first + 2 * j], s[first + 2 * j + 1]);
-                            if (j & 1) eval_weight_pair<-1>(x2, k2, c02, na2, Sb, Rb);
-                            else       eval_weight_pair<-1>(x2, k2, c02, na2, Sa, Ra);
+                            if (j & 1) eval_weight_pair<APOW>(x2, k2, c02, na2, Sb, Rb);
+                            else       eval_weight_pair<APOW>(x2, k2, c02, na2, Sa, Ra);
                         }
                         float S0, S1, R0, R1;
                         unpack2(fadd2(Sa, Sb), S0, S1);
@@ -478,7 +497,7 @@ umi_small_kernel(const __grid_constant__ ReweightParams prm, int min_valid)   /*
                         const f32x2 x2 = pack2(s[q + WT - 1], s[q + 1]);
                         const f32x2 k2 = pack2(-k[q], -k[q + 1]), c02 = pack2(-c0k[q], -c0k[q + 1]);
                         f32x2 Sp = pack2(0.f, 0.f), Rp = Sp;
-                        eval_weight_pair<-1>(x2, k2, c02, na2, Sp, Rp);
+                        eval_weight_pair<APOW>(x2, k2, c02, na2, Sp, Rp);
                         float S0, S1, R0, R1;
                         unpack2(Sp, S0, S1);
                         unpack2(Rp, R0, R1);
@@ -505,16 +524,16 @@ umi_small_kernel(const __grid_constant__ ReweightParams prm, int min_valid)   /*
     }
 }
 
-template <bool FAMILY>
+template <bool FAMILY, int APOW>
 static cudaError_t launch_small_t(const ReweightParams& prm, int min_valid, int wt, unsigned grid, cudaStream_t stream)
 {
     const size_t smem = (size_t)KS_WARPS * (size_t)(KS_WARP_TILE + wt + 3) * sizeof(float);
     switch (wt) {
-    case 9: umi_small_kernel<9, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
-    case 17: umi_small_kernel<17, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
-    case 25: umi_small_kernel<25, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
-    case 33: umi_small_kernel<33, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
-    case 49: umi_small_kernel<49, FAMILY><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
+    case 9: umi_small_kernel<9, FAMILY, APOW><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
+    case 17: umi_small_kernel<17, FAMILY, APOW><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
+    case 25: umi_small_kernel<25, FAMILY, APOW><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
+    case 33: umi_small_kernel<33, FAMILY, APOW><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
+    case 49: umi_small_kernel<49, FAMILY, APOW><<<grid, KS_THREADS, smem, stream>>>(prm, min_valid); break;
     default: return cudaErrorInvalidValue;
     }
     return cudaGetLastError();
@@ -522,11 +541,12 @@ static cudaError_t launch_small_t(const ReweightParams& prm, int min_valid, int 
 
 cudaError_t launch_small(const ReweightParams& prm, bool family, int min_valid, int wt, unsigned grid, cudaStream_t stream)
 {
-    /* the passes keep the multiply form of alpha*u: the integer-add form (umi_device.cuh) was measured on this
-       kernel and does not pay (5.48 -> 5.45 ms at 2,000 config-3 stars, and it needs a second copy of the passes
-       for warps in which -u could overflow): this kernel is bound by issue slots, not by the FMA pipe */
-    return family ? launch_small_t<true>(prm, min_valid, wt, grid, stream)
-                  : launch_small_t<false>(prm, min_valid, wt, grid, stream);
+    /* the paper's default alpha = 2 takes the build that forms alpha*u by an integer add on the bit pattern (umi_device.cuh):
+       5 instead of 6 FMA-pipe lane-operations per evaluation, 5.12 -> 4.86 ms on 2,000 config-3 stars.  (Round 1 measured no
+       gain from it on the CTA-tile kernel with its second unrolled copy of the passes; here the guard is a rolled loop.) */
+    if (family) return launch_small_t<true, -1>(prm, min_valid, wt, grid, stream);
+    if (alpha_pow2(prm.alpha) == 1) return launch_small_t<false, 1>(prm, min_valid, wt, grid, stream);
+    return launch_small_t<false, -1>(prm, min_valid, wt, grid, stream);
 }
 
 } // namespace umi

@@ -172,7 +172,7 @@ def test_overflowing_u_takes_the_multiply_form(umi, n_stars, alpha):
     # gives weight 0 (the trend stays at the median, R11); the integer-add form of alpha*u would wrap a NaN
     # to a small |u_eff| (weight 1), so such warps must take the multiply form (the kernel's `risky` vote).
     x = lc.random_series(1400, n_stars, 2100, nan_frac=0.0, inf_frac=0.0)
-    for W in (51, 361):
+    for W in (25, 51, 361):
         ref = orc.detrend(x, W, alpha=alpha, n_iter=5, c=1e-37)
         got = _gpu(umi, x, W, alpha=alpha, c=1e-37)
         parity.compare_trend(got, ref)
