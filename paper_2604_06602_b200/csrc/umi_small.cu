@@ -478,16 +478,13 @@ umi_small_kernel(const __grid_constant__ ReweightParams prm, int min_valid)   /*
                         constexpr int NPAIR = (WT - 1) / 2;
                         const int first = q + (q & 1);
                         const f32x2 k2 = pack2(-k[q], -k[q]), c02 = pack2(-c0k[q], -c0k[q]);   /* pairs work on -u */
-                        f32x2 Sa = pack2(0.f, 0.f), Sb = Sa, Ra = Sa, Rb = Sa;
+                        f32x2 Sa = pack2(0.f, 0.f), Ra = Sa;              /* one accumulator pair per position: the 4 positions interleave */
 #pragma unroll
-                        for (int j = 0; j < NPAIR; ++j) {
-                            const f32x2 x2 = pack2(s[first + 2 * j], s[first + 2 * j + 1]);
-                            if (j & 1) eval_weight_pair<APOW>(x2, k2, c02, na2, Sb, Rb);
-                            else       eval_weight_pair<APOW>(x2, k2, c02, na2, Sa, Ra);
-                        }
+                        for (int j = 0; j < NPAIR; ++j)
+                            eval_weight_pair<APOW>(pack2(s[first + 2 * j], s[first + 2 * j + 1]), k2, c02, na2, Sa, Ra);
                         float S0, S1, R0, R1;
-                        unpack2(fadd2(Sa, Sb), S0, S1);
-                        unpack2(fadd2(Ra, Rb), R0, R1);
+                        unpack2(Sa, S0, S1);
+                        unpack2(Ra, R0, R1);
                         S[q] = S0 + S1;
                         R[q] = -(R0 + R1);                          /* the pairs summed w*(-u) */
                     }
