@@ -51,7 +51,6 @@ constexpr int K2_THREADS = UMI_K2_THREADS;       /* reweighting kernel */
 constexpr int K2_WARPS = K2_THREADS / 32;        /* every warp owns tiles of its own: no CTA-wide barrier in the kernel */
 constexpr int K2_NPOS = 4;                       /* consecutive positions per thread */
 constexpr int K2_WARP_TILE = 32 * K2_NPOS;       /* positions per warp tile (throughput variant) */
-constexpr int K2_TILE = K2_THREADS * K2_NPOS;    /* positions per CTA and trip of its tile loop */
 #ifndef UMI_K2_SPLIT
 #define UMI_K2_SPLIT 8
 #endif

@@ -153,7 +153,7 @@ __device__ __forceinline__ void eval_scale_group(const f32x2 (&x01)[K2_NPOS], co
    and / or written out).  MODE 2: the same with Welsch weights. */
 /* SPLIT > 1 (small batches, where the grid would not fill the GPU): SPLIT adjacent lanes share the 4
    positions, each taking every SPLIT-th 128-bit group of the windows; the partial sums are combined
-   with xor shuffles after every pass.  A CTA then owns K2_TILE / SPLIT positions and a thread's serial
+   with xor shuffles after every pass.  A warp tile then holds K2_WARP_TILE / SPLIT positions and a thread's serial
    chain is SPLIT times shorter.  SPLIT = 1 is the throughput configuration.
    APOW >= 0: the launch has alpha = 2^APOW and the interior loop forms alpha*u without a multiply;
    warps in which -u could overflow run all their groups through the scalar edge loop instead. */
@@ -313,14 +313,14 @@ umi_reweight_kernel(ReweightParams prm)
         const float4* xs4 = reinterpret_cast<const float4*>(xs) + pt;
 
         if (__any_sync(0xFFFFFFFFu, any_act)) {
-            /* Edge groups hold samples that belong to some but not all of the thread's 4 windows.  They run the
-               same packed arithmetic as the interior groups on MASKED samples: position q sees the (centred)
-               sentinel in place of a sample outside its window -- never above a median, weight exactly 0 -- so
-               no (sample, position) evaluation is predicated.  The lane's edge groups: g < g_lo and g > g_hi. */
-            /* Split-window variant: the lane's groups g = sl, sl + SPLIT, ... < G in three runs: [sl, g_first) low
-               edge groups; [g_first, g_tail) interior groups, a multiple of 8 of them, through the unrolled loop;
-               [g_tail, G) the rest -- up to 7 interior groups and the high edge groups -- through the same rolled,
-               masked loop as the low edge groups (one copy of that loop body). */
+            /* Edge groups hold samples that belong to some but not all of the thread's 4 windows.  The throughput variant
+               (SPLIT = 1) runs its two or three of them one (sample, position) at a time, predicated.  The split-window
+               variant, where a lane has ~1/SPLIT of the groups and the edge groups weigh SPLIT times more, runs them through
+               the same packed arithmetic as the interior groups on MASKED samples: position q sees the (centred) sentinel
+               in place of a sample outside its window -- never above a median, weight exactly 0.  There the lane's groups
+               g = sl, sl + SPLIT, ... < G fall into three runs: [sl, g_first) low edge groups; [g_first, g_tail) interior
+               groups, a multiple of 8 of them, through the unrolled loop; [g_tail, G) the rest -- up to 7 interior groups and
+               the high edge groups -- through the same rolled, masked loop as the low edge groups (one copy of its body). */
             constexpr int UNR = K2_UNROLL;
             int g_tail = g_first;
             if (g_first <= g_hi) g_tail += ((g_hi - g_first) / SPLIT + 1) / UNR * (UNR * SPLIT);
