@@ -391,11 +391,18 @@ umi_reweight_kernel(ReweightParams prm)
                 for (int g = sl; g < (given ? 0 : G); g += SPLIT) {
                     const float4 v = xs4[g];
                     const float xv[4] = {v.x, v.y, v.z, v.w};
+                    if (g >= g_lo && g <= g_hi) {                   /* interior: every sample in all 4 windows */
 #pragma unroll
-                    for (int q = 0; q < K2_NPOS; ++q)
+                        for (int q = 0; q < K2_NPOS; ++q)
 #pragma unroll
-                        for (int r = 0; r < 4; ++r)
-                            if ((unsigned)(4 * g + r - delta - q) <= two_h) eval_scale(xv[r], mu[q], ss[q], cnt[q]);
+                            for (int r = 0; r < 4; ++r) eval_scale(xv[r], mu[q], ss[q], cnt[q]);
+                    } else {
+#pragma unroll
+                        for (int q = 0; q < K2_NPOS; ++q)
+#pragma unroll
+                            for (int r = 0; r < 4; ++r)
+                                if ((unsigned)(4 * g + r - delta - q) <= two_h) eval_scale(xv[r], mu[q], ss[q], cnt[q]);
+                    }
                 }
             }
             if constexpr (SPLIT > 1) {
