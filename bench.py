@@ -66,7 +66,7 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, choices=sorted(lc.CONFIGS))
     ap.add_argument("--stars", type=int, default=None, help="override the star count (debug)")
-    ap.add_argument("--row", default="base", choices=["base", "f1", "f2", "f4mad", "f4welsch"],
+    ap.add_argument("--row", default="base", choices=["base", "f1", "f2", "f2seg", "f4mad", "f4welsch"],
                     help="SURVEY.md 8(f) next rows on the same workload: f1 = umi_flatten, f2 = umi_detrend_gapped on the "
                          "compacted rows, f4mad / f4welsch = umi_detrend_family (symmetric biweight on the MAD / Welsch)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -409,19 +409,22 @@ def run_row(args, cfg, local_rank):
     if args.row == "f1":
         fn = lambda: umi.umi_flatten(None, d_flux, W, stream=stream, **kw)
         what = "umi_flatten: trend + flux/trend in the kernels' epilogue"
-    elif args.row == "f2":
+    elif args.row in ("f2", "f2seg"):
         t_np, f_np, _ = lc.compact(flux_np, cfg.dt_days, t0=1000.0, jitter=0.1, seed=args.config)
         d_t, d_f = torch.from_numpy(t_np).to(dev), torch.from_numpy(f_np).to(dev)
-        ws = torch.empty(umi.umi_gapped_workspace_bytes(S, N), dtype=torch.uint8, device=dev)
+        seg = dict(break_slots=W - 1, min_segment=W // 3, edge_cut=W // 10) if args.row == "f2seg" else {}
+        nbytes = umi.umi_gapped_ex_workspace_bytes(S, N) if seg else umi.umi_gapped_workspace_bytes(S, N)
+        ws = torch.empty(nbytes, dtype=torch.uint8, device=dev)
         fn = lambda: umi.umi_detrend_gapped(d_t, d_f, 1000.0, cfg.dt_days, N, W, flat=True, workspace=ws,
-                                            stream=stream, **kw)
-        what = "umi_detrend_gapped: compacted rows [%d x %d] + fp64 time -> grid [%d x %d] -> trend, flat" % (
-            S, f_np.shape[1], S, N)
+                                            stream=stream, **seg, **kw)
+        what = "umi_detrend_gapped%s: compacted rows [%d x %d] + fp64 time -> grid [%d x %d] -> trend, flat" % (
+            " with segments (break W-1 slots, min_segment W/3, edge_cut W/10)" if seg else "", S, f_np.shape[1], S, N)
         M = f_np.shape[1]
         # algorithmic bytes of the two regrid kernels + the NaN fill: scatter reads time (8) + flux (4) per
         # sample and writes 4 per valid sample; the fill writes 4 per slot; gather reads time (8) + flux (4)
         # + trend (4) and writes trend (4) + flat (4)
-        extra["regrid_bytes"] = int(S * M * (12 + 4) + S * N * 4 + S * M * (16 + 8))
+        if not seg:
+            extra["regrid_bytes"] = int(S * M * (12 + 4) + S * N * 4 + S * M * (16 + 8))
     else:
         wk = 1 if args.row == "f4welsch" else 0
         fn = lambda: umi.umi_detrend_family(None, d_flux, W, 1, wk, alpha=1.0, n_iter=cfg.n_iter, stream=stream)
@@ -449,7 +452,7 @@ def run_row(args, cfg, local_rank):
     base_ms = timed(base)
     row_ms = timed(fn)
     clocks = sampler.stop()
-    n_cad = int(np.isfinite(flux_np).sum()) if args.row == "f2" else S * N
+    n_cad = int(np.isfinite(flux_np).sum()) if args.row in ("f2", "f2seg") else S * N
     line = {"metric": METRIC, "row": args.row, "what": what, "value": n_cad / (row_ms * 1e-3), "unit": UNIT,
             "n_gpus": 1, "steps": args.steps, "warmup": max(args.warmup, 3), "ms_per_step": row_ms,
             "base_path_ms_per_step": base_ms, "overhead_ms": row_ms - base_ms, "higher_is_better": True,

@@ -138,6 +138,8 @@ umi_regrid_gather_kernel(RegridParams prm, const float* __restrict__ grid_trend,
  * `scratch`), backward (last slot and size of the segment).  Windows need no clipping: the entry point only
  * accepts break_slots >= h, and a window of half-width h cannot reach across more than h - 1 empty slots.
  */
+constexpr int SEG_BATCH = 8;                            /* chunks of 32 slots whose loads are issued together */
+
 __global__ void __launch_bounds__(128)
 umi_regrid_segments_kernel(float* __restrict__ grid_flux, uint8_t* __restrict__ grid_cut, int2* __restrict__ scratch,
                            int64_t n_stars, int64_t n_grid, int64_t break_slots, int64_t min_segment, int64_t edge_cut)
@@ -152,55 +154,79 @@ umi_regrid_segments_kernel(float* __restrict__ grid_flux, uint8_t* __restrict__ 
         /* forward: (first slot of the segment, index inside it) of every valid slot */
         bool have_prev = false;
         int64_t prev_slot = 0, cur_first = 0, cur_cnt = 0;
-        for (int64_t base = 0; base < n_grid; base += 32) {
-            const int64_t k = base + lane;
-            const bool valid = k < n_grid && finite_f32(frow[k]);
-            const unsigned vb = __ballot_sync(0xFFFFFFFFu, valid);
-            const int p = 31 - __clz((int)(vb & lt));                               /* previous valid lane, -1: none */
-            const bool none = p < 0 && !have_prev;
-            const int64_t ps = p >= 0 ? base + p : prev_slot;
-            const bool start = valid && (none || (break_slots >= 0 && k - ps - 1 > break_slots));
-            const unsigned sb = __ballot_sync(0xFFFFFFFFu, start);
-            if (valid) {
-                const int st = 31 - __clz((int)(sb & le));                          /* start lane of my segment, -1: before this chunk */
-                int2 rec;
-                if (st >= 0) { rec.x = (int)(base + st); rec.y = __popc(vb & le & ~((1u << st) - 1u)) - 1; }
-                else { rec.x = (int)cur_first; rec.y = (int)cur_cnt + __popc(vb & lt); }
-                srow[k] = rec;
+        for (int64_t base0 = 0; base0 < n_grid; base0 += 32 * SEG_BATCH) {
+            bool vld[SEG_BATCH];                                    /* the chain between chunks is scalar: all loads of a batch first */
+#pragma unroll
+            for (int c = 0; c < SEG_BATCH; ++c) {
+                const int64_t k = base0 + 32 * c + lane;
+                vld[c] = k < n_grid && finite_f32(__ldcs(frow + k));
             }
-            if (vb) { prev_slot = base + 31 - __clz((int)vb); have_prev = true; }
-            if (sb) { const int ls = 31 - __clz((int)sb); cur_first = base + ls; cur_cnt = __popc(vb & ~((1u << ls) - 1u)); }
-            else cur_cnt += __popc(vb);
+#pragma unroll
+            for (int c = 0; c < SEG_BATCH; ++c) {
+                const int64_t base = base0 + 32 * c;
+                if (base >= n_grid) break;
+                const int64_t k = base + lane;
+                const bool valid = vld[c];
+                const unsigned vb = __ballot_sync(0xFFFFFFFFu, valid);
+                const int p = 31 - __clz((int)(vb & lt));                           /* previous valid lane, -1: none */
+                const bool none = p < 0 && !have_prev;
+                const int64_t ps = p >= 0 ? base + p : prev_slot;
+                const bool start = valid && (none || (break_slots >= 0 && k - ps - 1 > break_slots));
+                const unsigned sb = __ballot_sync(0xFFFFFFFFu, start);
+                if (valid) {
+                    const int st = 31 - __clz((int)(sb & le));                      /* start lane of my segment, -1: before this chunk */
+                    int2 rec;
+                    if (st >= 0) { rec.x = (int)(base + st); rec.y = __popc(vb & le & ~((1u << st) - 1u)) - 1; }
+                    else { rec.x = (int)cur_first; rec.y = (int)cur_cnt + __popc(vb & lt); }
+                    srow[k] = rec;
+                }
+                if (vb) { prev_slot = base + 31 - __clz((int)vb); have_prev = true; }
+                if (sb) { const int ls = 31 - __clz((int)sb); cur_first = base + ls; cur_cnt = __popc(vb & ~((1u << ls) - 1u)); }
+                else cur_cnt += __popc(vb);
+            }
         }
         __syncwarp();
         /* backward: (last slot, size) of the segment; short segments erased, edges marked */
         bool have_next = false;
         int64_t next_slot = 0, cur_last = 0, cur_total = 0;
-        for (int64_t base = ((n_grid - 1) / 32) * 32; base >= 0; base -= 32) {
-            const int64_t k = base + lane;
-            const bool valid = k < n_grid && finite_f32(frow[k]);
-            const unsigned vb = __ballot_sync(0xFFFFFFFFu, valid);
-            const int nx = __ffs((int)(vb & gt)) - 1;                               /* next valid lane, -1: none */
-            const bool none = nx < 0 && !have_next;
-            const int64_t ns = nx >= 0 ? base + nx : next_slot;
-            const bool end = valid && (none || (break_slots >= 0 && ns - k - 1 > break_slots));
-            const unsigned eb = __ballot_sync(0xFFFFFFFFu, end);
-            int2 rec = make_int2(0, 0);
-            if (valid) rec = srow[k];
-            const int en = __ffs((int)(eb & ~lt)) - 1;                              /* end lane of my segment, -1: after this chunk */
-            const int idx_at_end = __shfl_sync(0xFFFFFFFFu, rec.y, en >= 0 ? en : 0);
-            const int64_t last = en >= 0 ? base + en : cur_last;
-            const int64_t total = en >= 0 ? (int64_t)idx_at_end + 1 : cur_total;
-            if (k < n_grid) {
-                const bool drop = valid && min_segment > 0 && total < min_segment;
-                if (drop) frow[k] = qnan;
-                crow[k] = (valid && !drop && edge_cut > 0 && (k - rec.x < edge_cut || last - k < edge_cut)) ? 1 : 0;
+        const int64_t top = ((n_grid - 1) / 32) * 32;
+        for (int64_t base0 = top; base0 >= 0; base0 -= 32 * SEG_BATCH) {
+            bool vld[SEG_BATCH];
+            int2 recs[SEG_BATCH];
+#pragma unroll
+            for (int c = 0; c < SEG_BATCH; ++c) {
+                const int64_t k = base0 - 32 * c + lane;
+                vld[c] = k >= 0 && k < n_grid && finite_f32(frow[k]);
+                recs[c] = vld[c] ? srow[k] : make_int2(0, 0);
             }
-            if (vb) { next_slot = base + __ffs((int)vb) - 1; have_next = true; }
-            if (eb) {
-                const int fe = __ffs((int)eb) - 1;
-                cur_last = base + fe;
-                cur_total = (int64_t)__shfl_sync(0xFFFFFFFFu, rec.y, fe) + 1;
+#pragma unroll
+            for (int c = 0; c < SEG_BATCH; ++c) {
+                const int64_t base = base0 - 32 * c;
+                if (base < 0) break;
+                const int64_t k = base + lane;
+                const bool valid = vld[c];
+                const int2 rec = recs[c];
+                const unsigned vb = __ballot_sync(0xFFFFFFFFu, valid);
+                const int nx = __ffs((int)(vb & gt)) - 1;                           /* next valid lane, -1: none */
+                const bool none = nx < 0 && !have_next;
+                const int64_t ns = nx >= 0 ? base + nx : next_slot;
+                const bool end = valid && (none || (break_slots >= 0 && ns - k - 1 > break_slots));
+                const unsigned eb = __ballot_sync(0xFFFFFFFFu, end);
+                const int en = __ffs((int)(eb & ~lt)) - 1;                          /* end lane of my segment, -1: after this chunk */
+                const int idx_at_end = __shfl_sync(0xFFFFFFFFu, rec.y, en >= 0 ? en : 0);
+                const int64_t last = en >= 0 ? base + en : cur_last;
+                const int64_t total = en >= 0 ? (int64_t)idx_at_end + 1 : cur_total;
+                if (k < n_grid) {
+                    const bool drop = valid && min_segment > 0 && total < min_segment;
+                    if (drop) frow[k] = qnan;
+                    crow[k] = (valid && !drop && edge_cut > 0 && (k - rec.x < edge_cut || last - k < edge_cut)) ? 1 : 0;
+                }
+                if (vb) { next_slot = base + __ffs((int)vb) - 1; have_next = true; }
+                if (eb) {
+                    const int fe = __ffs((int)eb) - 1;
+                    cur_last = base + fe;
+                    cur_total = (int64_t)__shfl_sync(0xFFFFFFFFu, rec.y, fe) + 1;
+                }
             }
         }
     }
