@@ -44,3 +44,27 @@ def test_injection_metric_with_a_perfect_and_a_transit_eating_detrender():
     eater = lambda x: np.ones_like(x)                     # trend == flux: everything absorbed
     err = ir.depth_errors(flux, cfg.dt_days, eater, depths_ppm=(1000.0,))
     assert abs(err[0] - 100.0) < 1e-6
+
+
+def test_bench_roofline_bookkeeping():
+    # bench.py's host-side roofline arithmetic: executed FMA-pipe lane-operations per window-sample per kernel build,
+    # the exact window-sample count, and the committed ncu record it quotes beside the live figure
+    import bench
+    assert bench.fma_ops_per_window_sample(361, 2.0, 5)[0] == 27        # 2 + 5 x 5: alpha = 2^m, integer-add form
+    assert bench.fma_ops_per_window_sample(361, 3.0, 5)[0] == 32        # 2 + 6 x 5: general alpha
+    assert bench.fma_ops_per_window_sample(25, 2.0, 5)[0] == 28         # fused short-window kernel, alpha = 2
+    assert bench.fma_ops_per_window_sample(25, 3.0, 5)[0] == 33
+    x = np.ones((2, 50), np.float32)
+    x[0, 10:20] = np.nan
+    # W = 5, min_valid = 1: every valid position counts its valid window members (brute force below)
+    want = 0
+    for b in range(2):
+        for i in range(50):
+            if np.isfinite(x[b, i]):
+                want += int(np.isfinite(x[b, max(0, i - 2):i + 3]).sum())
+    assert bench.exact_window_samples(x, 5, 1) == want
+    rec = bench.ncu_record(2, 1000, "umi_reweight_kernel")
+    assert rec is not None and rec["kernel"].startswith("umi_reweight_kernel<0, 1, 1>")
+    assert 50.0 < rec["fma_pipe_pct"] <= 100.0 and rec["local_ld"] == 0 and rec["local_st"] == 0
+    assert bench.ncu_record(2, 999, "umi_reweight_kernel") is None      # no capture of that size: no number
+    assert bench.ncu_record(3, 10000, "umi_small_kernel")["registers"] <= 80
