@@ -224,7 +224,8 @@ __device__ __noinline__ void small_position(const float* win, int W, float sent,
 } // namespace
 
 /* resident CTAs per SM the register allocation aims at: 6 for W = 25 (80 registers, nothing spilled; measured 5.30 ms on
-   2,000 config-3 stars against 5.38 with the compiler's own choice of 96 registers and 5.34 at 7 CTAs); the longer windows
+   2,000 config-3 stars against 5.38 with the compiler's own choice of 96 registers and 5.34 at 7 CTAs; the alpha = 2
+   build: 4 / 5 / 6 / 7 / 8 CTAs = 5.16 / 5.02 / 4.89 / 4.98 / 5.02 ms); the longer windows
    hold WT + 3 samples per thread and get the registers they need */
 constexpr int ks_min_ctas(int wt, bool family) { return wt <= 9 ? 6 : wt <= 17 ? 5 : wt <= 25 ? (family ? 5 : 6) : wt <= 33 ? 4 : 3; }
 
