@@ -249,7 +249,7 @@ umi_reweight_kernel(ReweightParams prm)
         bool act[K2_NPOS];
         bool any_act = false;
         unsigned has_med = 0u;                              /* bit q: position q has a median, i.e. a trend */
-        float mmin = INFINITY, mmax = -INFINITY;            /* range of the tile's medians */
+        float rabs = INFINITY, rval = 0.f;                  /* the tile's median of smallest magnitude: the reference */
 #pragma unroll
         for (int q = 0; q < K2_NPOS; ++q) {
             const int jl = 4 * pt + q;                      /* position inside the tile (32-bit from here on) */
@@ -269,7 +269,7 @@ umi_reweight_kernel(ReweightParams prm)
             has_med |= act[q] ? (1u << q) : 0u;
             any_act = any_act || act[q];
             mu[q] = act[q] ? med : 0.f;
-            if (act[q]) { mmin = fminf(mmin, med); mmax = fmaxf(mmax, med); }
+            if (act[q] && fabsf(med) < rabs) { rabs = fabsf(med); rval = med; }
             kk[q] = 0.f;
             cs[q] = 0.f;
             if constexpr (MODE != 0) {                              /* no trend, no scale */
@@ -281,8 +281,8 @@ umi_reweight_kernel(ReweightParams prm)
         for (int o = 16; o > 0; o >>= 1) {
             tmin = fminf(tmin, __shfl_xor_sync(0xFFFFFFFFu, tmin, o));
             tmax = fmaxf(tmax, __shfl_xor_sync(0xFFFFFFFFu, tmax, o));
-            mmin = fminf(mmin, __shfl_xor_sync(0xFFFFFFFFu, mmin, o));
-            mmax = fmaxf(mmax, __shfl_xor_sync(0xFFFFFFFFu, mmax, o));
+            const float oabs = __shfl_xor_sync(0xFFFFFFFFu, rabs, o), oval = __shfl_xor_sync(0xFFFFFFFFu, rval, o);
+            if (oabs < rabs || (oabs == rabs && oval < rval)) { rabs = oabs; rval = oval; }   /* (every lane ends with the same pick) */
         }
         /* sentinel: alpha*(mu - x)/(c s) >= 2 for every window of the tile, since
            mu >= tmin and s <= 0.6745 (tmax - tmin)  ("Sentinel") */
@@ -294,11 +294,14 @@ umi_reweight_kernel(ReweightParams prm)
                 sent = tmin - (MODE == 2 ? 24.f : 2.f) * prm.c_over_alpha * (tmax - tmin);
             sent = fmaxf(sent, -3.0e38f);
         }
-        /* Everything below works on samples centred on the middle of the range of the tile's MEDIANS: Eq. 4 is
-           then mu' = sum(w x') / sum(w) with |x'| small for every sample that can carry weight, i.e. exact to
-           fp32 without a separate sum of w*u.  The medians are robust, so a wild sample (a fill value, a
-           glitch of any size) keeps its own magnitude and leaves the precision of the others alone. */
-        const float xref = (mmin <= mmax) ? 0.5f * mmin + 0.5f * mmax : 0.f;
+        /* Everything below works on samples centred on ONE OF THE TILE'S MEDIANS, the one of smallest magnitude: Eq. 4 is
+           then mu' = sum(w x') / sum(w) with |x'| small for every sample that can carry weight, i.e. exact to fp32 without
+           a separate sum of w*u.  A median is robust: a wild sample (a fill value, a glitch of any size) cannot move it,
+           keeps its own magnitude in x' and leaves the precision of the others alone.  And the smallest one is safe when
+           the tile's medians themselves disagree (the edge of a run of unmasked fill values: medians of -9999 next to
+           medians of 1): |x_ref| <= |median of p| for every position p, so the samples near p's median lose at most one
+           bit to the centring, whatever the other positions of the tile look like. */
+        const float xref = (rabs < INFINITY) ? rval : 0.f;
         const float xsent = sent - xref;                    /* the sentinel as staged */
         const float xabs = (tmin <= tmax) ? fmaxf(fabsf(xsent), fabsf(tmax - xref)) : 0.f;         /* max |x'| staged */
         __syncwarp();                                       /* every lane has read its medians from xs */

@@ -160,7 +160,13 @@ __device__ __noinline__ void small_position(const float* win, int W, float sent,
     (void)sample(h, own_ok);
     const bool has = in_row && own_ok && n >= min_valid && n > 0;   /* (R4, R5) */
 
-    float mu = med;
+    /* mu is carried as an unevaluated pair hi + lo, and every residual is formed as (x - mu_hi) - mu_lo: the subtraction is
+       exact for the samples near mu, which are the ones that carry weight, wherever mu ends up -- next to the median (then
+       one ulp of a single fp32 mu, 6e-8 of the flux, would be ~2e-5 in units of u, which an expanding iteration amplifies:
+       heavy ties under alpha = 10, c = 2.5 with 9 passes gave 1.8e-5 in one of 3,000 random cases) or far from it (two valid
+       samples {-9999, 4.0}, min_valid = 1: the median is -9999 and the passes converge on 4.0006).  One more subtraction per
+       evaluation: this is the path that can afford it. */
+    float mu = med, mu_lo = 0.f;
     const bool want_scale = FAMILY && prm.scale_out != nullptr;
     if ((prm.n_iter > 0 || want_scale) && has) {
         bool on;
@@ -201,23 +207,30 @@ __device__ __noinline__ void small_position(const float* win, int W, float sent,
         const float k = on ? 1.f / cs : 0.f;
         /* ---- Phase 3 (Eq. 2-4) ---- */
         for (int it = 0; it < prm.n_iter; ++it) {
-            const float c0 = -mu * k;
+            const float c0 = -mu_lo * k;
             float S = 0.f, R = 0.f;
             for (int i = 0; i < W; ++i) {
                 const float xr = win[i];
-                const float x = finite_f32(xr) ? xr : sent;
+                const float x = (finite_f32(xr) ? xr : sent) - mu;
                 if (FAMILY && prm.weight_kind == WEIGHT_WELSCH) eval_u<true>(x, k, c0, nalpha, S, R);
                 else eval_u<false>(x, k, c0, nalpha, S, R);
             }
-            if (on && S > 0.f) mu = fmaf(R / S, cs, mu);            /* Eq. 4; (R11) */
+            if (on && S > 0.f) {                                    /* Eq. 4; (R11): (mu, mu_lo) += cs R / S, error-free */
+                const float step = (R / S) * cs;
+                const float t = mu + step, bb = t - mu;
+                const float lo = ((mu - (t - bb)) + (step - bb)) + mu_lo;
+                mu = t + lo;
+                mu_lo = lo - (mu - t);
+            }
         }
     } else if (want_scale && in_row) {
         prm.scale_out[gidx] = qnan;
     }
     if (in_row) {
-        prm.out[gidx] = has ? mu : qnan;
+        const float tr = mu;                                        /* hi of the normalised pair = fl(hi + lo) */
+        prm.out[gidx] = has ? tr : qnan;
         if (prm.flat != nullptr)                                    /* PAPER.md:155 normalisation */
-            prm.flat[gidx] = has ? win[h] / mu : qnan;
+            prm.flat[gidx] = has ? win[h] / tr : qnan;
     }
 }
 
@@ -395,9 +408,27 @@ umi_small_kernel(const __grid_constant__ ReweightParams prm, int min_valid)   /*
             mu[q] = med[q];
         }
         const float own[4] = {s[M], s[M + 1], s[M + 2], s[M + 3]};   /* the positions' own samples (for flux / trend) */
+        /* From here on everything is CENTRED on one of the thread's own medians, the one of smallest magnitude (a robust
+           reference, chosen as in umi_reweight.cu): x' = x - ref is exact for every sample that can carry weight, and mu
+           is carried as an offset, so its fp32 rounding is relative to the residuals and not to the flux.  (On raw samples
+           one ulp of mu is 6e-8 of the flux -- ~2e-5 in units of u -- which an expanding iteration, e.g. heavy ties under
+           alpha = 10, c = 2.5 with 9 passes, amplifies; small_position has the case that was measured.) */
+        float ref = 0.f, rabs = INFINITY;
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            if (has[q] && fabsf(med[q]) < rabs) { rabs = fabsf(med[q]); ref = med[q]; }
+        const float xsent = sent - ref;
         if (!clean) {
 #pragma unroll
-            for (int i = 0; i < NSAMP; ++i) s[i] = ((inv >> i) & 1) ? sent : s[i];
+            for (int i = 0; i < NSAMP; ++i) s[i] = ((inv >> i) & 1) ? xsent : s[i] - ref;
+        } else {
+#pragma unroll
+            for (int i = 0; i < NSAMP; ++i) s[i] -= ref;
+        }
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            med[q] = has[q] ? med[q] - ref : 0.f;
+            mu[q] = med[q];
         }
         const bool want_scale = FAMILY && prm.scale_out != nullptr;
         if (prm.n_iter > 0 || want_scale) {
@@ -446,7 +477,7 @@ umi_small_kernel(const __grid_constant__ ReweightParams prm, int min_valid)   /*
                on real data) take a rolled scalar loop over the staged window instead, which multiplies */
             bool risky = false;
             if constexpr (APOW >= 0) {
-                const float amax = 2.f * fmaxf(fabsf(sent), fmaxf(fabsf(tmin), fabsf(tmax)));
+                const float amax = 4.f * fmaxf(fabsf(sent), fmaxf(fabsf(tmin), fabsf(tmax)));   /* |x - ref|, |mu - ref| <= 2 max|x| */
 #pragma unroll
                 for (int q = 0; q < 4; ++q) risky = risky || !(k[q] * amax < 1.2676506e30f);   /* 2^100 */
                 risky = __any_sync(0xFFFFFFFFu, risky);
@@ -460,7 +491,7 @@ umi_small_kernel(const __grid_constant__ ReweightParams prm, int min_valid)   /*
 #pragma unroll 1
                     for (int i = 0; i < WT + 3; ++i) {
                         const float xr = xs[4 * lane + i];
-                        const float x = finite_f32(xr) ? xr : sent;
+                        const float x = finite_f32(xr) ? xr - ref : xsent;
 #pragma unroll
                         for (int q = 0; q < 4; ++q)
                             if (i >= q && i < q + WT) eval_u<false>(x, k[q], c0k[q], nalpha, S[q], R[q]);
@@ -514,8 +545,9 @@ umi_small_kernel(const __grid_constant__ ReweightParams prm, int min_valid)   /*
         for (int q = 0; q < 4; ++q) {
             if (jq + q < prm.N) {
                 const int64_t gi = star * prm.N + jq + q;
-                prm.out[gi] = has[q] ? mu[q] : qnan;
-                if (prm.flat != nullptr) prm.flat[gi] = has[q] ? own[q] / mu[q] : qnan;   /* PAPER.md:155 normalisation */
+                const float tr = mu[q] + ref;
+                prm.out[gi] = has[q] ? tr : qnan;
+                if (prm.flat != nullptr) prm.flat[gi] = has[q] ? own[q] / tr : qnan;   /* PAPER.md:155 normalisation */
             }
         }
         __syncwarp();                                               /* the slice is free for the next tile */

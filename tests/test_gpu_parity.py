@@ -383,3 +383,36 @@ def test_rows_that_are_not_16_byte_aligned(umi, W):
     torch.cuda.synchronize()
     parity.compare_trend(shifted.cpu().numpy(), ref)
     assert torch.equal(torch.nan_to_num(aligned), torch.nan_to_num(shifted))
+
+
+@pytest.mark.parametrize("W", [25, 29, 361])
+def test_expanding_iteration_under_heavy_ties(umi, W):
+    # flux quantised to a handful of levels under the aggressive preset (alpha = 10, c = 2.5) with 9 passes: dozens of
+    # tied samples sit near the cut-off together and one ulp of mu moves the result by hundreds of ulps.  Round 1
+    # excluded this from its fuzz test; a randomised run of 3,000 cases found it again in the short-window kernel
+    # (1.8e-5 at W = 29) while mu was still carried on raw samples there.  With mu carried as an offset from a
+    # median in every kernel the 1e-5 bar holds with nothing excluded.
+    for seed in range(4):
+        x = lc.random_series(7700 + 10 * W + seed, 150, 2014, nan_frac=0.02, inf_frac=0.0, ties=True)
+        t = np.tile(np.arange(2014, dtype=np.float64), (150, 1))
+        t[np.random.default_rng(seed).random(t.shape) < 0.01] = np.nan
+        _both(umi, x, W, alpha=10.0, c=2.5, n_iter=9, time=t)
+
+
+@pytest.mark.parametrize("n_stars", [2, 160])
+@pytest.mark.parametrize("W", [25, 361])
+def test_runs_of_unmasked_fill_values(umi, n_stars, W):
+    # a run of -9999 longer than half a window makes the MEDIANS inside it -9999 while the medians next to it stay ~1: the
+    # passes are centred on the tile's median of smallest magnitude, so the positions outside the run keep their precision
+    # (a mid-range of the medians would sit at -4999 and cost every position of the tile 12 bits)
+    x = lc.random_series(6000 + W, n_stars, 2100, nan_frac=0.01, inf_frac=0.0)
+    rng = np.random.default_rng(W + n_stars)
+    for b in range(n_stars):
+        a = int(rng.integers(100, 2100 - 2 * W))
+        x[b, a:a + W // 2 + int(rng.integers(5, W))] = -9999.0
+    _both(umi, x, W)
+    ref = orc.detrend(x, W)
+    got = _gpu(umi, x, W).astype(np.float64)
+    calm = np.isfinite(ref.trend64) & (np.abs(ref.trend64 - 1.0) < 0.1) & ~ref.near_cutoff.astype(bool)
+    assert calm.sum() > 0.3 * x.size
+    assert (np.abs(got[calm] - ref.trend64[calm]) <= 5e-7 * np.abs(ref.trend64[calm])).all()
