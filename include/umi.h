@@ -36,11 +36,11 @@
  *    bit-exact always.  The trend of a star may differ in its last bits (~1e-7 relative) between calls
  *    with different batch sizes, because small batches run the split-window variant of the
  *    reweighting kernel, which sums the same terms in another order.
- *  - Supported dynamic range (windows longer than 49 samples): the passes run on samples
- *    centred on the mid-range of the medians of 128 consecutive positions, so the 1e-5
- *    bar on the trend is relative to the LARGEST |median| among those 128 positions (for a
- *    light curve: the local flux); isolated samples of any finite magnitude (fill values,
- *    glitches) cost the others no precision.  (max - min) * 16 * max(1, 1/alpha) over the
+ *  - Supported dynamic range: the passes run on samples centred on one of the medians of
+ *    the 128 consecutive positions a warp owns (4 for windows of at most 49 samples), the
+ *    one of smallest magnitude, so the 1e-5 bar on the trend holds relative to the
+ *    position's own |median| (for a light curve: the local flux); samples of any finite
+ *    magnitude (fill values, glitches, whole runs of them) cost the others no precision.  (max - min) * 16 * max(1, 1/alpha) over the
  *    valid samples of those positions' windows must be finite in fp32.
  */
 #ifndef UMI_B200_H

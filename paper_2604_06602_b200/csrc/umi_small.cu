@@ -422,8 +422,9 @@ umi_small_kernel(const __grid_constant__ ReweightParams prm, int min_valid)   /*
 #pragma unroll
             for (int i = 0; i < NSAMP; ++i) s[i] = ((inv >> i) & 1) ? xsent : s[i] - ref;
         } else {
+            const f32x2 nref2 = pack2(-ref, -ref);                  /* NSAMP is even: register-aligned pairs, as the passes use them */
 #pragma unroll
-            for (int i = 0; i < NSAMP; ++i) s[i] -= ref;
+            for (int i = 0; i < NSAMP; i += 2) unpack2(fadd2(pack2(s[i], s[i + 1]), nref2), s[i], s[i + 1]);
         }
 #pragma unroll
         for (int q = 0; q < 4; ++q) {
