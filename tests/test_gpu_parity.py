@@ -416,3 +416,50 @@ def test_runs_of_unmasked_fill_values(umi, n_stars, W):
     calm = np.isfinite(ref.trend64) & (np.abs(ref.trend64 - 1.0) < 0.1) & ~ref.near_cutoff.astype(bool)
     assert calm.sum() > 0.3 * x.size
     assert (np.abs(got[calm] - ref.trend64[calm]) <= 5e-7 * np.abs(ref.trend64[calm])).all()
+
+
+def test_two_hundred_random_cases(umi):
+    # the randomised comparison behind DESIGN.md 5.3 in small: window, shape, batch size, parameters, time stamps and the
+    # entry point (device, fused normalisation, host batch driver) drawn at random; nothing excluded
+    import torch
+    worst = 0.0
+    for case in range(200):
+        rng = np.random.default_rng(31000 + case)
+        W = int(rng.choice([3, 5, 9, 11, 17, 21, 25, 29, 33, 41, 49, 51, 53, 77, 101, 215, 217, 301, 361, 385, 387, 511, 683, 685, 801, 1279])) | 1
+        S = int(rng.choice([1, 2, 3, 7, 40, 150, 300]))
+        N = int(rng.integers(1, 2600)) if S > 7 else int(rng.integers(1, 9000))
+        alpha = float(rng.choice([0.5, 1.0, 2.0, 2.0, 2.0, 3.0, 4.0, 10.0]))
+        c = float(rng.choice([2.5, 5.0, 5.0, 8.0]))
+        n_iter = int(rng.choice([0, 1, 3, 5, 5, 9]))
+        mv = int(rng.choice([-1, -1, 1, max(1, W // 2)]))
+        x = lc.random_series(32000 + case, S, N, nan_frac=float(rng.choice([0.0, 0.02, 0.2])),
+                             inf_frac=float(rng.choice([0.0, 0.01])), ties=bool(rng.integers(0, 2)))
+        x = (x * float(rng.choice([1.0, 1e-2, 1e3])) + float(rng.choice([0.0, 0.0, 3.0]))).astype(np.float32)
+        t = None
+        if rng.integers(0, 3) == 0:
+            t = np.tile(np.arange(N, dtype=np.float64), (S, 1))
+            t[rng.random((S, N)) < 0.01] = np.nan
+        kw = {} if mv < 0 else {"min_valid": mv}
+        ref = orc.detrend(x, W, alpha=alpha, n_iter=n_iter, c=c, time=t, **kw)
+        xd = torch.from_numpy(x).cuda()
+        td = None if t is None else torch.from_numpy(t).cuda()
+        mode = int(rng.integers(0, 3))
+        if mode == 1:
+            got, flat = umi.umi_flatten(td, xd, W, alpha=alpha, n_iter=n_iter, c=c, min_valid=mv)
+        elif mode == 2 and mv < 0 and c == 5.0:
+            got = torch.from_numpy(umi.umi_detrend_host(t, x, W, alpha=alpha, n_iter=n_iter, stars_per_batch=int(rng.choice([0, 1, 13]))))
+        else:
+            got = umi.umi_detrend(td, xd, W, alpha=alpha, n_iter=n_iter, c=c, **kw)
+        torch.cuda.synchronize()
+        g = got.cpu().numpy()
+        if n_iter == 0:
+            parity.compare_median(g, ref.median)
+        else:
+            worst = max(worst, parity.compare_trend(g, ref).max_rel)
+        if mode == 1:
+            want = orc.normalize(x, ref.trend64)
+            fl = flat.cpu().numpy().astype(np.float64)
+            assert np.array_equal(np.isnan(fl), np.isnan(want))
+            ok = ~np.isnan(want) & ~ref.near_cutoff.astype(bool)
+            assert (np.abs(fl[ok] - want[ok]) <= parity.TOL * np.abs(want[ok])).all()
+    assert worst <= parity.TOL
