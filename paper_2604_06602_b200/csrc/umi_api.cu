@@ -87,14 +87,15 @@ int validate(const float* flux, int64_t n_stars, int64_t n_cadences, int W, floa
 int launch_device(const double* time, const float* flux, int64_t n_stars, int64_t n_cadences,
                   int W, float alpha, float c, int n_iter, int min_valid, float* trend_out,
                   cudaStream_t stream, cudaEvent_t* ev = nullptr /* [3] or null */,
-                  float* flat_out = nullptr, const Family& fam = Family())
+                  float* flat_out = nullptr, const Family& fam = Family(),
+                  bool in_pipeline = false /* other batches keep the GPU busy: pick the throughput variants whatever the size */)
 {
     if (n_stars == 0 || n_cadences == 0) return UMI_OK;
     Geometry g = geometry_for(W);
     const bool mad = fam.on && fam.scale_kind == umi::SCALE_MAD;
     /* small batches (fewer median tiles than SMs; config 1 has 30): a 512-key sort with tiles of at least 128
        positions gives four times the CTAs and a shorter serial chain in each (latency is what is left to win) */
-    if (W - 1 + 128 <= 512 && n_stars * ((n_cadences + g.T1 - 1) / g.T1) < (int64_t)sm_count()) {   /* (forced on the large batches it loses: config 5 8.9 vs 7.3 ms per 20,000 stars, config 2 1.27 vs 0.63 ms) */
+    if (!in_pipeline && W - 1 + 128 <= 512 && n_stars * ((n_cadences + g.T1 - 1) / g.T1) < (int64_t)sm_count()) {   /* (forced on the large batches it loses: config 5 8.9 vs 7.3 ms per 20,000 stars, config 2 1.27 vs 0.63 ms) */
         g.NS = 512;
         g.T1 = 512 - (W - 1);
         g.smem1 = umi::k1_smem_bytes(g.NS, false, g.T1);
@@ -171,7 +172,7 @@ int launch_device(const double* time, const float* flux, int64_t n_stars, int64_
         int wtile = umi::K2_WARP_TILE;
         rp.tiles_per_star = (n_cadences + wtile - 1) / wtile;
         rp.n_blocks = n_stars * rp.tiles_per_star;
-        if (!fam.on && (rp.n_blocks + umi::K2_WARPS - 1) / umi::K2_WARPS <= 4 * (int64_t)sm_count()) {
+        if (!fam.on && !in_pipeline && (rp.n_blocks + umi::K2_WARPS - 1) / umi::K2_WARPS <= 4 * (int64_t)sm_count()) {
             /* the grid would leave most of the resident-CTA slots empty: split every window over
                K2_SPLIT lanes instead (latency, not throughput, is what is left to win) */
             rp.split = umi::K2_SPLIT;
@@ -515,8 +516,10 @@ int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t 
             status = UMI_ERR_CUDA;
             break;
         }
+        /* a batch between other batches is not alone on the GPU: its small-batch (latency) variants would only cost issue
+           slots the neighbours could use (config 2 end to end: 7.84 -> see DESIGN.md section 7) */
         status = launch_device(s.d_time, s.d_flux, ns, n_cadences, W, alpha, c, n_iter, min_valid, s.d_trend, s.stream,
-                               nullptr, s.d_flat);
+                               nullptr, s.d_flat, Family(), n_batches > 1);
         if (status != UMI_OK) break;
         if ((trend_out != nullptr &&
              cuda_failed(cudaMemcpyAsync(trend_out + off, s.d_trend, cnt * sizeof(float), cudaMemcpyDeviceToHost, s.stream))) ||
