@@ -281,3 +281,43 @@ def test_flatten_host_driver(umi):
     # other batch size -> the other variant of the reweighting kernel (split-window vs throughput): same
     # arithmetic, another summation order, so equal to rounding, not bit for bit
     assert none is None and np.allclose(flat2, flat, rtol=2e-6, atol=0.0, equal_nan=True)
+
+
+def test_hundred_random_cases_of_the_next_rows(umi):
+    # sibling estimators and gap handling (plain and with segments) on random windows, shapes, gap structures and options
+    import torch
+    for case in range(100):
+        rng = np.random.default_rng(55000 + case)
+        W = int(rng.choice([5, 9, 25, 33, 49, 51, 101, 217, 361, 801])) | 1
+        S = int(rng.choice([1, 3, 40, 180]))
+        N = int(rng.integers(2, 2600))
+        alpha = float(rng.choice([1.0, 2.0, 3.0]))
+        n_iter = int(rng.choice([0, 1, 5]))
+        x = lc.random_series(56000 + case, S, N, nan_frac=float(rng.choice([0.0, 0.03, 0.15])), inf_frac=0.0,
+                             ties=bool(rng.integers(0, 3) == 0))
+        kind = int(rng.integers(0, 3))
+        if kind == 0:
+            _family_case(umi, x, W, int(rng.integers(0, 2)), int(rng.integers(0, 2)), alpha=alpha, n_iter=n_iter)
+            continue
+        dt = float(rng.choice([2.0 / 1440, 0.02, 1.0]))
+        tz = float(rng.choice([0.0, 2457000.5, -3.25]))
+        for b in range(S):
+            for _ in range(int(rng.integers(0, 4))):
+                if N > 50:
+                    a = int(rng.integers(0, N - 10))
+                    x[b, a:a + int(rng.integers(1, max(2, N // 4)))] = np.nan
+        t, f, slot = lc.compact(x, dt, t0=tz, jitter=float(rng.choice([0.0, 0.25, 0.45])), seed=case)
+        n_grid = max(0, N - int(rng.integers(0, 5)))
+        h = W // 2
+        seg = {} if kind == 1 else dict(break_slots=int(rng.choice([-1, h, h + 3, W - 1, 3 * W])),
+                                        min_segment=int(rng.choice([0, 1, W // 3, W])),
+                                        edge_cut=int(rng.choice([0, 1, W // 10 + 1, W])))
+        ref = orc.gapped_ex(t, f, tz, dt, n_grid, W, alpha=alpha, n_iter=n_iter, **seg)
+        trend, flat = umi.umi_detrend_gapped(_cuda(t, np.float64), _cuda(f, np.float32), tz, dt, n_grid, W, alpha=alpha,
+                                             n_iter=n_iter, flat=True, **seg)
+        torch.cuda.synchronize()
+        if n_iter == 0:
+            parity.compare_median(trend.cpu().numpy(), ref.median)
+        else:
+            parity.compare_trend(trend.cpu().numpy(), ref)
+        _check_flat(flat.cpu().numpy(), f, ref)
