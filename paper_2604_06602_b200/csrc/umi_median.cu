@@ -116,13 +116,17 @@ __device__ __forceinline__ void bitonic_stage(uint32_t (&v)[E], uint32_t* buf, i
         const bool keep_min = (low == up);
         const uint32_t* other = buf + ((tid * E) ^ J);
         if constexpr (E % 4 == 0) {
+            /* 16-byte chunks, chunk c stored at c ^ ((c >> 3) & 7) within its group of 8: with E > 4 a thread's chunks
+               are E/4 apart, which would put a quarter-warp's 128-bit accesses on 2 (E = 16) or 4 (E = 8) bank groups */
+            auto chunk = [](int c) { return (c & ~7) | ((c ^ (c >> 3)) & 7); };
+            uint4* buf4 = reinterpret_cast<uint4*>(buf);
 #pragma unroll
             for (int e = 0; e < E; e += 4)
-                *reinterpret_cast<uint4*>(buf + tid * E + e) = make_uint4(v[e], v[e + 1], v[e + 2], v[e + 3]);
+                buf4[chunk((tid * E + e) >> 2)] = make_uint4(v[e], v[e + 1], v[e + 2], v[e + 3]);
             __syncthreads();
 #pragma unroll
             for (int e = 0; e < E; e += 4) {
-                const uint4 o4 = *reinterpret_cast<const uint4*>(other + e);
+                const uint4 o4 = buf4[chunk((((tid * E) ^ J) + e) >> 2)];
                 v[e] = keep_min ? min(v[e], o4.x) : max(v[e], o4.x);
                 v[e + 1] = keep_min ? min(v[e + 1], o4.y) : max(v[e + 1], o4.y);
                 v[e + 2] = keep_min ? min(v[e + 2], o4.z) : max(v[e + 2], o4.z);
