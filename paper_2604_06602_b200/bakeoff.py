@@ -37,6 +37,8 @@ def _lib():
     L.umi_bakeoff_median_radix.argtypes = [vp, i64, i64, ci, vp, vp]
     L.umi_bakeoff_median_warp_sorted.restype = ci
     L.umi_bakeoff_median_warp_sorted.argtypes = [vp, i64, i64, ci, ci, vp, vp]
+    L.umi_bakeoff_paper_design.restype = ci
+    L.umi_bakeoff_paper_design.argtypes = [vp, i64, i64, ci, cf, cf, ci, vp, vp]
     L.umi_bakeoff_reweight_warp_window.restype = ci
     L.umi_bakeoff_reweight_warp_window.argtypes = [vp, vp, i64, i64, ci, cf, cf, ci, vp, vp]
     return L
@@ -113,24 +115,34 @@ def run(out=None):
         rel = ((cand[fin] - trend[fin]).abs() / trend[fin].abs()).max().item()
         ok3 = bool(torch.equal(torch.isnan(cand), torch.isnan(trend)) and rel <= 2e-6)
         t3 = _timed(f3, flush)
-        rows.append((cid, S, N, W, prod_med, t1, ok1, t2[256], t2[1024], ok2, prod_rw, t3, ok3, rel))
+        # (0) the paper's design, whole path (W <= 385 only), against the product's whole step
+        t0 = ok0 = None
+        if W <= 385:
+            f0 = lambda: check(L.umi_bakeoff_paper_design(flux.data_ptr(), S, N, W, float(cfg.alpha), 5.0, int(cfg.n_iter), cand.data_ptr(), sptr))
+            f0()
+            torch.cuda.synchronize()
+            rel0 = ((cand[fin] - trend[fin]).abs() / trend[fin].abs()).max().item()
+            ok0 = bool(torch.equal(torch.isnan(cand), torch.isnan(trend)) and rel0 <= 1e-5)
+            t0 = _timed(f0, flush, steps=3, warmup=1)
+        rows.append((cid, S, N, W, prod_med, t1, ok1, t2[256], t2[1024], ok2, prod_rw, t3, ok3, rel, t0, ok0))
         del flux, med, trend, cand
     lines = ["| config (stars x cadences) | W | Phase 1: product (sort + walkers) | (i) radix select, warp per position | "
              "(ii) sorted window per warp, runs of 256 / 1024 | Phases 2-3: product (thread per 4 positions) | "
-             "(iii) warp per window + shuffles |",
-             "|---|---|---|---|---|---|---|"]
+             "(iii) warp per window + shuffles | whole path: product | (0) the paper's design, thread per position + quickselect in local memory |",
+             "|---|---|---|---|---|---|---|---|---|"]
     for r in rows:
-        cid, S, N, W, pm, t1, ok1, t2a, t2b, ok2, prw, t3, ok3, rel = r
+        cid, S, N, W, pm, t1, ok1, t2a, t2b, ok2, prw, t3, ok3, rel, t0, ok0 = r
+        paper = "n/a (W > 385)" if t0 is None else "%.1f ms (%.0fx), %s" % (t0, t0 / (pm + prw), "agrees" if ok0 else "MISMATCH")
         lines.append("| %d (%d x %d) | %d | %.3f ms | %.3f ms (%.1fx), %s | %.3f / %.3f ms (%.1fx), %s | %.3f ms | "
-                     "%.3f ms (%.2fx), %s (max rel diff %.1e) |"
+                     "%.3f ms (%.2fx), %s (max rel diff %.1e) | %.3f ms | %s |"
                      % (cid, S, N, W, pm, t1, t1 / pm, "bit-exact" if ok1 else "MISMATCH", t2a, t2b, min(t2a, t2b) / pm,
-                        "bit-exact" if ok2 else "MISMATCH", prw, t3, t3 / prw, "agrees" if ok3 else "MISMATCH", rel))
+                        "bit-exact" if ok2 else "MISMATCH", prw, t3, t3 / prw, "agrees" if ok3 else "MISMATCH", rel, pm + prw, paper))
     text = "\n".join(lines)
     print(text)
     if out:
         with open(out, "w") as f:
             f.write(text + "\n")
-    return all(r[6] and r[9] and r[12] for r in rows)
+    return all(r[6] and r[9] and r[12] and r[15] is not False for r in rows)
 
 
 if __name__ == "__main__":

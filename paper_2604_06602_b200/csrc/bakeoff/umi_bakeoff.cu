@@ -17,6 +17,11 @@
  *   (iii) umi_bakeoff_reweight_warp_window  a warp per window, its samples in registers (ceil(W/32) per
  *                                        lane), the sums of Eq. 1 and Eq. 4 by xor shuffles; same packed
  *                                        arithmetic as the product kernel (umi_device.cuh).
+ * And the prior art itself, for scale:
+ *   (0)  umi_bakeoff_paper_design        the paper's kernel design: one thread per (star, position)
+ *                                        copies its window into a private array (local memory), finds the median by
+ *                                        quickselect, then one upper-RMS pass and n_iter reweighting passes over the array;
+ *                                        written from that description, fp32, same readings (R1-R18).
  * Same validity rules as the product path (R2-R6, R16): NaN out where the own sample is invalid or the
  * window holds fewer than min_valid valid samples; lower middle for even counts.  No `time` argument.
  */
@@ -284,6 +289,68 @@ bk_reweight_warp_window(const float* __restrict__ flux, const float* __restrict_
     }
 }
 
+/* ------------------------------------------------------------------ (0) the paper's design: a thread per position */
+template <int WMAX>
+__global__ void __launch_bounds__(128)
+bk_paper_design(const float* __restrict__ flux, int64_t N, int64_t total, int W, int min_valid, float alpha, float c, int n_iter,
+                float* __restrict__ out)
+{
+    const int h = (W - 1) >> 1;
+    const float qnan = __int_as_float(0x7FC00000);
+    for (int64_t idx = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; idx < total; idx += (int64_t)gridDim.x * blockDim.x) {
+        const int64_t star = idx / N, p = idx - star * N;
+        const float* frow = flux + star * N;
+        float win[WMAX];                                            /* the thread's private copy of its window */
+        int n = 0;
+        for (int64_t j = p - h; j <= p + h; ++j) {
+            float x = 0.f;
+            if (load_sample(nullptr, frow, N, j, x)) win[n++] = x;
+        }
+        float own = 0.f;
+        const bool own_ok = load_sample(nullptr, frow, N, p, own);
+        if (!own_ok || n < min_valid || n == 0) { out[idx] = qnan; continue; }
+        /* quickselect (Hoare partition) for rank k = (n-1)/2 */
+        const int k = (n - 1) >> 1;
+        int lo = 0, hi = n - 1;
+        while (lo < hi) {
+            const float pivot = win[(lo + hi) >> 1];
+            int i = lo, j = hi;
+            while (i <= j) {
+                while (win[i] < pivot) ++i;
+                while (win[j] > pivot) --j;
+                if (i <= j) { const float t = win[i]; win[i] = win[j]; win[j] = t; ++i; --j; }
+            }
+            if (k <= j) hi = j; else if (k >= i) lo = i; else break;
+        }
+        const float med = win[k] + 0.f;
+        float ss = 0.f, cnt = 0.f;
+        for (int i = 0; i < n; ++i) {
+            const float d = win[i] - med;
+            if (d > 0.f) { ss = fmaf(d, d, ss); cnt += 1.f; }
+        }
+        float mu = med;
+        if (cnt > 0.f) {
+            const float s = SCALE_CONST * sqrtf(ss / cnt);
+            if (s > 0.f) {
+                const float cs = c * s, kk = 1.f / cs;
+                for (int it = 0; it < n_iter; ++it) {
+                    float S = 0.f, R = 0.f;
+                    for (int i = 0; i < n; ++i) {
+                        const float u = (win[i] - mu) * kk;
+                        const float e = u < 0.f ? -alpha * u : u;
+                        const float t = fmaxf(1.f - e * e, 0.f);
+                        const float w = t * t;
+                        S += w;
+                        R = fmaf(w, u, R);
+                    }
+                    if (S > 0.f) mu = fmaf(R / S, cs, mu);
+                }
+            }
+        }
+        out[idx] = mu;
+    }
+}
+
 int kpl_for(int W) { return (W + 31) / 32; }
 
 } // namespace
@@ -323,6 +390,21 @@ int umi_bakeoff_median_warp_sorted(const float* flux, int64_t n_stars, int64_t n
     else if (kpl <= 12) bk_median_warp_sorted<12><<<grid, 128, 0, s>>>(flux, n_cadences, rps, nr, run, W, mv, median_out);
     else if (kpl <= 34) bk_median_warp_sorted<34><<<grid, 128, 0, s>>>(flux, n_cadences, rps, nr, run, W, mv, median_out);
     else bk_median_warp_sorted<68><<<grid, 128, 0, s>>>(flux, n_cadences, rps, nr, run, W, mv, median_out);
+    return cudaGetLastError() == cudaSuccess ? 0 : 3;
+}
+
+/* (0): W <= 385 (a private window of 385 floats per thread) */
+int umi_bakeoff_paper_design(const float* flux, int64_t n_stars, int64_t n_cadences, int W, float alpha, float c, int n_iter,
+                             float* trend_out, void* stream)
+{
+    if (!flux || !trend_out || n_stars < 0 || n_cadences < 0 || W < 1 || !(W & 1) || W > 385 || n_iter < 0) return 1;
+    if (n_stars == 0 || n_cadences == 0) return 0;
+    const int64_t total = n_stars * n_cadences;
+    int64_t ctas = (total + 127) / 128;
+    if (ctas > 148 * 64) ctas = 148 * 64;
+    const int mv = W / 3 > 1 ? W / 3 : 1;
+    bk_paper_design<385><<<(unsigned)ctas, 128, 0, static_cast<cudaStream_t>(stream)>>>(flux, n_cadences, total, W, mv, alpha, c, n_iter,
+                                                                                   trend_out);
     return cudaGetLastError() == cudaSuccess ? 0 : 3;
 }
 

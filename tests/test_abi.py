@@ -133,7 +133,8 @@ def test_bakeoff_library_is_separate_and_exports_its_candidates():
     # the measured alternatives (csrc/bakeoff/) build into their own library and never into the product one
     from paper_2604_06602_b200 import build
     B = ctypes.CDLL(build.build_bakeoff())
-    for name in ("umi_bakeoff_median_radix", "umi_bakeoff_median_warp_sorted", "umi_bakeoff_reweight_warp_window"):
+    for name in ("umi_bakeoff_median_radix", "umi_bakeoff_median_warp_sorted", "umi_bakeoff_reweight_warp_window",
+                 "umi_bakeoff_paper_design"):
         assert hasattr(B, name)
     L = ctypes.CDLL(build.build())
     assert not hasattr(L, "umi_bakeoff_median_radix")
