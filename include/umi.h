@@ -20,9 +20,9 @@
  *    buffer is a caller-owned workspace (umi_detrend_gapped).  They are re-entrant and may
  *    be called concurrently from several host threads on different streams.  The HOST
  *    batch driver (umi_detrend_host, umi_flatten_host) has to own device buffers and
- *    streams; it takes them from a memory pool and a stream free list the library creates
- *    for itself per device (the device's default pool is never touched) and keeps them for
- *    the next call until umi_shutdown().  Nothing reads the process environment.
+ *    streams; it keeps them per device in a free list of slots (a stream and one buffer
+ *    that is only ever grown; plain cudaMalloc, no memory pool of the device or of its
+ *    own) for the next call, until umi_shutdown().  Nothing reads the process environment.
  *  - "DEVICE pointer": memory of the current CUDA device, readable/writable by
  *    kernels launched on `stream`.  "HOST pointer": ordinary host memory
  *    (pinned memory makes the copies asynchronous and faster, but is not
@@ -218,11 +218,11 @@ int umi_detrend_gapped_ex(const double* time, const float* flux,
  * device->host copy -- the only two no kernel hides -- are small), and
  * host->device copy, kernels and device->host copy of successive batches are
  * pipelined over `n_streams` CUDA streams (<= 0: 3, at most 16) with one device
- * buffer set per stream.  Buffers come from a memory pool the library creates for
- * itself on the current device (cudaMemPoolCreate, release threshold 1 GiB: what a
- * call frees is kept for the next one), streams from a free list; both are taken
- * when the call starts, given back when it returns, and destroyed by umi_shutdown().
- * Concurrent calls from several host threads are safe (each gets streams of its own).
+ * buffer per stream.  Stream and buffer form a slot; slots are kept per device in a
+ * free list between calls (the buffer is grown with cudaFree + cudaMalloc when a call
+ * needs more; creating streams and allocating per call cost 0.3-0.5 ms of an 8 ms job),
+ * taken when the call starts, given back when it returns, and freed by umi_shutdown().
+ * Concurrent calls from several host threads are safe (each gets slots of its own).
  *
  *   time, flux, trend_out   HOST pointers, same shapes as above; time may be NULL.
  * The call returns after every batch has been copied back (it synchronises).
@@ -274,8 +274,8 @@ int umi_detrend_profile(const double* time, const float* flux,
 int umi_launch_geometry(int W, int* median_tile, int* median_sort_n, int* weight_tile);
 
 /*
- * Releases what the HOST batch driver keeps between calls (its memory pools and idle
- * streams, on every device it was used on).  Call it when no umi_*_host call is running;
+ * Releases what the HOST batch driver keeps between calls (its idle slots: streams and
+ * device buffers, on every device it was used on).  Call it when no umi_*_host call is running;
  * the library can be used again afterwards.  Returns UMI_OK, or UMI_ERR_CUDA if a
  * destroy call failed.  The device entry points keep nothing, so programs that only use
  * those never need it.

@@ -355,16 +355,20 @@ int umi_detrend(const double* time, const float* flux, int64_t n_stars, int64_t 
 
 namespace {
 
-/* What the HOST batch driver keeps between calls, per device: a memory pool of its own for the per-stream
-   device buffers (cudaMemPoolCreate; the device's default pool and its attributes are never touched) and a
-   free list of CUDA streams (creating and destroying three streams per call cost ~0.3 ms of an 8.7 ms
-   config-2 job).  A call takes what it needs under the mutex and puts it back when it returns, so concurrent
-   callers never share a stream; umi_shutdown() destroys everything.  The DEVICE entry points use none of it. */
+/* What the HOST batch driver keeps between calls, per device: a free list of SLOTS, each a CUDA stream and one device
+   buffer that is only ever grown (creating and destroying three streams per call cost ~0.3 ms of an 8.7 ms config-2 job;
+   allocating the buffers per call another 0.1-0.2 ms).  A call takes the slots it needs under the mutex and puts them back
+   when it returns, so concurrent callers never share a stream or a buffer; umi_shutdown() frees everything.  No memory
+   pool, of the device or of the library, is involved.  The DEVICE entry points use none of this. */
 constexpr int MAX_DEVICES = 64;
+struct DriverSlot {
+    cudaStream_t stream = nullptr;
+    void* buf = nullptr;
+    size_t cap = 0;
+};
 struct HostDriverState {
     std::mutex lock;
-    cudaMemPool_t pool[MAX_DEVICES] = {};
-    std::vector<cudaStream_t> idle[MAX_DEVICES];
+    std::vector<DriverSlot> idle[MAX_DEVICES];
 };
 HostDriverState& driver_state()
 {
@@ -372,29 +376,8 @@ HostDriverState& driver_state()
     return *st;
 }
 
-/* the library's pool on device `dev` (created on first use; freed memory is kept up to 1 GiB for the next call) */
-cudaMemPool_t driver_pool(int dev)
-{
-    if (dev < 0 || dev >= MAX_DEVICES) return nullptr;
-    HostDriverState& st = driver_state();
-    std::lock_guard<std::mutex> guard(st.lock);
-    if (st.pool[dev] == nullptr) {
-        cudaMemPoolProps props = {};
-        props.allocType = cudaMemAllocationTypePinned;
-        props.handleTypes = cudaMemHandleTypeNone;
-        props.location.type = cudaMemLocationTypeDevice;
-        props.location.id = dev;
-        cudaMemPool_t pool = nullptr;
-        if (cuda_failed(cudaMemPoolCreate(&pool, &props))) return nullptr;
-        uint64_t thr = 1ull << 30;
-        (void)cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &thr);
-        (void)cudaGetLastError();
-        st.pool[dev] = pool;
-    }
-    return st.pool[dev];
-}
-
-bool take_streams(int dev, int n, std::vector<cudaStream_t>& out)
+/* n slots of the current device, each with a buffer of at least `bytes` (grown with cudaFree + cudaMalloc when it is not) */
+bool take_slots(int dev, int n, size_t bytes, std::vector<DriverSlot>& out)
 {
     out.clear();
     if (dev < 0 || dev >= MAX_DEVICES) return false;
@@ -407,20 +390,28 @@ bool take_streams(int dev, int n, std::vector<cudaStream_t>& out)
         }
     }
     while ((int)out.size() < n) {
-        cudaStream_t s = nullptr;
-        if (cuda_failed(cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking))) return false;
+        DriverSlot s;
+        if (cuda_failed(cudaStreamCreateWithFlags(&s.stream, cudaStreamNonBlocking))) return false;
         out.push_back(s);
+    }
+    for (auto& s : out) {
+        if (s.cap >= bytes) continue;
+        if (s.buf != nullptr) (void)cudaFree(s.buf);
+        s.buf = nullptr;
+        s.cap = 0;
+        if (cuda_failed(cudaMalloc(&s.buf, bytes))) return false;
+        s.cap = bytes;
     }
     return true;
 }
 
-void return_streams(int dev, std::vector<cudaStream_t>& streams)
+void return_slots(int dev, std::vector<DriverSlot>& slots)
 {
     if (dev < 0 || dev >= MAX_DEVICES) return;
     HostDriverState& st = driver_state();
     std::lock_guard<std::mutex> guard(st.lock);
-    for (cudaStream_t s : streams) st.idle[dev].push_back(s);
-    streams.clear();
+    for (const DriverSlot& s : slots) st.idle[dev].push_back(s);
+    slots.clear();
 }
 
 /* the batch driver behind umi_detrend_host / umi_flatten_host: trend_out and flat_out are HOST pointers,
@@ -482,25 +473,25 @@ int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t 
     const size_t elems = (size_t)stars_per_batch * (size_t)n_cadences;
     int status = UMI_OK;
 
+    /* one cached buffer per slot, carved into time | flux | trend | flat (each region a multiple of 256 bytes) */
+    auto region = [](size_t bytes) { return (bytes + 255) / 256 * 256; };
+    const size_t b_time = time != nullptr ? region(elems * sizeof(double)) : 0;
+    const size_t b_f32 = region(elems * sizeof(float));
+    const size_t b_slot = b_time + b_f32 * (flat_out != nullptr ? 3 : 2);
     int dev = 0;
     if (cuda_failed(cudaGetDevice(&dev))) return UMI_ERR_CUDA;
-    cudaMemPool_t pool = driver_pool(dev);
-    if (pool == nullptr) return UMI_ERR_CUDA;
-    std::vector<cudaStream_t> streams;
-    if (!take_streams(dev, n_streams, streams)) {
-        return_streams(dev, streams);
+    std::vector<DriverSlot> held;
+    if (!take_slots(dev, n_streams, b_slot, held)) {
+        return_slots(dev, held);
         return UMI_ERR_CUDA;
     }
-    for (size_t i = 0; i < slots.size(); ++i) slots[i].stream = streams[i];
-    for (auto& s : slots) {
-        if (/* stream-ordered allocations from the library's own pool: served from memory it kept after the first call */
-            cuda_failed(cudaMallocFromPoolAsync((void**)&s.d_flux, elems * sizeof(float), pool, s.stream)) ||
-            cuda_failed(cudaMallocFromPoolAsync((void**)&s.d_trend, elems * sizeof(float), pool, s.stream)) ||
-            (flat_out != nullptr && cuda_failed(cudaMallocFromPoolAsync((void**)&s.d_flat, elems * sizeof(float), pool, s.stream))) ||
-            (time != nullptr && cuda_failed(cudaMallocFromPoolAsync((void**)&s.d_time, elems * sizeof(double), pool, s.stream)))) {
-            status = UMI_ERR_CUDA;
-            break;
-        }
+    for (size_t i = 0; i < slots.size(); ++i) {
+        unsigned char* base = static_cast<unsigned char*>(held[i].buf);
+        slots[i].stream = held[i].stream;
+        slots[i].d_time = time != nullptr ? reinterpret_cast<double*>(base) : nullptr;
+        slots[i].d_flux = reinterpret_cast<float*>(base + b_time);
+        slots[i].d_trend = reinterpret_cast<float*>(base + b_time + b_f32);
+        slots[i].d_flat = flat_out != nullptr ? reinterpret_cast<float*>(base + b_time + 2 * b_f32) : nullptr;
     }
 
     int64_t s0 = 0;
@@ -528,16 +519,10 @@ int host_driver(const double* time, const float* flux, int64_t n_stars, int64_t 
             status = UMI_ERR_CUDA;
     }
 
-    for (auto& s : slots) {
-        if (s.stream == nullptr) continue;
-        if (s.d_flux) (void)cudaFreeAsync(s.d_flux, s.stream);
-        if (s.d_trend) (void)cudaFreeAsync(s.d_trend, s.stream);
-        if (s.d_flat) (void)cudaFreeAsync(s.d_flat, s.stream);
-        if (s.d_time) (void)cudaFreeAsync(s.d_time, s.stream);
-        if (cuda_failed(cudaStreamSynchronize(s.stream))) status = UMI_ERR_CUDA;
-    }
+    for (auto& s : slots)
+        if (s.stream != nullptr && cuda_failed(cudaStreamSynchronize(s.stream))) status = UMI_ERR_CUDA;
     (void)cudaGetLastError();
-    return_streams(dev, streams);
+    return_slots(dev, held);
     return status;
 }
 
@@ -550,15 +535,22 @@ int umi_shutdown(void)
     HostDriverState& st = driver_state();
     std::lock_guard<std::mutex> guard(st.lock);
     int status = UMI_OK;
+    bool any = false;
+    for (int dev = 0; dev < MAX_DEVICES; ++dev) any = any || !st.idle[dev].empty();
+    if (!any) return UMI_OK;                                /* nothing kept: no CUDA call at all */
+    int before = 0;
+    const bool have_dev = cudaGetDevice(&before) == cudaSuccess;
     for (int dev = 0; dev < MAX_DEVICES; ++dev) {
-        for (cudaStream_t s : st.idle[dev])
-            if (cuda_failed(cudaStreamDestroy(s))) status = UMI_ERR_CUDA;
-        st.idle[dev].clear();
-        if (st.pool[dev] != nullptr) {
-            if (cuda_failed(cudaMemPoolDestroy(st.pool[dev]))) status = UMI_ERR_CUDA;
-            st.pool[dev] = nullptr;
+        if (st.idle[dev].empty()) continue;
+        if (cuda_failed(cudaSetDevice(dev))) { status = UMI_ERR_CUDA; continue; }
+        for (const DriverSlot& s : st.idle[dev]) {
+            if (s.buf != nullptr && cuda_failed(cudaFree(s.buf))) status = UMI_ERR_CUDA;
+            if (s.stream != nullptr && cuda_failed(cudaStreamDestroy(s.stream))) status = UMI_ERR_CUDA;
         }
+        st.idle[dev].clear();
     }
+    if (have_dev) (void)cudaSetDevice(before);
+    (void)cudaGetLastError();
     return status;
 }
 
