@@ -68,3 +68,23 @@ def test_bench_roofline_bookkeeping():
     assert 50.0 < rec["fma_pipe_pct"] <= 100.0 and rec["local_ld"] == 0 and rec["local_st"] == 0
     assert bench.ncu_record(2, 999, "umi_reweight_kernel") is None      # no capture of that size: no number
     assert bench.ncu_record(3, 10000, "umi_small_kernel")["registers"] <= 80
+
+
+def test_bench_reference_arm_prints_the_contract_line():
+    # `bench.py --impl reference` (the oracle on host cores) must print ONE JSON line with the contract's keys
+    import json
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    res = subprocess.run([sys.executable, os.path.join(root, "bench.py"), "--impl", "reference", "--config", "1",
+                          "--steps", "1", "--warmup", "1"], capture_output=True, text=True, timeout=300, cwd=root)
+    assert res.returncode == 0, res.stderr[-500:]
+    lines = [ln for ln in res.stdout.splitlines() if ln.strip()]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["unit"] == "cadences/s" and d["higher_is_better"] is True
+    assert d["value"] > 0 and d["gpu_launches"] == 0 and d["dtype"] == "f64"
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["cpu_baseline"]["cores"] >= 1
+    assert d["e2e"] == {"value": d["value"], "unit": d["unit"], "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}
+    assert "workload" in d["config"] and "model" not in d["config"]
