@@ -4,7 +4,8 @@ snapshot.  Run `python -m paper_2604_06602_b200.build` or call build().
 
 Each .cu is compiled to an object of its own (in parallel, under _obj/) and the
 objects are linked into the shared library; an object is rebuilt when its source,
-any header or this file is newer.  `--bakeoff` builds libumi_bakeoff.so instead:
+any header or this file is newer.  `--define NAME=VALUE` compiles a measured, off-by-default
+alternative in (a plain build afterwards restores the default).  `--bakeoff` builds libumi_bakeoff.so instead:
 the selection / mapping candidates of csrc/bakeoff/ that were measured against the
 product kernels; they are never part of libumi_b200.so.
 """
@@ -95,11 +96,12 @@ def _build_lib(lib, sources, force, verbose, extra=()):
     return lib
 
 
-def build(force=False, verbose=False):
-    """Compile what is out of date and link libumi_b200.so.  Returns the library path."""
-    if not force and not verbose and not needs_build():
+def build(force=False, verbose=False, defines=()):
+    """Compile what is out of date and link libumi_b200.so.  Returns the library path.
+    defines: compile-time alternatives that were measured and are off by default (e.g. "UMI_K1_RADIX=1")."""
+    if not force and not verbose and not defines and not needs_build():
         return LIB
-    return _build_lib(LIB, SOURCES, force, verbose)
+    return _build_lib(LIB, SOURCES, force or bool(defines), verbose, extra=["-D" + d for d in defines])
 
 
 def build_bakeoff(force=False, verbose=False):
@@ -112,7 +114,8 @@ def build_bakeoff(force=False, verbose=False):
 
 if __name__ == "__main__":
     v = "-v" in sys.argv
+    defs = [sys.argv[i + 1] for i, a in enumerate(sys.argv[:-1]) if a == "--define"]
     if "--bakeoff" in sys.argv:
         print(build_bakeoff(force=True, verbose=v))
     else:
-        print(build(force=True, verbose=v))
+        print(build(force=True, verbose=v, defines=defs))

@@ -24,6 +24,13 @@
  */
 #include "umi_device.cuh"
 
+/* UMI_K1_RADIX = 1 (python -m paper_2604_06602_b200.build --define UMI_K1_RADIX=1) replaces the bitonic network + rank search by
+   least-significant-digit radix passes; measured and not the default: 0.82 against 0.63 ms on config 2, 9.13 against 7.25 ms on
+   20,000 config-5 stars */
+#ifndef UMI_K1_RADIX
+#define UMI_K1_RADIX 0
+#endif
+
 namespace umi {
 
 namespace {
@@ -200,6 +207,8 @@ umi_median_kernel(MedianParams prm)
     uint32_t* skey = reinterpret_cast<uint32_t*>(smem_raw + k1_smem_bytes(NS, false, prm.T)) - (NS + NS / 32);   /* [NS + NS/32] sorted keys, padded (skey_at) */
     float* sclbuf = reinterpret_cast<float*>(smem_raw + k1_smem_bytes(NS, false, prm.T));   /* MAD only: [T] scales */
     __shared__ int s_nvu;
+    __shared__ uint32_t s_kmin, s_kmax;                             /* radix path: range of the tile's valid keys */
+    __shared__ int s_wsum[K1_THREADS / 32];                         /* radix path: warp totals of the digit scan */
 
     const int W = prm.W;
     const int T = prm.T;
@@ -221,7 +230,7 @@ umi_median_kernel(MedianParams prm)
         const float* frow = prm.flux + star * prm.N;
         const double* trow = prm.time ? prm.time + star * prm.N : nullptr;
 
-        if (tid == 0) s_nvu = 0;
+        if (tid == 0) { s_nvu = 0; s_kmin = 0xFFFFFFFFu; s_kmax = 0u; }
         for (int i = tid; i < NW * BWP + NWB * BW; i += K1_THREADS) bits[i] = 0u;
         __syncthreads();
 
@@ -229,15 +238,121 @@ umi_median_kernel(MedianParams prm)
         uint32_t v[E];
         const bool vec = rows_vec && ((jbase + (int64_t)tid * E) & 3) == 0;
         int nvalid = load_keys<E>(trow, frow, prm.N, jbase + (int64_t)tid * E, vec, v);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) nvalid += __shfl_xor_sync(0xFFFFFFFFu, nvalid, o);
+        if (lane == 0 && nvalid) atomicAdd(&s_nvu, nvalid);
+#if UMI_K1_RADIX
+        /* Sort by LEAST-SIGNIFICANT-DIGIT RADIX passes on (key - smallest key of the tile): a tile's keys span a narrow
+           range (17-21 bits for flux of 1 +- a few per cent), so 2 or 3 passes of at most 9 bits do, where the bitonic
+           network needs 55 compare-exchange stages whatever the data.  The entries travel as key << 32 | union index, so
+           the last scatter writes srt[] and rank[] directly: no rank search, no tie counters.  One pass:
+             rank inside the warp   per round e, lanes with the same digit find each other with match.any; the lowest
+                                    of them bumps the warp's own histogram and hands the old count to the others
+             scan                   exclusive prefix over (digit, warp), digit-major: thread d owns digit d
+             scatter + reload       stable: warp w re-reads positions [32 E w, 32 E (w+1)), element (e, lane) at 32 e + lane
+           Invalid entries take no part: the first scatter compacts the valid ones to positions [0, nvu). */
+        {
+            const int warp = tid >> 5;
+            const unsigned lt = (1u << lane) - 1u;
+            uint32_t kmn = 0xFFFFFFFFu, kmx = 0u;
+            uint64_t el[E];
+            bool ok[E];
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                ok[e] = v[e] != KEY_INVALID;
+                el[e] = ((uint64_t)v[e] << 32) | (uint32_t)(tid * E + e);
+                if (ok[e]) { kmn = min(kmn, v[e]); kmx = max(kmx, v[e]); }
+                else rank[tid * E + e] = (uint16_t)0xFFFFu;
+            }
+            kmn = __reduce_min_sync(0xFFFFFFFFu, kmn);
+            kmx = __reduce_max_sync(0xFFFFFFFFu, kmx);
+            if (lane == 0 && kmn <= kmx) { atomicMin(&s_kmin, kmn); atomicMax(&s_kmax, kmx); }
+            __syncthreads();
+            const int nv = s_nvu;
+            const uint32_t kmin = s_kmin;
+            const int nbits = nv > 0 ? 32 - __clz((int)(s_kmax - kmin) | 1) : 1;
+            const int passes = (nbits + 8) / 9;
+            const int db = (nbits + passes - 1) / passes;           /* digit bits, <= 9 */
+            const int nb = 1 << db;
+            uint32_t* hist = bits;                                   /* [8 warps][nb] counters, in the bitset area */
+            uint32_t* hw = hist + warp * nb;
+            for (int pass = 0; pass < passes; ++pass) {
+                const int shift = pass * db;
+                for (int i = lane; i < nb; i += 32) hw[i] = 0u;
+                __syncwarp();
+                int off[E];
+                uint32_t dig[E];
+#pragma unroll
+                for (int e = 0; e < E; ++e) {
+                    const uint32_t d = ok[e] ? ((((uint32_t)(el[e] >> 32) - kmin) >> shift) & (uint32_t)(nb - 1)) : (uint32_t)nb;
+                    const unsigned peers = __match_any_sync(0xFFFFFFFFu, d);
+                    const int leader = __ffs((int)peers) - 1;
+                    uint32_t base = 0u;
+                    if (ok[e] && lane == leader) { base = hw[d]; hw[d] = base + (uint32_t)__popc(peers); }
+                    base = __shfl_sync(0xFFFFFFFFu, base, leader);
+                    off[e] = (int)base + __popc(peers & lt);
+                    dig[e] = d;
+                    __syncwarp();
+                }
+                __syncthreads();
+                /* exclusive prefix over (digit, warp): thread t owns the digits [t dpt, (t+1) dpt) */
+                {
+                    const int dpt = nb > K1_THREADS ? nb / K1_THREADS : 1;
+                    int mine = 0;
+                    for (int j = 0; j < dpt; ++j) {
+                        const int d = tid * dpt + j;
+                        if (d < nb)
+                            for (int w = 0; w < K1_THREADS / 32; ++w) mine += (int)hist[w * nb + d];
+                    }
+                    int incl = mine;
+#pragma unroll
+                    for (int o = 1; o < 32; o <<= 1) {
+                        const int t = __shfl_up_sync(0xFFFFFFFFu, incl, o);
+                        if (lane >= o) incl += t;
+                    }
+                    if (lane == 31) s_wsum[warp] = incl;
+                    __syncthreads();
+                    int run = incl - mine;
+                    for (int w = 0; w < warp; ++w) run += s_wsum[w];
+                    for (int j = 0; j < dpt; ++j) {
+                        const int d = tid * dpt + j;
+                        if (d < nb)
+                            for (int w = 0; w < K1_THREADS / 32; ++w) {
+                                const int c = (int)hist[w * nb + d];
+                                hist[w * nb + d] = (uint32_t)run;
+                                run += c;
+                            }
+                    }
+                }
+                __syncthreads();
+                const bool last = pass == passes - 1;
+#pragma unroll
+                for (int e = 0; e < E; ++e) {
+                    if (ok[e]) {
+                        const int pos = (int)hw[dig[e]] + off[e];
+                        srt[pos] = el[e];
+                        if (last) rank[(uint32_t)el[e]] = (uint16_t)pos;
+                    }
+                }
+                __syncthreads();
+                if (!last) {
+#pragma unroll
+                    for (int e = 0; e < E; ++e) {
+                        const int pp = warp * (32 * E) + 32 * e + lane;
+                        ok[e] = pp < nv;
+                        el[e] = ok[e] ? srt[pp] : 0ull;
+                    }
+                }
+            }
+            for (int i = tid; i < NW * BWP + NWB * BW; i += K1_THREADS) bits[i] = 0u;   /* the histograms lived in the bitset area */
+            __syncthreads();
+        }
+#else
         uint32_t own[E <= 8 ? E : 1];                               /* the entries' own keys, kept across the sort when they fit */
         if constexpr (E <= 8) {
 #pragma unroll
             for (int e = 0; e < E; ++e) own[e] = v[e];
         }
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) nvalid += __shfl_xor_sync(0xFFFFFFFFu, nvalid, o);
-        if (lane == 0 && nvalid) atomicAdd(&s_nvu, nvalid);
-
         bitonic_sort_blocked<E>(v, reinterpret_cast<uint32_t*>(srt), tid);
 
 #pragma unroll
@@ -272,6 +387,7 @@ umi_median_kernel(MedianParams prm)
         for (int e = 0; e < E; ++e)
             if (v[e] != 0xFFFFFFFFu) bits[v[e]] = 0u;                  /* the bitset area is all zero again */
         __syncthreads();
+#endif
         const int nvu = s_nvu;                                      /* valid entries = ranks [0, nvu) */
 
         /* 2. walker w owns positions [w*Ts, (w+1)*Ts).  Bitset of the ranks in its first window:
