@@ -296,72 +296,93 @@ def umi_detrend_profile(time, flux, W, alpha=2.0, n_iter=5, out=None, stream=Non
     return out.view(flux.shape), float(ms[0]), float(ms[1])
 
 
+_np = None
+_torch = None
+
+
+def _host_modules():
+    global _np, _torch
+    if _np is None:
+        import numpy
+        _np = numpy
+        try:
+            import torch
+            _torch = torch
+        except ImportError:  # pragma: no cover
+            _torch = False
+    return _np, (_torch or None)
+
+
+def _host_array(a, want, name):
+    """(address, shape, element count) of a C-contiguous host array: numpy array or CPU tensor of dtype `want`
+    ("float32" / "float64").  No copy, no conversion: anything else is a TypeError."""
+    np, torch = _host_modules()
+    if torch is not None and isinstance(a, torch.Tensor):
+        if a.is_cuda or a.dtype != getattr(torch, want) or not a.is_contiguous():
+            raise TypeError("%s must be a C-contiguous %s host array" % (name, want))
+        return a.data_ptr(), tuple(a.shape), a.numel()
+    if not isinstance(a, np.ndarray) or a.dtype != want or not a.flags.c_contiguous:
+        raise TypeError("%s must be a C-contiguous %s host array" % (name, want))
+    return a.ctypes.data, a.shape, a.size
+
+
+def _rows(shape):
+    if len(shape) == 1:
+        return 1, shape[0]
+    if len(shape) != 2:
+        raise ValueError("flux must be [n_stars, n_cadences]")
+    return shape
+
+
 def umi_detrend_host(time, flux, W, alpha=2.0, n_iter=5, out=None, stars_per_batch=0, n_streams=0):
     """Host path (batch driver).  `flux`: C-contiguous fp32 numpy array or CPU tensor
     [S, N]; `time`: None or fp64 of the same shape; pinned memory makes the copies
-    overlap.  Returns `out` (same kind as `flux`) after all batches are back."""
-    import numpy as np
-    try:
-        import torch
-    except ImportError:  # pragma: no cover
-        torch = None
-    is_torch = torch is not None and isinstance(flux, torch.Tensor)
-
-    def as_np(a, dtype, name):
-        if torch is not None and isinstance(a, torch.Tensor):
-            if a.is_cuda:
-                raise TypeError("%s must be a host array" % name)
-            a = a.numpy()
-        if not isinstance(a, np.ndarray) or a.dtype != dtype or not a.flags.c_contiguous:
-            raise TypeError("%s must be a C-contiguous %s host array" % (name, np.dtype(dtype).name))
-        return a
-
-    f = as_np(flux, np.float32, "flux")
-    f2 = f.reshape(1, -1) if f.ndim == 1 else f
-    if f2.ndim != 2:
-        raise ValueError("flux must be [n_stars, n_cadences]")
+    overlap.
+    Returns `out` (same kind as `flux`) after all batches are back."""
+    np, torch = _host_modules()
+    fptr, shape, size = _host_array(flux, "float32", "flux")
+    S, N = _rows(shape)
     tptr = None
     if time is not None:
-        t = as_np(time, np.float64, "time")
-        if t.size != f.size:
+        tptr, _, tsize = _host_array(time, "float64", "time")
+        if tsize != size:
             raise ValueError("time must have flux's shape")
-        tptr = t.ctypes.data
     if out is None:
-        out = torch.empty_like(flux) if is_torch else np.empty_like(f)
-    o = as_np(out, np.float32, "out")
-    if o.size != f.size:
+        out = torch.empty_like(flux) if (torch is not None and isinstance(flux, torch.Tensor)) else np.empty_like(flux)
+    optr, _, osize = _host_array(out, "float32", "out")
+    if osize != size:
         raise ValueError("out must have flux's shape")
-    S, N = f2.shape
     if S and N:
-        _check(lib().umi_detrend_host(tptr, f.ctypes.data, S, N, int(W), float(alpha), int(n_iter),
-                                      o.ctypes.data, int(stars_per_batch), int(n_streams)))
+        _check(lib().umi_detrend_host(tptr, fptr, S, N, int(W), float(alpha), int(n_iter),
+                                      optr, int(stars_per_batch), int(n_streams)))
     return out
 
 
 def umi_flatten_host(time, flux, W, alpha=2.0, n_iter=5, c=5.0, min_valid=-1, want_trend=True,
-                     stars_per_batch=0, n_streams=0):
-    """Host path with the normalisation fused in: returns (trend or None, flat) as numpy arrays of
-    flux's shape.  `flux`: C-contiguous fp32 numpy array or CPU tensor; pinned memory overlaps copies."""
-    import numpy as np
-    try:
-        import torch
-    except ImportError:  # pragma: no cover
-        torch = None
-    f = flux.numpy() if (torch is not None and isinstance(flux, torch.Tensor)) else flux
-    if not isinstance(f, np.ndarray) or f.dtype != np.float32 or not f.flags.c_contiguous:
-        raise TypeError("flux must be a C-contiguous float32 host array")
-    f2 = f.reshape(1, -1) if f.ndim == 1 else f
+                     stars_per_batch=0, n_streams=0, out_trend=None, out_flat=None):
+    """Host path with the normalisation fused in: returns (trend or None, flat), of flux's shape.
+    `flux`: C-contiguous fp32 numpy array or CPU tensor; `out_trend` / `out_flat`: optional
+    buffers of the same shape to fill (default: new numpy arrays); pinned memory overlaps copies."""
+    np, torch = _host_modules()
+    fptr, shape, size = _host_array(flux, "float32", "flux")
+    S, N = _rows(shape)
     tptr = None
     if time is not None:
-        t = time.numpy() if (torch is not None and isinstance(time, torch.Tensor)) else time
-        if not isinstance(t, np.ndarray) or t.dtype != np.float64 or not t.flags.c_contiguous or t.size != f.size:
+        tptr, _, tsize = _host_array(time, "float64", "time")
+        if tsize != size:
             raise TypeError("time must be a C-contiguous float64 host array of flux's shape")
-        tptr = t.ctypes.data
-    trend = np.empty_like(f) if want_trend else None
-    flat = np.empty_like(f)
-    S, N = f2.shape
+    trend = None
+    trptr = None
+    if want_trend:
+        trend = out_trend if out_trend is not None else np.empty(shape, dtype=np.float32)
+        trptr, _, n = _host_array(trend, "float32", "out_trend")
+        if n != size:
+            raise ValueError("out_trend must have flux's shape")
+    flat = out_flat if out_flat is not None else np.empty(shape, dtype=np.float32)
+    flptr, _, n = _host_array(flat, "float32", "out_flat")
+    if n != size:
+        raise ValueError("out_flat must have flux's shape")
     if S and N:
-        _check(lib().umi_flatten_host(tptr, f.ctypes.data, S, N, int(W), float(alpha), float(c), int(n_iter),
-                                      int(min_valid), trend.ctypes.data if want_trend else None, flat.ctypes.data,
-                                      int(stars_per_batch), int(n_streams)))
+        _check(lib().umi_flatten_host(tptr, fptr, S, N, int(W), float(alpha), float(c), int(n_iter),
+                                      int(min_valid), trptr, flptr, int(stars_per_batch), int(n_streams)))
     return trend, flat

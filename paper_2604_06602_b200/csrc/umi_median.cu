@@ -208,7 +208,9 @@ umi_median_kernel(MedianParams prm)
     float* sclbuf = reinterpret_cast<float*>(smem_raw + k1_smem_bytes(NS, false, prm.T));   /* MAD only: [T] scales */
     __shared__ int s_nvu;
     __shared__ uint32_t s_kmin, s_kmax;                             /* radix path: range of the tile's valid keys */
+#if UMI_K1_RADIX
     __shared__ int s_wsum[K1_THREADS / 32];                         /* radix path: warp totals of the digit scan */
+#endif
 
     const int W = prm.W;
     const int T = prm.T;

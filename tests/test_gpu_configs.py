@@ -151,3 +151,51 @@ def test_host_path_default_batches_ramp_up_and_down(umi, n_stars):
     th.start()
     th.join()
     parity.compare_trend(res["out"], ref)
+
+
+@pytest.mark.parametrize("W,n_iter", [(361, 5), (361, 0), (25, 5), (2161, 5)])
+def test_host_path_single_small_batch_pinned_and_pageable(umi, W, n_iter):
+    # the latency case (config 1's shape): one batch, caller-supplied pinned output (CPU tensors go through by address,
+    # no numpy round trip) and pageable numpy buffers.  Both must equal the device entry point bit for bit, and the
+    # oracle to tolerance.
+    import torch
+    flux = lc.stars(1, range(1)).copy()
+    flux[0, 4000:4700] = np.nan                             # a gap longer than the short windows
+    ref = orc.detrend(flux, W, n_iter=n_iter)
+    dev = umi.umi_detrend(None, torch.from_numpy(flux).cuda(), W, n_iter=n_iter).cpu().numpy()
+    pinned_in = torch.from_numpy(flux).pin_memory()
+    pinned_out = torch.full(flux.shape, 7.0, dtype=torch.float32).pin_memory()
+    got = umi.umi_detrend_host(None, pinned_in, W, n_iter=n_iter, out=pinned_out)
+    assert got is pinned_out
+    np.testing.assert_array_equal(got.numpy(), dev)
+    pageable = umi.umi_detrend_host(None, flux, W, n_iter=n_iter)
+    np.testing.assert_array_equal(pageable, dev)
+    if n_iter == 0:
+        parity.compare_median(got.numpy(), ref.median)
+    else:
+        parity.compare_trend(got.numpy(), ref)
+    # a view into the middle of a pinned allocation, and two stars forced into one batch
+    two = lc.stars(1, range(2))
+    big = torch.empty(3 * two.size, dtype=torch.float32).pin_memory()
+    out2 = big[two.size // 2: two.size // 2 + two.size].view(two.shape)
+    umi.umi_detrend_host(None, torch.from_numpy(two).pin_memory(), W, n_iter=n_iter, out=out2, stars_per_batch=2)
+    dev2 = umi.umi_detrend(None, torch.from_numpy(two).cuda(), W, n_iter=n_iter).cpu().numpy()
+    np.testing.assert_array_equal(out2.numpy(), dev2)
+
+
+@pytest.mark.parametrize("want_trend", [True, False])
+def test_flatten_host_caller_supplied_pinned_outputs(umi, want_trend):
+    import torch
+    flux = lc.stars(1, range(1))
+    W = 361
+    tr_dev, fl_dev = umi.umi_flatten(None, torch.from_numpy(flux).cuda(), W)
+    out_trend = torch.empty(flux.shape, dtype=torch.float32).pin_memory() if want_trend else None
+    out_flat = torch.empty(flux.shape, dtype=torch.float32).pin_memory()
+    tr, fl = umi.umi_flatten_host(None, torch.from_numpy(flux).pin_memory(), W, want_trend=want_trend,
+                                  out_trend=out_trend, out_flat=out_flat)
+    assert fl is out_flat and (tr is out_trend)
+    np.testing.assert_array_equal(fl.numpy(), fl_dev.cpu().numpy())
+    if want_trend:
+        np.testing.assert_array_equal(tr.numpy(), tr_dev.cpu().numpy())
+    ref = orc.detrend(flux, W)
+    parity.compare_trend((flux / fl.numpy()).astype(np.float32), ref, tol=2e-5)   # flat = flux / trend, rounded twice
