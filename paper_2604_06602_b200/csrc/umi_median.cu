@@ -5,11 +5,15 @@
  * live inside one union of U = T + W - 1 = NS samples (NS a power of two).
  *   1. sort the 32-bit keys of the union ONCE per tile: bitonic network, E = NS/256 keys per
  *      thread -- strides < E in registers, strides < 32 E with warp shuffles, only the top three
- *      strides through shared memory; a compare-exchange is two VIMNMX.  The rank of an entry is
- *      then the lower bound of its key in the sorted keys (binary search in shared memory) plus
- *      its turn among the entries with the same key (a shared-memory counter per key value);
- *      srt[rank] = key << 32 | index and rank[index] are scattered from that.  (Sorting 64-bit
- *      key|index entries directly cost 4-6 instructions per exchange and two shuffles.)
+ *      strides through shared memory; a compare-exchange is two VIMNMX.  What is sorted is
+ *      (key - smallest key of the tile) << log2 NS | union index whenever that fits 32 bits (the
+ *      keys of a tile normally span 2^17 .. 2^21 values): rank and index of every entry are then
+ *      read off the sorted words.  Otherwise (a wild sample, a deep eclipse in the tile) the bare
+ *      keys are sorted and the rank of an entry is the lower bound of its key in the sorted keys
+ *      (binary search in shared memory) plus its turn among the entries with the same key (a
+ *      shared-memory counter per key value).  Either way srt[rank] = key << 32 | index and
+ *      rank[index] come out.  (Sorting 64-bit key|index entries directly cost 4-6 instructions
+ *      per exchange and two shuffles.)
  *   2. NW "walkers" (one thread each) own T/NW consecutive positions.  A walker's
  *      first window is selected from a bitset of the union ranks it holds; the NW
  *      bitsets are built together as an exclusive-or prefix scan over the entries
@@ -233,7 +237,8 @@ umi_median_kernel(MedianParams prm)
         const double* trow = prm.time ? prm.time + star * prm.N : nullptr;
 
         if (tid == 0) { s_nvu = 0; s_kmin = 0xFFFFFFFFu; s_kmax = 0u; }
-        for (int i = tid; i < NW * BWP + NWB * BW; i += K1_THREADS) bits[i] = 0u;
+        static_assert((NW * BWP + NWB * BW) % 4 == 0, "the bitset area is zeroed 16 bytes at a time");
+        for (int i = tid; i < (NW * BWP + NWB * BW) / 4; i += K1_THREADS) reinterpret_cast<uint4*>(bits)[i] = make_uint4(0u, 0u, 0u, 0u);
         __syncthreads();
 
         /* 1. load E consecutive union entries and sort their 32-bit keys */
@@ -350,13 +355,55 @@ umi_median_kernel(MedianParams prm)
             __syncthreads();
         }
 #else
-        uint32_t own[E <= 8 ? E : 1];                               /* the entries' own keys, kept across the sort when they fit */
-        if constexpr (E <= 8) {
+        constexpr int OWN_MAX = 4;                                  /* (E = 8 spilled with them under its 48-register bound: it reloads, like E = 16 and 32) */
+        uint32_t own[E <= OWN_MAX ? E : 1];                               /* the entries' own keys, kept across the sort when they fit */
+        if constexpr (E <= OWN_MAX) {
 #pragma unroll
             for (int e = 0; e < E; ++e) own[e] = v[e];
         }
+        /* The keys of a tile normally span a narrow range (flux of 1 +- a few per cent: 2^17 .. 2^21 key values), so
+           (key - smallest key) and the entry's union index fit ONE 32-bit word: sorting those words sorts the entries,
+           and each thread reads rank and index of the entries it ends up holding straight off them -- no rank search,
+           no tie counters.  Ties come out in index order.  A tile whose keys span 2^(32 - log2 NS) - 1 values or more (a wild
+           sample, a deep eclipse) sorts the bare keys and searches, as before. */
+        constexpr int LOG_NS = 31 - __builtin_clz((unsigned)NS);
+        constexpr uint32_t KSPAN = (1u << (32 - LOG_NS)) - 1u;      /* also: the packed key of an invalid entry */
+        {
+            uint32_t kmn = 0xFFFFFFFFu, kmx = 0u;
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                kmn = min(kmn, v[e]);                               /* KEY_INVALID is the largest word */
+                kmx = max(kmx, v[e] != KEY_INVALID ? v[e] : 0u);
+            }
+            kmn = __reduce_min_sync(0xFFFFFFFFu, kmn);
+            kmx = __reduce_max_sync(0xFFFFFFFFu, kmx);
+            if (lane == 0 && nvalid) { atomicMin(&s_kmin, kmn); atomicMax(&s_kmax, kmx); }
+        }
+        __syncthreads();
+        const uint32_t kmin = s_kmin;
+        const bool pk = s_nvu > 0 && (s_kmax - kmin) < KSPAN;
+        if (pk) {
+#pragma unroll
+            for (int e = 0; e < E; ++e)
+                v[e] = ((v[e] != KEY_INVALID ? v[e] - kmin : KSPAN) << LOG_NS) | (uint32_t)(tid * E + e);
+        }
         bitonic_sort_blocked<E>(v, reinterpret_cast<uint32_t*>(srt), tid);
 
+        if (pk) {
+            __syncthreads();                                        /* every read of the exchange buffer (srt) is done */
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                const int r = tid * E + e;
+                const uint32_t u = v[e] & (uint32_t)(NS - 1), d = v[e] >> LOG_NS;
+                if (d != KSPAN) {
+                    rank[u] = (uint16_t)r;
+                    srt[r] = ((uint64_t)(kmin + d) << 32) | u;
+                } else {
+                    rank[u] = (uint16_t)0xFFFFu;
+                }
+            }
+            __syncthreads();
+        } else {
 #pragma unroll
         for (int e = 0; e < E; ++e) skey[skey_at(tid * E + e)] = v[e];
         __syncthreads();                                            /* also: every read of the exchange buffer is done */
@@ -365,11 +412,11 @@ umi_median_kernel(MedianParams prm)
            with that key (a counter per key value, borrowed from the still all-zero bitset area and zeroed
            again below).  Tied entries carry the same value, so which of them gets which rank changes
            nothing that is computed from ranks.  Invalid entries get a rank above every valid one. */
-        if constexpr (E > 8) (void)load_keys<E>(trow, frow, prm.N, jbase + (int64_t)tid * E, vec, v);   /* the same words again (L1 / L2) */
+        if constexpr (E > OWN_MAX) (void)load_keys<E>(trow, frow, prm.N, jbase + (int64_t)tid * E, vec, v);   /* the same words again (L1 / L2) */
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             const int u = tid * E + e;
-            const uint32_t key = (E <= 8) ? own[(E <= 8) ? e : 0] : v[e];
+            const uint32_t key = (E <= OWN_MAX) ? own[(E <= OWN_MAX) ? e : 0] : v[e];
             if (key != KEY_INVALID) {
                 int pos = 0;
 #pragma unroll
@@ -389,6 +436,7 @@ umi_median_kernel(MedianParams prm)
         for (int e = 0; e < E; ++e)
             if (v[e] != 0xFFFFFFFFu) bits[v[e]] = 0u;                  /* the bitset area is all zero again */
         __syncthreads();
+        }
 #endif
         const int nvu = s_nvu;                                      /* valid entries = ranks [0, nvu) */
 
@@ -398,7 +446,8 @@ umi_median_kernel(MedianParams prm)
         const int Ts = (Tact + NW - 1) / NW;
         const int nwa = (Tact + Ts - 1) / Ts;                       /* active walkers */
         const int span = (nwa - 1) * Ts;                            /* start of the last active walker */
-        const float inv_ts = 1.0f / (float)Ts;
+        const uint32_t ts_magic = 0xFFFFFFFFu / (uint32_t)Ts + 1u;   /* ceil(2^32 / Ts): u / Ts = umulhi(u, magic), exact while u Ts < 2^32 (Ts = 1: magic wraps to 0, handled) */
+        auto walker_of = [&](int u) { return Ts > 1 ? (int)__umulhi((uint32_t)u, ts_magic) : u; };
 #pragma unroll
         for (int e = 0; e < E; ++e) {
             const int u = tid * E + e;
@@ -408,16 +457,12 @@ umi_median_kernel(MedianParams prm)
                 const int wi = r >> 5;
                 if (u < W) atomicXor(&bits[wi], bit);
                 if (u < span) {
-                    int w = (int)((float)u * inv_ts);
-                    w += ((w + 1) * Ts <= u) ? 1 : 0;
-                    w -= (w * Ts > u) ? 1 : 0;
+                    const int w = walker_of(u);
                     atomicXor(&bits[(w + 1) * BWP + wi], bit);
                 }
                 const int ue = u - W;
                 if (ue >= 0 && ue < span) {
-                    int w = (int)((float)ue * inv_ts);
-                    w += ((w + 1) * Ts <= ue) ? 1 : 0;
-                    w -= (w * Ts > ue) ? 1 : 0;
+                    const int w = walker_of(ue);
                     atomicXor(&bits[(w + 1) * BWP + wi], bit);
                 }
             }

@@ -463,3 +463,27 @@ def test_two_hundred_random_cases(umi):
             ok = ~np.isnan(want) & ~ref.near_cutoff.astype(bool)
             assert (np.abs(fl[ok] - want[ok]) <= parity.TOL * np.abs(want[ok])).all()
     assert worst <= parity.TOL
+
+
+@pytest.mark.parametrize("W,log_ns", [(361, 10), (1081, 11), (2161, 12), (4097, 13)])
+def test_key_span_at_the_limit_of_the_packed_sort(umi, W, log_ns):
+    # The median kernel sorts (key - smallest key of the tile) << log2(NS) | union index in one 32-bit word when the
+    # tile's keys span fewer than 2^(32 - log2 NS) - 1 values, and bare keys + a rank search otherwise (umi_median.cu).
+    # Rows whose every tile spans exactly limit - 1 (widest packed), limit and limit + 1 (search), built on the bit
+    # patterns of the floats above 1.0; plus duplicates of the extremes and NaN, and a negative row (descending keys).
+    limit = (1 << (32 - log_ns)) - 1
+    rng = np.random.default_rng(1000 + W)
+    N = 6000
+    rows = []
+    for span in (limit - 2, limit - 1, limit, limit + 1):
+        k = rng.integers(0, span + 1, size=N, dtype=np.int64)
+        k[::97] = 0                                         # both extremes in every window, several times over
+        k[50::97] = span
+        bits = (np.float32(1.0).view(np.int32).astype(np.int64) + k).astype(np.int32)
+        x = bits.view(np.float32).copy()
+        x[rng.random(N) < 0.03] = np.nan
+        rows.append(x)
+        rows.append(-x)
+    x = np.stack(rows)
+    assert np.isfinite(x[~np.isnan(x)]).all()
+    _both(umi, x, W)
