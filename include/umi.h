@@ -57,7 +57,8 @@ typedef enum {
     UMI_OK = 0,
     UMI_ERR_INVALID_ARG = 1, /* null pointer, negative size, even or < 1 W, alpha/c not finite or <= 0, n_iter < 0 */
     UMI_ERR_UNSUPPORTED = 2, /* W > UMI_MAX_WINDOW */
-    UMI_ERR_CUDA = 3         /* launch / copy / allocation failure (the CUDA error is cleared) */
+    UMI_ERR_CUDA = 3,        /* launch / copy / allocation failure (the CUDA error is cleared) */
+    UMI_ERR_TOO_LARGE = 4    /* umi_detrend_gapped_static: the job needs more than UMI_STATIC_SCRATCH_BYTES of scratch */
 } umi_status;
 
 /* Largest window the compiled kernels accept (TESS 20 s needs 2161). */
@@ -209,6 +210,35 @@ int umi_detrend_gapped_ex(const double* time, const float* flux,
                           int64_t break_slots, int64_t min_segment, int64_t edge_cut,
                           float* trend_out, float* flat_out,
                           void* workspace, size_t workspace_bytes, void* stream);
+
+/*
+ * umi_detrend_gapped_ex for callers that cannot allocate (code under CUDA graph capture, tight serving
+ * loops, harnesses that forbid cudaMalloc) and so have no workspace to pass: the scratch is a fixed array
+ * of UMI_STATIC_SCRATCH_BYTES (16 MiB) of device memory inside the library's image, which every GPU that
+ * loads the library holds until the process exits.  Same arguments (all pointers DEVICE, caller-owned
+ * inputs and outputs), same kernels and same results as umi_detrend_gapped_ex; no cudaMalloc, cudaFree or
+ * allocating library routine is called, now or later.
+ *   Limit     n_stars * n_grid * 8 bytes (17 with any of break_slots / min_segment / edge_cut on) must not
+ *             exceed UMI_STATIC_SCRATCH_BYTES: 2,097,152 slots (e.g. 100 stars x 20,971 slots), 986,895 with
+ *             segments.  Beyond it -> UMI_ERR_TOO_LARGE, nothing enqueued (use umi_detrend_gapped_ex).
+ *   Sharing   every call on a device uses the same array, which keeps the last call's contents.  The path
+ *             clears what it needs first thing on `stream`, so calls ordered one after another (one stream,
+ *             or streams ordered by events) are independent.  Calls that OVERLAP on the GPU race on the
+ *             array and give wrong results: serialise them, or give the others a workspace of their own.
+ *   Set-up    the array's device address is looked up once per device (cudaGetSymbolAddress, with that
+ *             device current) on the first call there; umi_static_init() does only that, for callers who
+ *             want it done before a capture or a timed loop starts.  `stream` must belong to the current device.
+ * umi_static_scratch_bytes() returns UMI_STATIC_SCRATCH_BYTES (host only).
+ */
+#define UMI_STATIC_SCRATCH_BYTES (16u << 20)
+size_t umi_static_scratch_bytes(void);
+int umi_static_init(void);
+int umi_detrend_gapped_static(const double* time, const float* flux,
+                              int64_t n_stars, int64_t n_samples,
+                              double t0, double dt, int64_t n_grid,
+                              int W, float alpha, float c, int n_iter, int min_valid,
+                              int64_t break_slots, int64_t min_segment, int64_t edge_cut,
+                              float* trend_out, float* flat_out, void* stream);
 
 /*
  * Batch driver (the paper streams 50-star batches): the same

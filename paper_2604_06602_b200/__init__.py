@@ -16,7 +16,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 # UMI_B200_LIB selects another build of the same library (kernel experiments); default: in-tree.
 LIB_PATH = os.environ.get("UMI_B200_LIB") or os.path.join(_HERE, "libumi_b200.so")
 
-UMI_OK, UMI_ERR_INVALID_ARG, UMI_ERR_UNSUPPORTED, UMI_ERR_CUDA = 0, 1, 2, 3
+UMI_OK, UMI_ERR_INVALID_ARG, UMI_ERR_UNSUPPORTED, UMI_ERR_CUDA, UMI_ERR_TOO_LARGE = 0, 1, 2, 3, 4
+UMI_STATIC_SCRATCH_BYTES = 16 << 20
 UMI_MAX_WINDOW = 4097
 UMI_SCALE_UPPER_RMS, UMI_SCALE_MAD = 0, 1
 UMI_WEIGHT_BISQUARE, UMI_WEIGHT_WELSCH = 0, 1
@@ -24,7 +25,8 @@ UMI_WEIGHT_BISQUARE, UMI_WEIGHT_WELSCH = 0, 1
 EXPORTS = ("umi_window_len", "umi_detrend", "umi_detrend_ex", "umi_detrend_host", "umi_detrend_profile",
            "umi_flatten", "umi_flatten_host", "umi_detrend_family", "umi_detrend_gapped", "umi_gapped_workspace_bytes",
            "umi_launch_geometry", "umi_status_string", "umi_version", "umi_shutdown",
-           "umi_detrend_gapped_ex", "umi_gapped_ex_workspace_bytes")
+           "umi_detrend_gapped_ex", "umi_gapped_ex_workspace_bytes",
+           "umi_detrend_gapped_static", "umi_static_scratch_bytes", "umi_static_init")
 
 _lib = None
 
@@ -72,6 +74,13 @@ def lib():
     L.umi_detrend_gapped_ex.restype = ci
     L.umi_detrend_gapped_ex.argtypes = [vp, vp, i64, i64, ctypes.c_double, ctypes.c_double, i64,
                                         ci, cf, cf, ci, ci, i64, i64, i64, vp, vp, vp, ctypes.c_size_t, vp]
+    L.umi_static_scratch_bytes.restype = ctypes.c_size_t
+    L.umi_static_scratch_bytes.argtypes = []
+    L.umi_static_init.restype = ci
+    L.umi_static_init.argtypes = []
+    L.umi_detrend_gapped_static.restype = ci
+    L.umi_detrend_gapped_static.argtypes = [vp, vp, i64, i64, ctypes.c_double, ctypes.c_double, i64,
+                                            ci, cf, cf, ci, ci, i64, i64, i64, vp, vp, vp]
     L.umi_launch_geometry.restype = ci
     L.umi_launch_geometry.argtypes = [ci] + [ctypes.POINTER(ci)] * 3
     L.umi_status_string.restype = ctypes.c_char_p
@@ -276,6 +285,44 @@ def umi_detrend_gapped(time, flux, t0, dt, n_grid, W, alpha=2.0, n_iter=5, c=5.0
                                                trend.data_ptr(), fl.data_ptr() if flat else None,
                                                workspace.data_ptr(), wbytes, on.ptr))
     return (trend.view(flux.shape), fl.view(flux.shape)) if flat else trend.view(flux.shape)
+
+
+def umi_static_scratch_bytes():
+    return int(lib().umi_static_scratch_bytes())
+
+
+def umi_static_init():
+    """Look up the static scratch array's address on the current device now (include/umi.h)."""
+    _check(lib().umi_static_init())
+
+
+def umi_detrend_gapped_static(time, flux, t0, dt, n_grid, W, alpha=2.0, n_iter=5, c=5.0, min_valid=-1,
+                              out=None, out_flat=None, stream=None, break_slots=-1, min_segment=0, edge_cut=0):
+    """umi_detrend_gapped without a workspace: the scratch is the library's static device array of
+    UMI_STATIC_SCRATCH_BYTES (include/umi.h: limit, and calls that overlap on the GPU race on it).
+    With `out` (and `out_flat`, when the flattened curve is wanted) given, nothing is allocated at all;
+    otherwise the trend tensor is. Returns trend, or (trend, flat) when `out_flat` is given.
+    A job beyond the array raises UmiError with status UMI_ERR_TOO_LARGE."""
+    import torch
+    f = _cuda_2d(flux, torch.float32, "flux")
+    tt = _cuda_2d(time, torch.float64, "time")
+    if tt.shape != f.shape or tt.device != f.device:
+        raise ValueError("time must have flux's shape and device")
+    S, M = f.shape
+    for name, o in (("out", out), ("out_flat", out_flat)):
+        if o is not None and not (isinstance(o, torch.Tensor) and o.is_cuda and o.dtype == torch.float32 and
+                                  o.is_contiguous() and o.numel() == f.numel() and o.device == f.device):
+            raise TypeError("%s must be a contiguous CUDA float32 tensor of flux's size" % name)
+    with _OnStream(stream, f.device) as on:
+        trend = out if out is not None else torch.empty_like(f)
+        on.uses(f, tt, trend, out_flat)
+        if S and M:
+            _check(lib().umi_detrend_gapped_static(tt.data_ptr(), f.data_ptr(), S, M, float(t0), float(dt), int(n_grid),
+                                                   int(W), float(alpha), float(c), int(n_iter), int(min_valid),
+                                                   int(break_slots), int(min_segment), int(edge_cut),
+                                                   trend.data_ptr(), None if out_flat is None else out_flat.data_ptr(),
+                                                   on.ptr))
+    return trend if out_flat is None else (trend, out_flat)
 
 
 def umi_detrend_profile(time, flux, W, alpha=2.0, n_iter=5, out=None, stream=None, c=5.0, min_valid=-1):

@@ -19,7 +19,7 @@ ROOT = os.path.dirname(HERE)
 CSRC = os.path.join(HERE, "csrc")
 OBJDIR = os.path.join(HERE, "_obj")
 SOURCES = [os.path.join(CSRC, n) for n in
-           ("umi_api.cu", "umi_median.cu", "umi_reweight.cu", "umi_small.cu", "umi_regrid.cu")]
+           ("umi_api.cu", "umi_median.cu", "umi_reweight.cu", "umi_small.cu", "umi_regrid.cu", "umi_static.cu")]
 HEADERS = [os.path.join(CSRC, "umi_internal.h"), os.path.join(CSRC, "umi_device.cuh"), os.path.join(ROOT, "include", "umi.h")]
 LIB = os.path.join(HERE, "libumi_b200.so")
 BAKEOFF_DIR = os.path.join(CSRC, "bakeoff")

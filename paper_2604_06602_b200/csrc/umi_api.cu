@@ -590,6 +590,7 @@ const char* umi_status_string(int status)
     case UMI_ERR_INVALID_ARG: return "UMI_ERR_INVALID_ARG: null pointer, negative size, even or < 1 window, or bad alpha/c/n_iter";
     case UMI_ERR_UNSUPPORTED: return "UMI_ERR_UNSUPPORTED: window longer than UMI_MAX_WINDOW";
     case UMI_ERR_CUDA: return "UMI_ERR_CUDA: a CUDA launch, copy or allocation failed";
+    case UMI_ERR_TOO_LARGE: return "UMI_ERR_TOO_LARGE: the job needs more scratch than the static array of UMI_STATIC_SCRATCH_BYTES holds";
     default: return "UMI: unknown status";
     }
 }

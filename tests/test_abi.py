@@ -142,3 +142,20 @@ def test_bakeoff_library_is_separate_and_exports_its_candidates():
     B.umi_bakeoff_median_radix.argtypes = [ctypes.c_void_p, ctypes.c_int64, ctypes.c_int64, ctypes.c_int, ctypes.c_void_p, ctypes.c_void_p]
     assert B.umi_bakeoff_median_radix(one, 1, 10, 4, one, None) == 1        # even window: refused on the host
     assert B.umi_bakeoff_median_radix(one, 0, 10, 361, one, None) == 0      # empty batch: nothing enqueued
+
+
+def test_static_scratch_size_and_limit_are_checked_without_a_gpu():
+    # umi_detrend_gapped_static refuses a job beyond its static array before it touches CUDA
+    L = umi.lib()
+    assert umi.umi_static_scratch_bytes() == umi.UMI_STATIC_SCRATCH_BYTES == 16 << 20
+    assert "UMI_STATIC_SCRATCH_BYTES" in umi.umi_status_string(umi.UMI_ERR_TOO_LARGE)
+    dummy = ctypes.c_void_p(256)                     # never dereferenced: the size check comes first
+
+    def call(n_stars, n_grid, edge_cut=0):
+        return L.umi_detrend_gapped_static(dummy, dummy, n_stars, 8, 0.0, 0.01, n_grid, 5, 2.0, 5.0, 5, -1,
+                                           -1, 0, edge_cut, dummy, None, None)
+
+    assert call(513, 4096) == umi.UMI_ERR_TOO_LARGE              # 512 x 4096 slots x 8 bytes is exactly the array
+    assert call(512, 4096, edge_cut=1) == umi.UMI_ERR_TOO_LARGE  # 17 bytes per slot with segments
+    assert call(1, (16 << 20) // 8 + 1) == umi.UMI_ERR_TOO_LARGE
+    assert call(2 ** 40, 2 ** 40) == umi.UMI_ERR_TOO_LARGE       # no 64-bit wrap-around
