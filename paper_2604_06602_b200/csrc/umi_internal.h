@@ -12,16 +12,18 @@ namespace umi {
 #ifndef UMI_K1_THREADS
 #define UMI_K1_THREADS 256
 #endif
-constexpr int K1_THREADS = UMI_K1_THREADS;       /* median kernel */
+constexpr int K1_THREADS = UMI_K1_THREADS;       /* median kernel (128 for the 1024-key sort: launch_median) */
 #ifndef UMI_K1_MIN_SORT
 #define UMI_K1_MIN_SORT 1024
 #endif
 constexpr int K1_MIN_SORT = UMI_K1_MIN_SORT;     /* smallest per-tile sort length */
-/* walkers per tile of the median kernel and its dynamic shared memory (bytes) */
-#ifndef UMI_K1_WALKER_BUDGET
-#define UMI_K1_WALKER_BUDGET 131072
+/* walkers per tile of the median kernel, per sort length, and its dynamic shared memory (bytes).  Measured:
+   512 keys (small batches): one walker per position pair; 1024: every one of the CTA's 128 threads; beyond that as many as
+   leave the CTAs per SM of k1_min_ctas (umi_median.cu) their shared memory -- a multiple of 32, not necessarily a power of two */
+#ifndef UMI_K1_WALKERS
+#define UMI_K1_WALKERS(ns) ((ns) <= 512 ? 256 : (ns) == 1024 ? 128 : (ns) == 2048 ? 96 : (ns) == 4096 ? 96 : 64)
 #endif
-__host__ __device__ constexpr int k1_walkers(int ns) { return (UMI_K1_WALKER_BUDGET / ns) > 32 ? ((UMI_K1_WALKER_BUDGET / ns) < K1_THREADS ? (UMI_K1_WALKER_BUDGET / ns) : K1_THREADS) : 32; }
+__host__ __device__ constexpr int k1_walkers(int ns) { return UMI_K1_WALKERS(ns); }
 /* t = positions per tile (T = ns - W + 1; 0: the worst case ns) */
 __host__ __device__ constexpr size_t k1_smem_bytes(int ns, bool mad = false, int t = 0)
 {

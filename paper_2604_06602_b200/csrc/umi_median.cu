@@ -162,13 +162,13 @@ __device__ __forceinline__ void bitonic_merge(uint32_t (&v)[E], uint32_t* buf, i
     }
 }
 
-/* Bitonic sort of NS = 256*E keys, ascending. */
-template <int E, int K = 2>
+/* Bitonic sort of NS = THREADS*E keys, ascending. */
+template <int E, int THREADS, int K = 2>
 __device__ __forceinline__ void bitonic_sort_blocked(uint32_t (&v)[E], uint32_t* buf, int tid)
 {
-    if constexpr (K <= K1_THREADS * E) {
+    if constexpr (K <= THREADS * E) {
         bitonic_merge<E, K, K / 2>(v, buf, tid);
-        bitonic_sort_blocked<E, K * 2>(v, buf, tid);
+        bitonic_sort_blocked<E, THREADS, K * 2>(v, buf, tid);
     }
 }
 
@@ -185,11 +185,14 @@ struct MadRange {
     int L, R, cnt;
 };
 
-template <int E, bool MAD>
-__global__ void __launch_bounds__(K1_THREADS, E <= 4 ? 6 : E == 8 ? 5 : E == 16 ? 3 : 1)   /* as many CTAs per SM as their shared memory allows (NS = 1024: 6, 2048: 5, 4096: 3, 8192: 1) */
+/* CTAs per SM the registers must allow, per sort length: what the shared memory of that length admits (k1_smem_bytes) */
+__host__ __device__ constexpr int k1_min_ctas(int ns) { return ns <= 512 ? 6 : ns == 1024 ? 7 : ns == 2048 ? 4 : ns == 4096 ? 2 : 1; }
+
+template <int E, int THREADS, bool MAD>
+__global__ void __launch_bounds__(THREADS, k1_min_ctas(THREADS * E))
 umi_median_kernel(MedianParams prm)
 {
-    constexpr int NS = K1_THREADS * E;
+    constexpr int NS = THREADS * E;
     constexpr int BW = NS / 32;                                     /* bitset words per walker */
     constexpr int BWP = BW + 1;                                     /* padded row stride: conflict-free both ways */
 #ifndef UMI_K1_MAD_WALKERS
@@ -213,7 +216,7 @@ umi_median_kernel(MedianParams prm)
     __shared__ int s_nvu;
     __shared__ uint32_t s_kmin, s_kmax;                             /* radix path: range of the tile's valid keys */
 #if UMI_K1_RADIX
-    __shared__ int s_wsum[K1_THREADS / 32];                         /* radix path: warp totals of the digit scan */
+    __shared__ int s_wsum[THREADS / 32];                         /* radix path: warp totals of the digit scan */
 #endif
 
     const int W = prm.W;
@@ -238,7 +241,7 @@ umi_median_kernel(MedianParams prm)
 
         if (tid == 0) { s_nvu = 0; s_kmin = 0xFFFFFFFFu; s_kmax = 0u; }
         static_assert((NW * BWP + NWB * BW) % 4 == 0, "the bitset area is zeroed 16 bytes at a time");
-        for (int i = tid; i < (NW * BWP + NWB * BW) / 4; i += K1_THREADS) reinterpret_cast<uint4*>(bits)[i] = make_uint4(0u, 0u, 0u, 0u);
+        for (int i = tid; i < (NW * BWP + NWB * BW) / 4; i += THREADS) reinterpret_cast<uint4*>(bits)[i] = make_uint4(0u, 0u, 0u, 0u);
         __syncthreads();
 
         /* 1. load E consecutive union entries and sort their 32-bit keys */
@@ -304,12 +307,12 @@ umi_median_kernel(MedianParams prm)
                 __syncthreads();
                 /* exclusive prefix over (digit, warp): thread t owns the digits [t dpt, (t+1) dpt) */
                 {
-                    const int dpt = nb > K1_THREADS ? nb / K1_THREADS : 1;
+                    const int dpt = nb > THREADS ? nb / THREADS : 1;
                     int mine = 0;
                     for (int j = 0; j < dpt; ++j) {
                         const int d = tid * dpt + j;
                         if (d < nb)
-                            for (int w = 0; w < K1_THREADS / 32; ++w) mine += (int)hist[w * nb + d];
+                            for (int w = 0; w < THREADS / 32; ++w) mine += (int)hist[w * nb + d];
                     }
                     int incl = mine;
 #pragma unroll
@@ -324,7 +327,7 @@ umi_median_kernel(MedianParams prm)
                     for (int j = 0; j < dpt; ++j) {
                         const int d = tid * dpt + j;
                         if (d < nb)
-                            for (int w = 0; w < K1_THREADS / 32; ++w) {
+                            for (int w = 0; w < THREADS / 32; ++w) {
                                 const int c = (int)hist[w * nb + d];
                                 hist[w * nb + d] = (uint32_t)run;
                                 run += c;
@@ -351,7 +354,7 @@ umi_median_kernel(MedianParams prm)
                     }
                 }
             }
-            for (int i = tid; i < NW * BWP + NWB * BW; i += K1_THREADS) bits[i] = 0u;   /* the histograms lived in the bitset area */
+            for (int i = tid; i < NW * BWP + NWB * BW; i += THREADS) bits[i] = 0u;   /* the histograms lived in the bitset area */
             __syncthreads();
         }
 #else
@@ -387,7 +390,7 @@ umi_median_kernel(MedianParams prm)
             for (int e = 0; e < E; ++e)
                 v[e] = ((v[e] != KEY_INVALID ? v[e] - kmin : KSPAN) << LOG_NS) | (uint32_t)(tid * E + e);
         }
-        bitonic_sort_blocked<E>(v, reinterpret_cast<uint32_t*>(srt), tid);
+        bitonic_sort_blocked<E, THREADS>(v, reinterpret_cast<uint32_t*>(srt), tid);
 
         if (pk) {
             __syncthreads();                                        /* every read of the exchange buffer (srt) is done */
@@ -469,7 +472,7 @@ umi_median_kernel(MedianParams prm)
         }
         __syncthreads();
         /* scan over walkers, one (block of 32 walkers, word column) pair per work item */
-        for (int item = tid; item < NWB * BW; item += K1_THREADS) {
+        for (int item = tid; item < NWB * BW; item += THREADS) {
             const int col = item % BW, blk = item / BW;
             uint32_t acc = 0u;
             uint32_t* pcol = bits + (blk * 32) * BWP + col;
@@ -482,7 +485,7 @@ umi_median_kernel(MedianParams prm)
         }
         __syncthreads();
         if (NWB > 1) {
-            for (int col = tid; col < BW; col += K1_THREADS) {
+            for (int col = tid; col < BW; col += THREADS) {
                 uint32_t acc = 0u;
                 for (int blk = 0; blk < NWB; ++blk) {
                     const uint32_t t = boff[blk * BW + col];
@@ -491,7 +494,7 @@ umi_median_kernel(MedianParams prm)
                 }
             }
         } else {
-            for (int col = tid; col < BW; col += K1_THREADS) boff[col] = 0u;
+            for (int col = tid; col < BW; col += THREADS) boff[col] = 0u;
         }
         __syncthreads();
 
@@ -673,7 +676,7 @@ umi_median_kernel(MedianParams prm)
                Eq. 1 (R7) = the n - 1 - (n-1)/2 members above the median in rank, less those that tie with it
                in value (they follow it directly in sorted order). */
             uint32_t* wrow = reinterpret_cast<uint32_t*>(orow);
-            for (int p = tid; p < Tact; p += K1_THREADS) {
+            for (int p = tid; p < Tact; p += THREADS) {
                 const int rho = rhobuf[p];
                 uint32_t word = HANDOVER_NONE;
                 if (rho != 0xFFFF) {
@@ -688,15 +691,15 @@ umi_median_kernel(MedianParams prm)
                 wrow[p] = word;
             }
         } else {
-            for (int p = tid; p < Tact; p += K1_THREADS) orow[p] = medbuf[p];
+            for (int p = tid; p < Tact; p += THREADS) orow[p] = medbuf[p];
         }
         if constexpr (MAD) {
             float* srow = prm.scale + star * prm.N + j0;
-            for (int p = tid; p < Tact; p += K1_THREADS) srow[p] = sclbuf[p];
+            for (int p = tid; p < Tact; p += THREADS) srow[p] = sclbuf[p];
         }
         if (prm.flat != nullptr) {                                  /* PAPER.md:155 normalisation, n_iter = 0 */
             float* flrow = prm.flat + star * prm.N + j0;
-            for (int p = tid; p < Tact; p += K1_THREADS) {
+            for (int p = tid; p < Tact; p += THREADS) {
                 const float m = medbuf[p];
                 flrow[p] = (m == m) ? __ldg(frow + j0 + p) / m : m;
             }
@@ -709,19 +712,23 @@ cudaError_t launch_median(const MedianParams& prm, unsigned grid, size_t smem, c
 {
     void (*k1)(MedianParams) = nullptr;
     const bool mad = prm.scale != nullptr;
-    switch (prm.NS / K1_THREADS) {
-    case 2: k1 = mad ? umi_median_kernel<2, true> : umi_median_kernel<2, false>; break;
-    case 4: k1 = mad ? umi_median_kernel<4, true> : umi_median_kernel<4, false>; break;
-    case 8: k1 = mad ? umi_median_kernel<8, true> : umi_median_kernel<8, false>; break;
-    case 16: k1 = mad ? umi_median_kernel<16, true> : umi_median_kernel<16, false>; break;
-    case 32: k1 = mad ? umi_median_kernel<32, true> : umi_median_kernel<32, false>; break;
+    int threads = K1_THREADS;
+    switch (prm.NS) {
+    /* NS = 1024 runs 128 threads of 8 keys: every thread holds a walker (with 256 threads half of the CTA's warps idle through
+       the walk), 7 CTAs per SM instead of 6, three of the sort's exchanges in registers instead of two
+       (config 2: 0.584 -> 0.558 ms, config 5: 6.78 -> 6.27 ms per 20,000 stars); the longer sorts lose that way */
+    case 512: k1 = mad ? umi_median_kernel<2, 256, true> : umi_median_kernel<2, 256, false>; break;
+    case 1024: k1 = mad ? umi_median_kernel<8, 128, true> : umi_median_kernel<8, 128, false>; threads = 128; break;
+    case 2048: k1 = mad ? umi_median_kernel<8, 256, true> : umi_median_kernel<8, 256, false>; break;
+    case 4096: k1 = mad ? umi_median_kernel<16, 256, true> : umi_median_kernel<16, 256, false>; break;
+    case 8192: k1 = mad ? umi_median_kernel<32, 256, true> : umi_median_kernel<32, 256, false>; break;
     default: return cudaErrorInvalidValue;
     }
     if (smem + 1024 > 48 * 1024) {        /* static shared memory counts towards the 48 KiB default limit too */
         const cudaError_t e = cudaFuncSetAttribute(k1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (e != cudaSuccess) return e;
     }
-    k1<<<grid, K1_THREADS, smem, stream>>>(prm);
+    k1<<<grid, threads, smem, stream>>>(prm);
     return cudaGetLastError();
 }
 
