@@ -97,7 +97,7 @@ def test_static_scratch_calls_allocate_no_device_memory(umi):
     torch.cuda.synchronize()
     free_after, _ = torch.cuda.mem_get_info()
     assert torch.cuda.memory_reserved() == reserved_before                       # not through torch's allocator
-    assert free_after == free_before                                             # nor behind its back
+    assert free_after >= free_before                                             # nor behind its back (cudaMalloc would lower it)
     _same(o, umi.umi_detrend_gapped(td, fd, T0, DT, N, W))
 
 
