@@ -34,6 +34,9 @@
 #ifndef UMI_K1_RADIX
 #define UMI_K1_RADIX 0
 #endif
+#ifndef UMI_K1_TRANSPOSED_SCATTER
+#define UMI_K1_TRANSPOSED_SCATTER 1
+#endif
 
 namespace umi {
 
@@ -394,10 +397,30 @@ umi_median_kernel(MedianParams prm)
 
         if (pk) {
             __syncthreads();                                        /* every read of the exchange buffer (srt) is done */
+            /* A thread holds E consecutive ranks: written from there, the 8-byte entries of a warp's lanes lie 8 E bytes apart
+               (16-way bank conflicts at E = 8: a fifth of the kernel's shared-memory wavefronts).  So the sorted words take
+               one more trip through the exchange buffer (128-bit stores, chunks XOR-swizzled as in the sort) and come back
+               striped -- word j THREADS + tid to thread tid -- and consecutive lanes write consecutive entries
+               (config 2: 0.557 -> 0.537 ms, config 5: 6.27 -> 6.03 ms per 20,000 stars).  Not at E = 2 (2-way, two barriers more). */
+            constexpr bool STRIPED = UMI_K1_TRANSPOSED_SCATTER && (E % 4 == 0);
+            if constexpr (STRIPED) {
+                uint32_t* wbuf = reinterpret_cast<uint32_t*>(srt);
+                auto chunk = [](int c) { return (c & ~7) | ((c ^ (c >> 3)) & 7); };
 #pragma unroll
-            for (int e = 0; e < E; ++e) {
-                const int r = tid * E + e;
-                const uint32_t u = v[e] & (uint32_t)(NS - 1), d = v[e] >> LOG_NS;
+                for (int e = 0; e < E; e += 4)
+                    reinterpret_cast<uint4*>(wbuf)[chunk((tid * E + e) >> 2)] = make_uint4(v[e], v[e + 1], v[e + 2], v[e + 3]);
+                __syncthreads();
+#pragma unroll
+                for (int j = 0; j < E; ++j) {
+                    const int i = j * THREADS + tid;
+                    v[j] = wbuf[4 * chunk(i >> 2) + (i & 3)];
+                }
+                __syncthreads();                                    /* the words are in registers: srt may be overwritten */
+            }
+#pragma unroll
+            for (int j = 0; j < E; ++j) {
+                const int r = STRIPED ? j * THREADS + tid : tid * E + j;
+                const uint32_t u = v[j] & (uint32_t)(NS - 1), d = v[j] >> LOG_NS;
                 if (d != KSPAN) {
                     rank[u] = (uint16_t)r;
                     srt[r] = ((uint64_t)(kmin + d) << 32) | u;
