@@ -3,8 +3,8 @@
  *
  * CTA = one star x one tile of T consecutive positions.  The T windows of a tile
  * live inside one union of U = T + W - 1 = NS samples (NS a power of two).
- *   1. sort the 32-bit keys of the union ONCE per tile: bitonic network, E = NS/256 keys per
- *      thread -- strides < E in registers, strides < 32 E with warp shuffles, only the top three
+ *   1. sort the 32-bit keys of the union ONCE per tile: bitonic network, E = NS/THREADS keys per
+ *      thread (128 threads of 8 at NS = 1024, 256 threads beyond) -- strides < E in registers, strides < 32 E with warp shuffles, only the top three
  *      strides through shared memory; a compare-exchange is two VIMNMX.  What is sorted is
  *      (key - smallest key of the tile) << log2 NS | union index whenever that fits 32 bits (the
  *      keys of a tile normally span 2^17 .. 2^21 values): rank and index of every entry are then
