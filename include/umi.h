@@ -41,7 +41,10 @@
  *    one of smallest magnitude, so the 1e-5 bar on the trend holds relative to the
  *    position's own |median| (for a light curve: the local flux); samples of any finite
  *    magnitude (fill values, glitches, whole runs of them) cost the others no precision.  (max - min) * 16 * max(1, 1/alpha) over the
- *    valid samples of those positions' windows must be finite in fp32.
+ *    valid samples of those positions' windows must be finite in fp32.  Where the trend itself is a
+ *    cancellation (a series already brought to zero mean, flux - 1) a bar relative to |trend| is not
+ *    meaningful: the error there is bounded by 2e-6 of the typical |sample| of the window plus 1e-5 |trend|
+ *    (measured: 3.5e-7 of it).
  */
 #ifndef UMI_B200_H
 #define UMI_B200_H

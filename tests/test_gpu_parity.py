@@ -487,3 +487,25 @@ def test_key_span_at_the_limit_of_the_packed_sort(umi, W, log_ns):
     x = np.stack(rows)
     assert np.isfinite(x[~np.isnan(x)]).all()
     _both(umi, x, W)
+
+
+@pytest.mark.parametrize("W,S,N", [(25, 3, 6000), (217, 40, 1055), (361, 2, 3218), (361, 320, 2000), (1367, 3, 9000)])
+def test_zero_mean_series_are_bounded_relative_to_their_spread(umi, W, S, N):
+    # flux - 1: the trend crosses zero, so a bar relative to |trend| means nothing there; what fp32 promises (DESIGN.md 5.2,
+    # "fp32 tolerance"; include/umi.h, "supported dynamic range") is an error of <= 2e-6 of the typical |sample| + 1e-5 |trend|.
+    # Medians stay bit-exact (signs, values next to zero, -0.0).
+    x = lc.random_series(4400 + W, S, N, nan_frac=0.02, inf_frac=0.0)
+    x = (x - np.float32(1.0)).astype(np.float32)
+    x[0, 5:9] = np.float32(-0.0)
+    ref = orc.detrend(x, W)
+    parity.compare_median(_gpu(umi, x, W, n_iter=0), ref.median)
+    got = _gpu(umi, x, W).astype(np.float64)
+    want = ref.trend64
+    assert np.array_equal(np.isnan(got), np.isnan(want))
+    ok = ~np.isnan(want)
+    spread = float(np.nanmedian(np.abs(x)))
+    bound = 2e-6 * spread + 1e-5 * np.abs(want[ok])
+    err = np.abs(got[ok] - want[ok])
+    assert (err <= bound).all(), (err / bound).max()
+    if W <= 361:
+        assert (np.abs(want[ok]) < 1e-2 * spread).any()      # the case is real: some trends are ~0 against the spread
