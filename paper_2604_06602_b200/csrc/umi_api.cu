@@ -595,6 +595,6 @@ const char* umi_status_string(int status)
     }
 }
 
-int umi_version(void) { return 300; /* 0.3.0 */ }
+int umi_version(void) { return 400; /* 0.4.0: umi_detrend_gapped_static, UMI_ERR_TOO_LARGE */ }
 
 } /* extern "C" */
