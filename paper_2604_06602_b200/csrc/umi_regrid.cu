@@ -232,6 +232,217 @@ umi_regrid_segments_kernel(float* __restrict__ grid_flux, uint8_t* __restrict__ 
     }
 }
 
+/*
+ * The same with one CTA of SEGP_WARPS warps per row, for batches with too few rows to fill the GPU with one warp each
+ * (1,000 rows of 19,440 slots: 1,000 warps, each a chain of 608 dependent chunk steps, twice).  Warp p owns the p-th part of
+ * the row's chunks.  What a part does to the scan state depends on the state it receives only through its FIRST valid
+ * slot (does a segment start there?); everything else -- its last valid slot, its count, the last segment start strictly
+ * inside it -- is the part's own.  So: a summary pass per part, the summaries folded in order (at most SEGP_WARPS - 1 steps,
+ * every warp for itself), then the scan proper with the right state coming in.  The backward pass needs no summary pass of its
+ * own: a segment END strictly inside a part is the valid slot in front of a START strictly inside it, which the forward pass
+ * has just seen.  Results are identical to umi_regrid_segments_kernel (same records, same flags).
+ * Measured on config 2 (1,000 rows x 19,440 slots), whole F2-with-segments step over the base path: warp per row +0.72 ms;
+ * 8 warps per row +0.55 (104 registers), 8 / 4 CTAs per SM +0.49, 16 / 2 +0.47 (batch 4: 64 registers, no spills; batch 8
+ * spilled), 16 / 1 +0.54-0.57, 32 / 1 +0.53, 4 / 8 +0.51.
+ */
+#ifndef UMI_SEGP_WARPS
+#define UMI_SEGP_WARPS 16
+#endif
+#ifndef UMI_SEGP_MIN_CTAS
+#define UMI_SEGP_MIN_CTAS 2     /* 64 registers, nothing spilled with SEGP_BATCH = 4 */
+#endif
+constexpr int SEGP_WARPS = UMI_SEGP_WARPS;
+#ifndef UMI_SEGP_BATCH
+#define UMI_SEGP_BATCH 4
+#endif
+constexpr int SEGP_BATCH = UMI_SEGP_BATCH;          /* chunks whose loads are issued together */
+
+struct SegPart {                /* forward summary of a part; slots are 32-bit (n_grid <= 2^31 - 1) */
+    int fv, lv, nv;             /* first / last valid slot (-1: none), number of valid slots */
+    int ls, cnt_ls;             /* last segment start strictly inside the part (-1: none), valid slots from it to the part's end */
+    int e_low, tot_low;         /* backward: lowest segment end strictly inside the part (-1: none), size of the segment ending there */
+    int idx_lv;                 /* backward: index inside its segment of the part's last valid slot */
+};
+
+__global__ void __launch_bounds__(32 * SEGP_WARPS, UMI_SEGP_MIN_CTAS)
+umi_regrid_segments_cta_kernel(float* __restrict__ grid_flux, uint8_t* __restrict__ grid_cut, int2* __restrict__ scratch,
+                               int64_t n_stars, int64_t n_grid, int64_t break_slots, int64_t min_segment, int64_t edge_cut)
+{
+    __shared__ SegPart part[SEGP_WARPS];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned lt = (1u << lane) - 1u, le = lt | (1u << lane), gt = ~le;
+    const float qnan = __int_as_float(0x7FC00000);
+    const int64_t n_chunks = (n_grid + 31) / 32;
+    const int64_t cpp = (n_chunks + SEGP_WARPS - 1) / SEGP_WARPS;          /* chunks per part */
+    const int64_t c_lo = warp * cpp, c_hi = (c_lo + cpp < n_chunks) ? c_lo + cpp : n_chunks;   /* my chunks [c_lo, c_hi) */
+    for (int64_t b = blockIdx.x; b < n_stars; b += gridDim.x) {
+        float* frow = grid_flux + b * n_grid;
+        uint8_t* crow = grid_cut + b * n_grid;
+        int2* srow = scratch + b * n_grid;
+        /* 1. summary of my part (valid bits only; starts strictly inside: both slots of the gap are mine) */
+        {
+            int fv = -1, lv = -1, nv = 0, ls = -1, cnt_ls = 0;
+            for (int64_t c0 = c_lo; c0 < c_hi; c0 += SEGP_BATCH) {
+                bool vld[SEGP_BATCH];
+#pragma unroll
+                for (int c = 0; c < SEGP_BATCH; ++c) {
+                    const int64_t k = (c0 + c) * 32 + lane;
+                    vld[c] = c0 + c < c_hi && k < n_grid && finite_f32(__ldcg(frow + k));
+                }
+#pragma unroll
+                for (int c = 0; c < SEGP_BATCH; ++c) {
+                    if (c0 + c >= c_hi) break;
+                    const int base = (int)((c0 + c) * 32);
+                    const unsigned vb = __ballot_sync(0xFFFFFFFFu, vld[c]);
+                    if (vb == 0u) continue;
+                    const int p = 31 - __clz((int)(vb & lt));
+                    const int ps = p >= 0 ? base + p : lv;                          /* previous valid slot inside the part, -1: none */
+                    const bool start = vld[c] && ps >= 0 && break_slots >= 0 && (int64_t)(base + lane) - ps - 1 > break_slots;
+                    const unsigned sb = __ballot_sync(0xFFFFFFFFu, start);
+                    if (fv < 0) fv = base + __ffs((int)vb) - 1;
+                    lv = base + 31 - __clz((int)vb);
+                    nv += __popc(vb);
+                    if (sb) { const int l2 = 31 - __clz((int)sb); ls = base + l2; cnt_ls = __popc(vb & ~((1u << l2) - 1u)); }
+                    else cnt_ls += __popc(vb);
+                }
+            }
+            if (lane == 0) { part[warp].fv = fv; part[warp].lv = lv; part[warp].nv = nv; part[warp].ls = ls; part[warp].cnt_ls = cnt_ls; }
+        }
+        __syncthreads();
+        /* 2. the state my part receives: parts 0 .. warp-1 folded in order */
+        bool have_prev = false;
+        int64_t prev_slot = 0, cur_first = 0, cur_cnt = 0;
+        for (int q = 0; q < warp; ++q) {
+            const SegPart s = part[q];
+            if (s.nv == 0) continue;
+            const bool bstart = !have_prev || (break_slots >= 0 && (int64_t)s.fv - prev_slot - 1 > break_slots);
+            if (s.ls >= 0) { cur_first = s.ls; cur_cnt = s.cnt_ls; }
+            else if (bstart) { cur_first = s.fv; cur_cnt = s.nv; }
+            else cur_cnt += s.nv;
+            prev_slot = s.lv;
+            have_prev = true;
+        }
+        /* 3. forward over my part: (first slot of the segment, index inside it) of every valid slot; on the way, the lowest
+              segment end strictly inside the part (the valid slot in front of the first start strictly inside it) */
+        {
+            int e_low = -1, tot_low = 0, idx_lv = 0;
+            int own_prev = -1, own_prev_idx = 0;                                    /* my part's previous valid slot and its index */
+            for (int64_t c0 = c_lo; c0 < c_hi; c0 += SEGP_BATCH) {
+                bool vld[SEGP_BATCH];
+#pragma unroll
+                for (int c = 0; c < SEGP_BATCH; ++c) {
+                    const int64_t k = (c0 + c) * 32 + lane;
+                    vld[c] = c0 + c < c_hi && k < n_grid && finite_f32(__ldcg(frow + k));
+                }
+#pragma unroll
+                for (int c = 0; c < SEGP_BATCH; ++c) {
+                    if (c0 + c >= c_hi) break;
+                    const int64_t base = (c0 + c) * 32;
+                    const int64_t k = base + lane;
+                    const bool valid = vld[c];
+                    const unsigned vb = __ballot_sync(0xFFFFFFFFu, valid);
+                    const int p = 31 - __clz((int)(vb & lt));
+                    const bool none = p < 0 && !have_prev;
+                    const int64_t ps = p >= 0 ? base + p : prev_slot;
+                    const bool start = valid && (none || (break_slots >= 0 && k - ps - 1 > break_slots));
+                    const unsigned sb = __ballot_sync(0xFFFFFFFFu, start);
+                    int my_idx = 0;
+                    if (valid) {
+                        const int st = 31 - __clz((int)(sb & le));
+                        int2 rec;
+                        if (st >= 0) { rec.x = (int)(base + st); rec.y = __popc(vb & le & ~((1u << st) - 1u)) - 1; }
+                        else { rec.x = (int)cur_first; rec.y = (int)cur_cnt + __popc(vb & lt); }
+                        srow[k] = rec;
+                        my_idx = rec.y;
+                    }
+                    if (vb) {
+                        /* the first start strictly inside the part: its previous valid slot is mine (own_prev, or a lane of this chunk) */
+                        if (e_low < 0 && sb) {
+                            unsigned cand = sb;
+                            if (own_prev < 0) cand &= ~(1u << (__ffs((int)vb) - 1));     /* the part's very first valid slot: its predecessor is not mine */
+                            if (cand) {
+                                const int sl = __ffs((int)cand) - 1;                /* lane of that start */
+                                const unsigned below = vb & ((1u << sl) - 1u);
+                                if (below) {
+                                    const int pl = 31 - __clz((int)below);
+                                    e_low = (int)base + pl;
+                                    tot_low = __shfl_sync(0xFFFFFFFFu, my_idx, pl) + 1;
+                                } else {
+                                    e_low = own_prev;
+                                    tot_low = own_prev_idx + 1;
+                                }
+                            }
+                        }
+                        const int hl = 31 - __clz((int)vb);
+                        own_prev = (int)base + hl;
+                        own_prev_idx = __shfl_sync(0xFFFFFFFFu, my_idx, hl);
+                        idx_lv = own_prev_idx;
+                        prev_slot = base + hl;
+                        have_prev = true;
+                    }
+                    if (sb) { const int l2 = 31 - __clz((int)sb); cur_first = base + l2; cur_cnt = __popc(vb & ~((1u << l2) - 1u)); }
+                    else cur_cnt += __popc(vb);
+                }
+            }
+            if (lane == 0) { part[warp].e_low = e_low; part[warp].tot_low = tot_low; part[warp].idx_lv = idx_lv; }
+        }
+        __syncthreads();                                            /* records and summaries are complete */
+        /* 4. the state my part receives going backward: parts SEGP_WARPS-1 .. warp+1 folded in order */
+        bool have_next = false;
+        int64_t next_slot = 0, cur_last = 0, cur_total = 0;
+        for (int q = SEGP_WARPS - 1; q > warp; --q) {
+            const SegPart s = part[q];
+            if (s.nv == 0) continue;
+            const bool bend = !have_next || (break_slots >= 0 && next_slot - (int64_t)s.lv - 1 > break_slots);
+            if (s.e_low >= 0) { cur_last = s.e_low; cur_total = s.tot_low; }
+            else if (bend) { cur_last = s.lv; cur_total = (int64_t)s.idx_lv + 1; }
+            next_slot = s.fv;
+            have_next = true;
+        }
+        /* 5. backward over my part: (last slot, size) of the segment; short segments erased, edges marked */
+        for (int64_t c0 = c_hi - 1; c0 >= c_lo; c0 -= SEGP_BATCH) {
+            bool vld[SEGP_BATCH];
+            int2 recs[SEGP_BATCH];
+#pragma unroll
+            for (int c = 0; c < SEGP_BATCH; ++c) {
+                const int64_t k = (c0 - c) * 32 + lane;
+                vld[c] = c0 - c >= c_lo && k < n_grid && finite_f32(frow[k]);
+                recs[c] = vld[c] ? srow[k] : make_int2(0, 0);
+            }
+#pragma unroll
+            for (int c = 0; c < SEGP_BATCH; ++c) {
+                if (c0 - c < c_lo) break;
+                const int64_t base = (c0 - c) * 32;
+                const int64_t k = base + lane;
+                const bool valid = vld[c];
+                const int2 rec = recs[c];
+                const unsigned vb = __ballot_sync(0xFFFFFFFFu, valid);
+                const int nx = __ffs((int)(vb & gt)) - 1;
+                const bool none = nx < 0 && !have_next;
+                const int64_t ns = nx >= 0 ? base + nx : next_slot;
+                const bool end = valid && (none || (break_slots >= 0 && ns - k - 1 > break_slots));
+                const unsigned eb = __ballot_sync(0xFFFFFFFFu, end);
+                const int en = __ffs((int)(eb & ~lt)) - 1;
+                const int idx_at_end = __shfl_sync(0xFFFFFFFFu, rec.y, en >= 0 ? en : 0);
+                const int64_t last = en >= 0 ? base + en : cur_last;
+                const int64_t total = en >= 0 ? (int64_t)idx_at_end + 1 : cur_total;
+                if (k < n_grid) {
+                    const bool drop = valid && min_segment > 0 && total < min_segment;
+                    if (drop) frow[k] = qnan;
+                    crow[k] = (valid && !drop && edge_cut > 0 && (k - rec.x < edge_cut || last - k < edge_cut)) ? 1 : 0;
+                }
+                if (vb) { next_slot = base + __ffs((int)vb) - 1; have_next = true; }
+                if (eb) {
+                    const int fe = __ffs((int)eb) - 1;
+                    cur_last = base + fe;
+                    cur_total = (int64_t)__shfl_sync(0xFFFFFFFFu, rec.y, fe) + 1;
+                }
+            }
+        }
+        __syncthreads();                                            /* part[] is free for the next row */
+    }
+}
+
 dim3 regrid_grid(int64_t n_stars, int64_t M)
 {
     int64_t bx = (M + RG_THREADS * RG_ITEMS - 1) / (RG_THREADS * RG_ITEMS);
@@ -261,6 +472,15 @@ cudaError_t launch_regrid_gather(const RegridParams& prm, const float* grid_tren
 cudaError_t launch_regrid_segments(float* grid_flux, uint8_t* grid_cut, void* scratch, int64_t n_stars, int64_t n_grid,
                                    int64_t break_slots, int64_t min_segment, int64_t edge_cut, cudaStream_t stream)
 {
+    /* rows enough to fill the GPU with a warp each (64 warps x ~150 SMs): one warp per row; fewer: a CTA per row */
+#ifndef UMI_SEG_CTA_BELOW
+#define UMI_SEG_CTA_BELOW 4096
+#endif
+    if (n_stars < UMI_SEG_CTA_BELOW) {
+        umi_regrid_segments_cta_kernel<<<(unsigned)n_stars, 32 * SEGP_WARPS, 0, stream>>>(grid_flux, grid_cut, static_cast<int2*>(scratch),
+                                                                                            n_stars, n_grid, break_slots, min_segment, edge_cut);
+        return cudaGetLastError();
+    }
     int64_t ctas = (n_stars + 3) / 4;
     if (ctas > 0x7FFFFFFF) ctas = 0x7FFFFFFF;
     umi_regrid_segments_kernel<<<(unsigned)ctas, 128, 0, stream>>>(grid_flux, grid_cut, static_cast<int2*>(scratch), n_stars,

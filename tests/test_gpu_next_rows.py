@@ -321,3 +321,44 @@ def test_hundred_random_cases_of_the_next_rows(umi):
         else:
             parity.compare_trend(trend.cpu().numpy(), ref)
         _check_flat(flat.cpu().numpy(), f, ref)
+
+
+def test_gapped_segments_rows_that_leave_whole_parts_empty(umi):
+    # The segment scan of small batches runs one CTA per row, every warp one part of the row (umi_regrid.cu): rows whose
+    # valid slots sit in one part only, at the part seams, nowhere, or everywhere; breaks exactly at / next to the limit.
+    import torch
+    dt, N, W = 0.01, 8000, 25                               # 250 chunks of 32 slots: parts of 32 chunks = 1024 slots
+    rng = np.random.default_rng(5)
+    grid = np.full((10, N), np.nan, np.float32)
+    val = (1.0 + 1e-3 * rng.standard_normal(N)).astype(np.float32)
+    grid[1, 4000] = val[4000]                               # one valid slot
+    grid[2, 0] = val[0]; grid[2, N - 1] = val[N - 1]        # the two ends of the row
+    grid[3, 1000:1048] = val[1000:1048]                     # across the seam of parts 0 and 1 (slot 1024)
+    grid[4, 900:1024] = val[900:1024]; grid[4, 1024 + 13:1200] = val[1024 + 13:1200]     # a break of 13 empty slots exactly at a seam
+    grid[5, 900:1024] = val[900:1024]; grid[5, 1024 + 12:1200] = val[1024 + 12:1200]     # 12: not a break
+    grid[6] = val                                           # one segment over all parts
+    grid[7, 100:300] = val[100:300]; grid[7, 7000:7300] = val[7000:7300]                 # parts 1 .. 5 empty
+    grid[8] = val; grid[8, 1023::1024] = np.nan; grid[8, 2040:2060] = np.nan             # holes at the seams, a break next to one
+    grid[9, ::40] = val[::40]                               # every valid slot a segment of its own (gaps of 39 > 12)
+    t, f, slot = lc.compact(grid, dt, t0=3.5, jitter=0.0, seed=1)
+    for brk, mseg, ecut in ((12, 0, 0), (12, 30, 4), (40, 2, 1), (-1, 0, 10)):
+        ref = orc.gapped_ex(t, f, 3.5, dt, N, W, break_slots=brk, min_segment=mseg, edge_cut=ecut)
+        got = umi.umi_detrend_gapped(_cuda(t, np.float64), _cuda(f, np.float32), 3.5, dt, N, W,
+                                     break_slots=brk, min_segment=mseg, edge_cut=ecut)
+        torch.cuda.synchronize()
+        parity.compare_trend(got.cpu().numpy(), ref)
+
+
+def test_gapped_segments_warp_per_row_and_cta_per_row_scans_agree(umi):
+    # 4,200 rows take the warp-per-row scan, the same rows 100 at a time the CTA-per-row scan: identical results, and the oracle's
+    import torch
+    dt, N, W = 2.0 / 1440, 1301, 25
+    t, f, slot = _segment_rows(77, 4200, N, dt)
+    kw = dict(break_slots=12, min_segment=12, edge_cut=3)
+    td, fd = _cuda(t, np.float64), _cuda(f, np.float32)
+    big = umi.umi_detrend_gapped(td, fd, 7.25, dt, N, W, **kw).cpu().numpy()
+    for a in (0, 2100, 4100):
+        small = umi.umi_detrend_gapped(td[a:a + 100].contiguous(), fd[a:a + 100].contiguous(), 7.25, dt, N, W, **kw).cpu().numpy()
+        np.testing.assert_array_equal(small, big[a:a + 100])
+    ref = orc.gapped_ex(t[:150], f[:150], 7.25, dt, N, W, **kw)
+    parity.compare_trend(big[:150], ref)
