@@ -18,23 +18,30 @@ constexpr int K1_THREADS = UMI_K1_THREADS;       /* median kernel (128 for the 1
 #endif
 constexpr int K1_MIN_SORT = UMI_K1_MIN_SORT;     /* smallest per-tile sort length */
 /* walkers per tile of the median kernel, per sort length, and its dynamic shared memory (bytes).  Measured:
-   512 keys (small batches): one walker per position pair; 1024: every one of the CTA's 128 threads; beyond that as many as
-   leave the CTAs per SM of k1_min_ctas (umi_median.cu) their shared memory -- a multiple of 32, not necessarily a power of two */
+   512 keys (small batches): one walker per position pair; 1024: three of the CTA's four warps; beyond that as many as
+   leave the CTAs per SM of k1_min_ctas (umi_median.cu) their shared memory -- a multiple of 32, not necessarily a power of two.
+   The MAD build stages one more fp32 per position: at 8192 keys it has room for 64 walkers only. */
 #ifndef UMI_K1_WALKERS
-#define UMI_K1_WALKERS(ns) ((ns) <= 512 ? 256 : (ns) == 1024 ? 128 : (ns) == 2048 ? 96 : (ns) == 4096 ? 96 : 64)
+#define UMI_K1_WALKERS(ns) ((ns) <= 512 ? 256 : 96)
 #endif
-__host__ __device__ constexpr int k1_walkers(int ns) { return UMI_K1_WALKERS(ns); }
-/* t = positions per tile (T = ns - W + 1; 0: the worst case ns) */
-__host__ __device__ constexpr size_t k1_smem_bytes(int ns, bool mad = false, int t = 0)
+__host__ __device__ constexpr int k1_walkers(int ns, bool mad = false)
 {
-    /* u64 sorted entries + u16 ranks + max(rank bitsets [NW][NS/32+1] + scan offsets [NW/32][NS/32], f32 medians)
-       + u32 sorted keys, one pad word per 32 */
-    const size_t bw = (size_t)ns / 32, nw = (size_t)k1_walkers(ns);
+    return (mad && ns >= 8192) ? 64 : ((mad && UMI_K1_WALKERS(ns) > 128) ? 128 : UMI_K1_WALKERS(ns));
+}
+/* t = positions per tile (T = ns - W + 1; 0: the worst case ns).  Layout: u64 sorted entries + u16 ranks + max(rank bitsets
+   [NW][NS/32+1] + scan offsets [NW/32][NS/32], staging of the tile's results) + u32 sorted keys, one pad word per 32
+   (k1_smem_base: the MAD build's scales start there) + in the MAD build one fp32 per position */
+__host__ __device__ constexpr size_t k1_smem_base(int ns, bool mad, int t)
+{
+    const size_t bw = (size_t)ns / 32, nw = (size_t)k1_walkers(ns, mad);
     const size_t bits = 4 * (nw * (bw + 1) + (nw / 32) * bw);
     /* f32 medians [T], then u16 median ranks [T] and u16 window counts [T] (for n+ and the packed hand-over), rounded to 16 bytes */
     const size_t med = ((8 * (size_t)(t > 0 ? t : ns)) + 15) / 16 * 16;
-    /* the MAD variant stages one more fp32 per position (the scale) behind everything else */
-    return (size_t)ns * 10 + (bits > med ? bits : med) + 4 * ((size_t)ns + (size_t)ns / 32) + (mad ? 4 * (size_t)ns : 0);
+    return (size_t)ns * 10 + (bits > med ? bits : med) + 4 * ((size_t)ns + (size_t)ns / 32);
+}
+__host__ __device__ constexpr size_t k1_smem_bytes(int ns, bool mad = false, int t = 0)
+{
+    return k1_smem_base(ns, mad, t) + (mad ? 4 * (size_t)ns : 0);
 }
 
 /* sibling estimators; values match include/umi.h */

@@ -34,6 +34,9 @@
 #ifndef UMI_K1_RADIX
 #define UMI_K1_RADIX 0
 #endif
+#ifndef UMI_K1_BITWALK
+#define UMI_K1_BITWALK 1
+#endif
 #ifndef UMI_K1_TRANSPOSED_SCATTER
 #define UMI_K1_TRANSPOSED_SCATTER 1
 #endif
@@ -196,26 +199,26 @@ __global__ void __launch_bounds__(THREADS, k1_min_ctas(THREADS * E))
 umi_median_kernel(MedianParams prm)
 {
     constexpr int NS = THREADS * E;
+    constexpr bool BITWALK = MAD || UMI_K1_BITWALK;                 /* walkers keep their rank bitsets current through the walk */
     constexpr int BW = NS / 32;                                     /* bitset words per walker */
     constexpr int BWP = BW + 1;                                     /* padded row stride: conflict-free both ways */
-#ifndef UMI_K1_MAD_WALKERS
-#define UMI_K1_MAD_WALKERS 128
-#endif
-    /* walkers per tile: the MAD variant keeps the same count (with the member-by-member set-up of the range,
-       32 / 64 / 128 walkers measured 20.4 / 18.3 / 18.1 ms per config-2 step: fewer, longer walks lose more in
-       parallelism than they save in set-up; the set-up itself is now word-by-word from the bitset) */
-    constexpr int NW = MAD ? (UMI_K1_MAD_WALKERS < k1_walkers(NS) ? UMI_K1_MAD_WALKERS : k1_walkers(NS)) : k1_walkers(NS);
+    /* walkers per tile (umi_internal.h) */
+    constexpr int NW = k1_walkers(NS, MAD);
     constexpr int NWB = NW / 32;                                    /* walker blocks of 32 */
     extern __shared__ __align__(16) unsigned char smem_raw[];
     uint64_t* srt = reinterpret_cast<uint64_t*>(smem_raw);          /* [NS] key<<32 | union index, sorted */
     uint16_t* rank = reinterpret_cast<uint16_t*>(srt + NS);         /* [NS] union index -> rank           */
     uint32_t* bits = reinterpret_cast<uint32_t*>(rank + NS);        /* [NW][BWP] rank bitsets, then ...   */
     uint32_t* boff = bits + NW * BWP;                               /* [NWB][BW] block offsets of the scan */
-    float* medbuf = reinterpret_cast<float*>(bits);                 /* ... aliased: [T] medians of the tile */
-    uint16_t* rhobuf = reinterpret_cast<uint16_t*>(medbuf + prm.T); /* ... [T] median ranks and [T] window counts behind them */
+    uint32_t* skey = reinterpret_cast<uint32_t*>(smem_raw + k1_smem_base(NS, MAD, prm.T)) - (NS + NS / 32);   /* [NS + NS/32] sorted keys, padded (skey_at) */
+    /* [T] medians of the tile: aliased onto the bitsets, which are dead by then -- except in the MAD build, whose walkers keep
+       their bitsets up to date through the walk (below) and stage the medians in the sorted-key area instead (free after the ranks) */
+    float* medbuf = BITWALK ? reinterpret_cast<float*>(skey) : reinterpret_cast<float*>(bits);
+    /* ... [T] median ranks and [T] window counts behind them (a launch stages either medians or these: in the sorted-key area,
+       which holds 4 T bytes but not 8 T, they take the medians' place) */
+    uint16_t* rhobuf = BITWALK ? reinterpret_cast<uint16_t*>(medbuf) : reinterpret_cast<uint16_t*>(medbuf + prm.T);
     uint16_t* cntbuf = rhobuf + prm.T;
-    uint32_t* skey = reinterpret_cast<uint32_t*>(smem_raw + k1_smem_bytes(NS, false, prm.T)) - (NS + NS / 32);   /* [NS + NS/32] sorted keys, padded (skey_at) */
-    float* sclbuf = reinterpret_cast<float*>(smem_raw + k1_smem_bytes(NS, false, prm.T));   /* MAD only: [T] scales */
+    float* sclbuf = reinterpret_cast<float*>(smem_raw + k1_smem_base(NS, MAD, prm.T));   /* MAD only: [T] scales */
     __shared__ int s_nvu;
     __shared__ uint32_t s_kmin, s_kmax;                             /* radix path: range of the tile's valid keys */
 #if UMI_K1_RADIX
@@ -525,14 +528,20 @@ umi_median_kernel(MedianParams prm)
         int n = 0, rho = -1;
         MadRange mr = {0, 0, 0};
         if (tid < nwa) {
-            const uint32_t* row = bits + tid * BWP;
+            uint32_t* row = bits + tid * BWP;
             const uint32_t* off = boff + (tid >> 5) * BW;
+            if constexpr (BITWALK) {                                /* the bitset proper, in place: the walk keeps it current */
 #pragma unroll 4
-            for (int i = 0; i < BW; ++i) n += __popc(row[i] ^ off[i]);
+                for (int i = 0; i < BW; ++i) { const uint32_t w0 = row[i] ^ off[i]; row[i] = w0; n += __popc(w0); }
+            } else {
+#pragma unroll 4
+                for (int i = 0; i < BW; ++i) n += __popc(row[i] ^ off[i]);
+            }
+            auto wd = [&](int i) { return BITWALK ? row[i] : (row[i] ^ off[i]); };      /* word i of my bitset */
             if (n > 0) {
                 int need = (n - 1) >> 1;                            /* (R6) lower median */
                 for (int i = 0; i < BW; ++i) {
-                    const uint32_t word = row[i] ^ off[i];
+                    const uint32_t word = wd(i);
                     const int pc = __popc(word);
                     if (need < pc) {
                         rho = i * 32 + (int)__fns(word, 0, need + 1);
@@ -548,7 +557,7 @@ umi_median_kernel(MedianParams prm)
                     const int target = ((n - 1) >> 1) + 1;
                     const float med = key_to_float((uint32_t)(srt[rho] >> 32));
                     int wl = rho >> 5, wr = wl;
-                    int cnt = __popc(row[wl] ^ off[wl]);
+                    int cnt = __popc(wd(wl));
                     const int wmax = (nvu - 1) >> 5;
                     while (cnt < target) {
                         const bool can_l = wl > 0, can_r = wr < wmax;
@@ -559,18 +568,18 @@ umi_median_kernel(MedianParams prm)
                             const float dr = key_to_float((uint32_t)(srt[32 * (wr + 1)] >> 32)) - med;
                             left = dl <= dr;
                         }
-                        if (left) { --wl; cnt += __popc(row[wl] ^ off[wl]); }
-                        else      { ++wr; cnt += __popc(row[wr] ^ off[wr]); }
+                        if (left) { --wl; cnt += __popc(wd(wl)); }
+                        else      { ++wr; cnt += __popc(wd(wr)); }
                     }
-                    while ((row[wl] ^ off[wl]) == 0u) ++wl;             /* rho's word is inside: both loops stop */
-                    while ((row[wr] ^ off[wr]) == 0u) --wr;
-                    mr.L = 32 * wl + __ffs((int)(row[wl] ^ off[wl])) - 1;
-                    mr.R = 32 * wr + 31 - __clz((int)(row[wr] ^ off[wr]));
+                    while ((wd(wl)) == 0u) ++wl;             /* rho's word is inside: both loops stop */
+                    while ((wd(wr)) == 0u) --wr;
+                    mr.L = 32 * wl + __ffs((int)(wd(wl))) - 1;
+                    mr.R = 32 * wr + 31 - __clz((int)(wd(wr)));
                     mr.cnt = cnt;
                 }
             }
         }
-        __syncthreads();                                            /* bitsets are dead: medbuf reuses them */
+        __syncthreads();                                            /* bitsets are dead: medbuf reuses them (MAD build: they live on, medbuf is elsewhere) */
 
         /* 3. walk: a slide removes one entry and adds one */
         if (tid < nwa) {
@@ -582,13 +591,39 @@ umi_median_kernel(MedianParams prm)
             float mad = 0.f;
             /* window members next to rank r, under the window of position q */
             auto val = [&](int r) { return key_to_float((uint32_t)(srt[r] >> 32)); };
+            /* MAD build: every slide repairs both ends of the range, several neighbour searches each, so the walker keeps its
+               rank bitset current (one bit cleared, one set per slide) and finds the next member with a mask and a count of
+               leading / trailing zeros instead of stepping over the ~U/W non-members in between one entry at a time */
+            uint32_t* mrow = bits + tid * BWP;
             auto nextm = [&](int r, int q) {
-                do { ++r; } while (r < nvu && ((uint32_t)srt[r] - (uint32_t)q) >= uW);
-                return r;
+                if constexpr (BITWALK) {
+                    int w = (r + 1) >> 5;
+                    if (w >= BW) return nvu;
+                    uint32_t m = mrow[w] & (0xFFFFFFFFu << ((r + 1) & 31));
+                    while (m == 0u) {
+                        if (++w >= BW) return nvu;
+                        m = mrow[w];
+                    }
+                    return (w << 5) + __ffs((int)m) - 1;
+                } else {
+                    do { ++r; } while (r < nvu && ((uint32_t)srt[r] - (uint32_t)q) >= uW);
+                    return r;
+                }
             };
             auto prevm = [&](int r, int q) {
-                do { --r; } while (r >= 0 && ((uint32_t)srt[r] - (uint32_t)q) >= uW);
-                return r;
+                if constexpr (BITWALK) {
+                    if (r <= 0) return -1;
+                    int w = (r - 1) >> 5;
+                    uint32_t m = mrow[w] & (0xFFFFFFFFu >> (31 - ((r - 1) & 31)));
+                    while (m == 0u) {
+                        if (--w < 0) return -1;
+                        m = mrow[w];
+                    }
+                    return (w << 5) + 31 - __clz((int)m);
+                } else {
+                    do { --r; } while (r >= 0 && ((uint32_t)srt[r] - (uint32_t)q) >= uW);
+                    return r;
+                }
             };
             /* restore the invariant for window q (median rank rho, n members) and return the MAD */
             auto mad_fix = [&](int q) {
@@ -642,6 +677,10 @@ umi_median_kernel(MedianParams prm)
                 const int ro = rank[p - 1], ri = rank[p + W - 1];
                 const bool vo = ro < nvu, vi = ri < nvu;
                 const int n2 = n - (vo ? 1 : 0) + (vi ? 1 : 0);
+                if constexpr (BITWALK) {                            /* my bitset becomes that of window p */
+                    if (vo) mrow[ro >> 5] &= ~(1u << (ro & 31));
+                    if (vi) mrow[ri >> 5] |= 1u << (ri & 31);
+                }
                 if (n2 == 0) {
                     rho = -1;
                 } else if (n == 0) {
@@ -650,6 +689,19 @@ umi_median_kernel(MedianParams prm)
                     const int k2 = (n2 - 1) >> 1;
                     int below = ((n - 1) >> 1) - ((vo && ro < rho) ? 1 : 0) + ((vi && ri < rho) ? 1 : 0);
                     const uint32_t up = (uint32_t)p;
+                    if constexpr (BITWALK) {                        /* the same moves on the bitset */
+                        if (vo && ro == rho) {
+                            const int r = nextm(rho, p);
+                            if (r < nvu) {
+                                rho = r;
+                            } else {
+                                rho = max(prevm(rho, p), 0);
+                                --below;
+                            }
+                        }
+                        while (below > k2) { rho = max(prevm(rho, p), 0); --below; }
+                        while (below < k2) { rho = min(nextm(rho, p), nvu - 1); ++below; }
+                    } else {
                     if (vo && ro == rho) {                          /* the median itself left */
                         int r = rho + 1;
                         while (r < nvu && ((uint32_t)srt[r] - up) >= uW) ++r;
@@ -673,6 +725,7 @@ umi_median_kernel(MedianParams prm)
                         while (r < nvu - 1 && ((uint32_t)srt[r] - up) >= uW) ++r;
                         rho = r;
                         ++below;
+                    }
                     }
                 }
                 n = n2;
