@@ -192,7 +192,7 @@ struct MadRange {
 };
 
 /* CTAs per SM the registers must allow, per sort length: what the shared memory of that length admits (k1_smem_bytes) */
-__host__ __device__ constexpr int k1_min_ctas(int ns) { return ns <= 512 ? 6 : ns == 1024 ? 7 : ns == 2048 ? 4 : ns == 4096 ? 2 : 1; }
+__host__ __device__ constexpr int k1_min_ctas(int ns) { return ns <= 512 ? 6 : ns == 1024 ? 8 : ns == 2048 ? 4 : ns == 4096 ? 2 : 1; }
 
 template <int E, int THREADS, bool MAD>
 __global__ void __launch_bounds__(THREADS, k1_min_ctas(THREADS * E))
@@ -790,8 +790,8 @@ cudaError_t launch_median(const MedianParams& prm, unsigned grid, size_t smem, c
     const bool mad = prm.scale != nullptr;
     int threads = K1_THREADS;
     switch (prm.NS) {
-    /* NS = 1024 runs 128 threads of 8 keys: every thread holds a walker (with 256 threads half of the CTA's warps idle through
-       the walk), 7 CTAs per SM instead of 6, three of the sort's exchanges in registers instead of two
+    /* NS = 1024 runs 128 threads of 8 keys: three of the four warps hold walkers (with 256 threads half of the CTA's warps idle
+       through the walk), 8 CTAs per SM instead of 6, three of the sort's exchanges in registers instead of two
        (config 2: 0.584 -> 0.558 ms, config 5: 6.78 -> 6.27 ms per 20,000 stars); the longer sorts lose that way */
     case 512: k1 = mad ? umi_median_kernel<2, 256, true> : umi_median_kernel<2, 256, false>; break;
     case 1024: k1 = mad ? umi_median_kernel<8, 128, true> : umi_median_kernel<8, 128, false>; threads = 128; break;
